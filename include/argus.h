@@ -1,0 +1,210 @@
+/* argus.h — C ABI of libargus.so: the B200 (sm_100a) hot path of ARGUS
+ * (arxiv/paper_2606_20374): kernel-event reduction + cross-rank diagnosis.
+ *
+ * Citations: "PAPER.md:<line>" is /root/reference/PAPER.md; "NS" is the north_star text of
+ * BASELINE.json, which fixes record layouts, the summary contents and the detection rule;
+ * "R<n>" is reading n of DESIGN.md §3 (where the paper and NS are silent).
+ *
+ * This header holds POD layouts and prototypes only: no inline logic.  Every pointer argument is
+ * tagged [host] or [device].  Device pointers are plain CUDA global-memory addresses owned by the
+ * caller (e.g. torch uint8 tensors); the library borrows them until the work queued on the given
+ * stream has completed and never frees them.  `stream` arguments are a `cudaStream_t` passed as
+ * `void*` (0 = the legacy default stream).  All functions return ARGUS_OK (0) or a negative
+ * ARGUS_E* code; none throws.  Calls on one ctx are not thread-safe.  There is no CPU fallback:
+ * without a CUDA device argus_create fails with ARGUS_ECUDA.
+ */
+#ifndef ARGUS_H_
+#define ARGUS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes -------------------------------------------------------------------------- */
+#define ARGUS_OK       0
+#define ARGUS_EINVAL  -1  /* null / misaligned pointer, zero or out-of-range dimension          */
+#define ARGUS_ECUDA   -2  /* a CUDA call failed; see argus_last_cuda_error                      */
+#define ARGUS_ESIZE   -3  /* n too large for one call, or dims beyond what the kernels support  */
+#define ARGUS_ESTATE  -4  /* call order violated (e.g. aggregate on records that were not reset) */
+#define ARGUS_ENOMEM  -5  /* host or device allocation of ctx workspace failed                  */
+
+/* ---- config flags ------------------------------------------------------------------------- */
+/* Performance hint (R18): records arrive grouped by (rank, step) — the segmented kernel is used.
+ * Results never depend on the hint; a violated hint only costs time. */
+#define ARGUS_FLAG_SORTED 0x1u
+
+/* ---- limits ------------------------------------------------------------------------------- */
+#define ARGUS_HIST_BUCKETS 32
+#define ARGUS_MAX_PHASES   64     /* n_phases <= 64                                              */
+#define ARGUS_MAX_RANKS    16384  /* n_ranks  <= 16384 (selection holds one series per CTA)      */
+
+/* ---- flag values written by argus_diagnose (R14) ------------------------------------------ */
+#define ARGUS_FLAG_NONE 0
+#define ARGUS_FLAG_HIGH 1  /* x > median and |x - median| > 3*MAD */
+#define ARGUS_FLAG_LOW  2  /* x < median and |x - median| > 3*MAD */
+
+/* Raw kernel event (NS: "32-byte record {u32 rank, u32 step, u32 sig, u16 stream, u16 phase,
+ * i64 start_ns, i64 end_ns}"; the paper's CUPTI activity record — name, launch time, duration,
+ * stream — PAPER.md:104, 142).  Little-endian, naturally aligned, no padding (R1). */
+typedef struct argus_event {
+  uint32_t rank;
+  uint32_t step;
+  uint32_t sig;      /* interned kernel signature */
+  uint16_t stream;   /* carried, not part of the key (R16), not validated (R3) */
+  uint16_t phase;
+  int64_t  start_ns;
+  int64_t  end_ns;
+} argus_event;       /* 32 B */
+
+/* Per-(rank, step, sig) summary (NS: "count, u64 sum, min and max of duration, and a 32-bucket
+ * log2 duration histogram"; stands where the paper keeps per-cluster (count, p50, p99) triples on
+ * a log-duration grid).  Empty cell = reduction identities (R7):
+ * count 0, sum 0, min UINT64_MAX, max 0, hist 0.
+ * bucket(d) = d==0 ? 0 : min(31, floor(log2 d))  (R4). */
+typedef struct argus_cell {
+  uint64_t count;
+  uint64_t sum_ns;   /* wraps mod 2^64 (R6) */
+  uint64_t min_ns;
+  uint64_t max_ns;
+  uint32_t hist[ARGUS_HIST_BUCKETS];
+} argus_cell;        /* 160 B */
+
+/* Per-(rank, step, phase) span and, at index n_phases, the whole-iteration span
+ * (NS: "Iteration time is max(end) minus min(start) over a rank-step, and phase time uses the same
+ * rule within each phase"; the quantities the paper measures with CUDA events, PAPER.md:128,
+ * 222-224).  Empty span (R7): min_start INT64_MAX, max_end INT64_MIN, span 0, n_events 0. */
+typedef struct argus_span {
+  int64_t  min_start_ns;
+  int64_t  max_end_ns;
+  uint64_t span_ns;   /* n_events ? max_end - min_start : 0; valid after argus_phase_times */
+  uint64_t n_events;
+} argus_span;         /* 32 B */
+
+/* Header of the fixed-size per-(rank, step) record (NS (5) "summary encoder that emits the
+ * fixed-size per-rank-step record"; R17).  Written by argus_phase_times. */
+#define ARGUS_RECORD_MAGIC   0x53475241u /* 'ARGS' little-endian */
+#define ARGUS_RECORD_VERSION 1
+typedef struct argus_record_header {
+  uint32_t magic;
+  uint16_t version;
+  uint16_t n_phases;
+  uint32_t n_sigs;
+  uint32_t rank;
+  uint32_t step;       /* absolute: step_base + t */
+  uint32_t reserved0;  /* 0 */
+  uint64_t n_events;   /* = whole span n_events */
+  int64_t  min_start_ns;
+  int64_t  max_end_ns;
+  uint64_t iter_ns;    /* = whole span span_ns */
+  uint64_t reserved1;  /* 0 */
+} argus_record_header; /* 64 B */
+
+/* Record layout, record (r, t) at byte offset (r*n_steps + t) * argus_record_bytes(cfg):
+ *   argus_record_header            64 B
+ *   argus_span  span[n_phases + 1] index n_phases = whole iteration
+ *   argus_cell  cell[n_sigs]
+ */
+
+typedef struct argus_config {
+  uint32_t n_ranks;    /* R, 1..ARGUS_MAX_RANKS */
+  uint32_t n_steps;    /* T >= 1; a record is addressed by step - step_base in [0, T) (R19) */
+  uint32_t n_sigs;     /* S >= 1 */
+  uint32_t n_phases;   /* P, 1..ARGUS_MAX_PHASES */
+  uint32_t step_base;
+  uint32_t flags;      /* ARGUS_FLAG_* */
+  int32_t  device;     /* CUDA device ordinal */
+  uint32_t reserved;   /* 0 */
+} argus_config;
+
+/* Per-series result of the cross-rank rule (NS: "per (step, sig), the exact median and MAD over
+ * ranks of the u64 summed duration"; R10 median of an even count = lo + (hi-lo)/2). */
+typedef struct argus_series_stat {
+  uint64_t median;
+  uint64_t mad;
+  uint32_t n_high;
+  uint32_t n_low;
+  uint64_t reserved;   /* 0 */
+} argus_series_stat;   /* 32 B */
+
+/* Outputs of argus_diagnose: a [host] struct of caller-allocated [device] pointers; any may be
+ * NULL to skip that output.  T = n_steps, S = n_sigs, P = n_phases, R = n_ranks. */
+typedef struct argus_diag_out {
+  argus_series_stat* sig_stats;      /* [T][S]       series x[r] = cell[r][t][s].sum_ns (0 if empty, R11) */
+  uint8_t*           sig_flags;      /* [T][S][R]    ARGUS_FLAG_* */
+  argus_series_stat* span_stats;     /* [T][P+1]     series x[r] = span[r][t][k].span_ns; k = P whole iteration (R15) */
+  uint8_t*           span_flags;     /* [T][P+1][R] */
+  uint32_t*          rank_score;     /* [T][R]       # sigs flagged HIGH for (t, r)  — straggler ranks (R15) */
+  uint32_t*          step_anomalous; /* [T]          # ranks whose whole-iteration span is HIGH — anomalous steps (R15) */
+} argus_diag_out;
+
+typedef struct argus_ctx argus_ctx;  /* opaque */
+
+/* Create a context for one table geometry.  Allocates only small device workspace (per-record
+ * state words, counters).  [host] cfg, [host] out. */
+int argus_create(const argus_config* cfg, argus_ctx** out);
+int argus_destroy(argus_ctx* ctx);
+
+/* Bytes of one record = 64 + 32*(P+1) + 160*S, and of the whole [R][T] table.  0 if cfg is NULL. */
+size_t argus_record_bytes(const argus_config* cfg);
+size_t argus_table_bytes(const argus_config* cfg);
+
+/* Start a new accumulation into [device] d_records (argus_table_bytes, 16-byte aligned).
+ * Lazy: marks every record "identity, not yet materialised" in ctx state and zeroes the counters;
+ * the table bytes themselves are defined only after argus_phase_times (which materialises the
+ * identities of R7 for records no event touched).  Asynchronous on `stream`. */
+int argus_reset(argus_ctx* ctx, void* d_records, void* stream);
+
+/* NS (2) ingest: asynchronous copy of n events from [host] pinned memory h_src to [device] d_dst
+ * on `copy_stream`, followed by an internal CUDA event that the next argus_aggregate on this ctx
+ * waits for (so copy and compute overlap across chunks).  n may be 0. */
+int argus_ingest(argus_ctx* ctx, const argus_event* h_src, uint64_t n, argus_event* d_dst,
+                 void* copy_stream);
+
+/* NS (3) aggregate: fold n events at [device] d_events (16-byte aligned; n < 2^32) into the table.
+ * May be called repeatedly (chunks may cut rank-steps anywhere; summaries are a monoid, R7).
+ * Invalid events (R2: end < start or start < 0; R3: rank/step/sig/phase out of range) are skipped
+ * and counted.  Waits for the last argus_ingest.  d_records must be the table given to
+ * argus_reset, else ARGUS_ESTATE.  Asynchronous on `stream`. */
+int argus_aggregate(argus_ctx* ctx, const argus_event* d_events, uint64_t n, void* d_records,
+                    void* stream);
+
+/* NS (2)+(3) streamed aggregate: copy n events from [host] pinned h_events in chunks of
+ * chunk_events through a [device] ring of ring_slots slots (each chunk_events*32 bytes) on an
+ * internal copy stream, overlapped with aggregation of earlier chunks on `stream`.
+ * Equivalent to argus_ingest + argus_aggregate per chunk with ring-slot reuse ordered by events. */
+int argus_aggregate_host(argus_ctx* ctx, const argus_event* h_events, uint64_t n,
+                         uint64_t chunk_events, argus_event* d_ring, uint32_t ring_slots,
+                         void* d_records, void* stream);
+
+/* Finalise (never re-reads events): materialise untouched records, set every span_ns, derive the
+ * whole-iteration span (index P) from the phase spans, write the record headers (NS (5), R17).
+ * If [device] d_spans_out is non-NULL also writes a compact copy argus_span[R][T][P+1].
+ * Idempotent; may be followed by more argus_aggregate calls and another argus_phase_times. */
+int argus_phase_times(argus_ctx* ctx, void* d_records, argus_span* d_spans_out, void* stream);
+
+/* NS (4) cross-rank diagnosis on a finalised table (call argus_phase_times first).  For every
+ * step t and every series family (sigs, phases, whole iteration): exact median and MAD over the
+ * R ranks, flag[r] = |x[r]-med| > sat3(MAD) ? (x[r] > med ? HIGH : LOW) : NONE  (R10-R14),
+ * plus the roll-ups of R15.  [host] outs holds [device] pointers. */
+int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* outs, void* stream);
+
+/* Synchronises all streams the ctx has used and returns the event counters since argus_reset.
+ * Asynchronous kernel faults surface here as ARGUS_ECUDA.  [host] outputs, may be NULL. */
+int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid);
+
+/* Tuning knobs for measurement (not needed for correctness): which = ARGUS_TUNE_*.  */
+#define ARGUS_TUNE_GRID_CTAS   1  /* persistent CTAs of the segmented kernel (0 = #SMs)  */
+#define ARGUS_TUNE_FORCE_PATH  2  /* 0 = by flags, 1 = segmented, 2 = global-table        */
+int argus_tune(argus_ctx* ctx, int which, int64_t value);
+
+const char* argus_strerror(int code);
+int         argus_last_cuda_error(const argus_ctx* ctx); /* cudaError_t of the last ARGUS_ECUDA */
+const char* argus_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ARGUS_H_ */
