@@ -1,0 +1,238 @@
+"""Thin ctypes binding of libargus.so (include/argus.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; torch is used for device memory
+and streams.  There is no CPU fallback: if the library cannot be built/loaded or no CUDA device is
+present, the calls raise."""
+from __future__ import annotations
+
+import ctypes
+from typing import Optional
+
+import numpy as np
+
+from ._build import build_argus
+
+OK, EINVAL, ECUDA, ESIZE, ESTATE, ENOMEM = 0, -1, -2, -3, -4, -5
+FLAG_SORTED = 0x1
+TUNE_GRID_CTAS, TUNE_FORCE_PATH = 1, 2
+PATH_AUTO, PATH_SEGMENTED, PATH_GLOBAL = 0, 1, 2
+
+EVENT_DTYPE = np.dtype(
+    [("rank", "<u4"), ("step", "<u4"), ("sig", "<u4"), ("stream", "<u2"), ("phase", "<u2"),
+     ("start_ns", "<i8"), ("end_ns", "<i8")])
+CELL_DTYPE = np.dtype([("count", "<u8"), ("sum", "<u8"), ("min", "<u8"), ("max", "<u8"),
+                       ("hist", "<u4", (32,))])
+SPAN_DTYPE = np.dtype([("min_start", "<i8"), ("max_end", "<i8"), ("span", "<u8"), ("n", "<u8")])
+STAT_DTYPE = np.dtype([("median", "<u8"), ("mad", "<u8"), ("n_high", "<u4"), ("n_low", "<u4"),
+                       ("reserved", "<u8")])
+HEADER_DTYPE = np.dtype([("magic", "<u4"), ("version", "<u2"), ("n_phases", "<u2"),
+                         ("n_sigs", "<u4"), ("rank", "<u4"), ("step", "<u4"), ("reserved0", "<u4"),
+                         ("n_events", "<u8"), ("min_start", "<i8"), ("max_end", "<i8"),
+                         ("iter_ns", "<u8"), ("reserved1", "<u8")])
+
+EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes", "argus_reset",
+           "argus_ingest", "argus_aggregate", "argus_aggregate_host", "argus_phase_times",
+           "argus_diagnose", "argus_stats", "argus_tune", "argus_strerror", "argus_last_cuda_error",
+           "argus_version"]
+
+
+class ArgusConfig(ctypes.Structure):
+    _fields_ = [("n_ranks", ctypes.c_uint32), ("n_steps", ctypes.c_uint32),
+                ("n_sigs", ctypes.c_uint32), ("n_phases", ctypes.c_uint32),
+                ("step_base", ctypes.c_uint32), ("flags", ctypes.c_uint32),
+                ("device", ctypes.c_int32), ("reserved", ctypes.c_uint32)]
+
+
+class ArgusDiagOut(ctypes.Structure):
+    _fields_ = [("sig_stats", ctypes.c_void_p), ("sig_flags", ctypes.c_void_p),
+                ("span_stats", ctypes.c_void_p), ("span_flags", ctypes.c_void_p),
+                ("rank_score", ctypes.c_void_p), ("step_anomalous", ctypes.c_void_p)]
+
+
+class ArgusError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"argus error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """Build (if stale) and load libargus.so; declare the prototypes of include/argus.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    lib = ctypes.CDLL(build_argus())
+    vp, u64, i32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int
+    cfgp = ctypes.POINTER(ArgusConfig)
+    lib.argus_create.restype = i32
+    lib.argus_create.argtypes = [cfgp, ctypes.POINTER(vp)]
+    lib.argus_destroy.restype = i32
+    lib.argus_destroy.argtypes = [vp]
+    lib.argus_record_bytes.restype = ctypes.c_size_t
+    lib.argus_record_bytes.argtypes = [cfgp]
+    lib.argus_table_bytes.restype = ctypes.c_size_t
+    lib.argus_table_bytes.argtypes = [cfgp]
+    lib.argus_reset.restype = i32
+    lib.argus_reset.argtypes = [vp, vp, vp]
+    lib.argus_ingest.restype = i32
+    lib.argus_ingest.argtypes = [vp, vp, u64, vp, vp]
+    lib.argus_aggregate.restype = i32
+    lib.argus_aggregate.argtypes = [vp, vp, u64, vp, vp]
+    lib.argus_aggregate_host.restype = i32
+    lib.argus_aggregate_host.argtypes = [vp, vp, u64, u64, vp, ctypes.c_uint32, vp, vp]
+    lib.argus_phase_times.restype = i32
+    lib.argus_phase_times.argtypes = [vp, vp, vp, vp]
+    lib.argus_diagnose.restype = i32
+    lib.argus_diagnose.argtypes = [vp, vp, ctypes.POINTER(ArgusDiagOut), vp]
+    lib.argus_stats.restype = i32
+    lib.argus_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    lib.argus_tune.restype = i32
+    lib.argus_tune.argtypes = [vp, i32, ctypes.c_int64]
+    lib.argus_strerror.restype = ctypes.c_char_p
+    lib.argus_strerror.argtypes = [i32]
+    lib.argus_last_cuda_error.restype = i32
+    lib.argus_last_cuda_error.argtypes = [vp]
+    lib.argus_version.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _ptr(x) -> Optional[int]:
+    """Raw address of a torch tensor / numpy array / int / None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    if isinstance(x, np.ndarray):
+        return x.ctypes.data
+    raise TypeError(type(x))
+
+
+def _stream(s) -> Optional[int]:
+    if s is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream or None
+    if isinstance(s, int):
+        return s or None
+    return s.cuda_stream or None
+
+
+class Argus:
+    """One context = one table geometry (R ranks x T steps x S sigs, P phases).  Methods carry the
+    names of the C entry points; all work is queued on CUDA streams."""
+
+    def __init__(self, n_ranks: int, n_steps: int, n_sigs: int, n_phases: int, step_base: int = 0,
+                 sorted_hint: bool = True, device: int = 0):
+        self.lib = load()
+        self.cfg = ArgusConfig(n_ranks, n_steps, n_sigs, n_phases, step_base,
+                               FLAG_SORTED if sorted_hint else 0, device, 0)
+        self.R, self.T, self.S, self.P = n_ranks, n_steps, n_sigs, n_phases
+        self.device = device
+        h = ctypes.c_void_p()
+        rc = self.lib.argus_create(ctypes.byref(self.cfg), ctypes.byref(h))
+        self._h = h if rc == OK else None
+        self._check(rc)
+
+    # ---- plumbing ---------------------------------------------------------------------------
+    def _check(self, rc: int) -> None:
+        if rc != OK:
+            msg = self.lib.argus_strerror(rc).decode()
+            if rc == ECUDA and self._h:
+                msg += f" [cudaError {self.lib.argus_last_cuda_error(self._h)}]"
+            raise ArgusError(rc, msg)
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            self.lib.argus_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def record_bytes(self) -> int:
+        return int(self.lib.argus_record_bytes(ctypes.byref(self.cfg)))
+
+    @property
+    def table_bytes(self) -> int:
+        return int(self.lib.argus_table_bytes(ctypes.byref(self.cfg)))
+
+    def alloc_records(self):
+        import torch
+        return torch.empty(self.table_bytes, dtype=torch.uint8, device=f"cuda:{self.device}")
+
+    def alloc_diag(self) -> dict:
+        import torch
+        dev = f"cuda:{self.device}"
+        R, T, S, P = self.R, self.T, self.S, self.P
+        u8 = torch.uint8
+        return dict(sig_stats=torch.empty(T * S * 32, dtype=u8, device=dev),
+                    sig_flags=torch.empty(T * S * R, dtype=u8, device=dev),
+                    span_stats=torch.empty(T * (P + 1) * 32, dtype=u8, device=dev),
+                    span_flags=torch.empty(T * (P + 1) * R, dtype=u8, device=dev),
+                    rank_score=torch.empty(T * R, dtype=torch.int32, device=dev),
+                    step_anomalous=torch.empty(T, dtype=torch.int32, device=dev))
+
+    # ---- the C entry points -----------------------------------------------------------------
+    def reset(self, d_records, stream=None) -> None:
+        self._check(self.lib.argus_reset(self._h, _ptr(d_records), _stream(stream)))
+
+    def ingest(self, h_src, n: int, d_dst, copy_stream) -> None:
+        self._check(self.lib.argus_ingest(self._h, _ptr(h_src), n, _ptr(d_dst), _stream(copy_stream)))
+
+    def aggregate(self, d_events, n: int, d_records, stream=None) -> None:
+        self._check(self.lib.argus_aggregate(self._h, _ptr(d_events), n, _ptr(d_records),
+                                             _stream(stream)))
+
+    def aggregate_host(self, h_events, n: int, chunk_events: int, d_ring, ring_slots: int,
+                       d_records, stream=None) -> None:
+        self._check(self.lib.argus_aggregate_host(self._h, _ptr(h_events), n, chunk_events,
+                                                  _ptr(d_ring), ring_slots, _ptr(d_records),
+                                                  _stream(stream)))
+
+    def phase_times(self, d_records, d_spans_out=None, stream=None) -> None:
+        self._check(self.lib.argus_phase_times(self._h, _ptr(d_records), _ptr(d_spans_out),
+                                               _stream(stream)))
+
+    def diagnose(self, d_records, outs: dict, stream=None) -> None:
+        o = ArgusDiagOut(*[_ptr(outs.get(k)) for k in ("sig_stats", "sig_flags", "span_stats",
+                                                       "span_flags", "rank_score", "step_anomalous")])
+        self._check(self.lib.argus_diagnose(self._h, _ptr(d_records), ctypes.byref(o),
+                                            _stream(stream)))
+
+    def stats(self):
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self.lib.argus_stats(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return int(a.value), int(b.value)
+
+    def tune(self, which: int, value: int) -> None:
+        self._check(self.lib.argus_tune(self._h, which, value))
+
+    # ---- host-side views of device results (test / report convenience; no arithmetic) ---------
+    def records_to_host(self, d_records) -> np.ndarray:
+        return d_records.cpu().numpy().reshape(self.R * self.T, self.record_bytes)
+
+    def split_records(self, rec: np.ndarray):
+        """uint8 [R*T, record_bytes] -> (headers [R,T], spans [R,T,P+1], cells [R,T,S])."""
+        R, T, S, P = self.R, self.T, self.S, self.P
+        hdr = rec[:, :64].copy().view(HEADER_DTYPE).reshape(R, T)
+        sp = rec[:, 64:64 + 32 * (P + 1)].copy().view(SPAN_DTYPE).reshape(R, T, P + 1)
+        ce = rec[:, 64 + 32 * (P + 1):].copy().view(CELL_DTYPE).reshape(R, T, S)
+        return hdr, sp, ce
+
+    def diag_to_host(self, outs: dict) -> dict:
+        R, T, S, P = self.R, self.T, self.S, self.P
+        return dict(
+            sig_stats=outs["sig_stats"].cpu().numpy().view(STAT_DTYPE).reshape(T, S),
+            sig_flags=outs["sig_flags"].cpu().numpy().reshape(T, S, R),
+            span_stats=outs["span_stats"].cpu().numpy().view(STAT_DTYPE).reshape(T, P + 1),
+            span_flags=outs["span_flags"].cpu().numpy().reshape(T, P + 1, R),
+            rank_score=outs["rank_score"].cpu().numpy().view(np.uint32).reshape(T, R),
+            step_anomalous=outs["step_anomalous"].cpu().numpy().view(np.uint32).reshape(T))

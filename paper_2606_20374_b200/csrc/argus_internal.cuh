@@ -1,0 +1,111 @@
+// argus_internal.cuh — shared declarations of libargus.so (CUDA side only; never seen by the oracle).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "argus.h"
+
+// ---- per-record state words (ctx workspace, one u32 per (rank, step)) -------------------------
+// 0: identity, bytes of the record not written yet (lazy argus_reset)
+// 2: one CTA holds the claim and is writing the record with plain stores
+// 1: materialised — every further contribution merges with atomics
+#define ARGUS_ST_LAZY 0u
+#define ARGUS_ST_BUSY 2u
+#define ARGUS_ST_LIVE 1u
+
+struct argus_dims {
+  uint32_t R, T, S, P, step_base;
+  uint32_t rec_bytes;   // 64 + 32*(P+1) + 160*S
+  uint32_t span_off;    // 64
+  uint32_t cell_off;    // 64 + 32*(P+1)
+};
+
+struct argus_ctx {
+  argus_config cfg;
+  argus_dims dims;
+  int sm_count;
+  int max_smem_optin;
+  uint32_t* d_state;          // [R*T]
+  unsigned long long* d_counters;  // [2] n_valid, n_invalid
+  void* d_records;            // table given to the last argus_reset
+  cudaEvent_t ingest_event;   // recorded after every argus_ingest copy
+  bool ingest_pending;
+  cudaStream_t copy_stream;   // internal, for argus_aggregate_host
+  cudaEvent_t* slot_free;     // ring-slot reuse events (argus_aggregate_host)
+  cudaEvent_t* slot_full;
+  uint32_t n_slot_events;
+  cudaStream_t last_stream;
+  int last_cuda_error;
+  int tune_grid;
+  int tune_path;
+};
+
+// kernels' host-side launchers (each returns cudaError_t of the launch)
+cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
+                                       void* d_records, cudaStream_t s);
+cudaError_t argus_launch_aggregate_global(argus_ctx* ctx, const argus_event* ev, uint64_t n,
+                                          void* d_records, cudaStream_t s);
+cudaError_t argus_launch_materialise_all(argus_ctx* ctx, void* d_records, cudaStream_t s);
+cudaError_t argus_launch_finalize(argus_ctx* ctx, void* d_records, argus_span* d_spans_out,
+                                  cudaStream_t s);
+cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
+                                  cudaStream_t s);
+bool argus_seg_supported(const argus_ctx* ctx);
+
+// ---- device helpers shared by the kernels ------------------------------------------------------
+#ifdef __CUDACC__
+
+// R4: bucket(d) = d==0 ? 0 : min(31, floor(log2 d)), with count-leading-zeros.
+__device__ __forceinline__ uint32_t argus_bucket64(uint64_t d) {
+  uint32_t b = 63u - (uint32_t)__clzll((long long)(d | 1ull));
+  return b > 31u ? 31u : b;
+}
+
+// Event validity (R2, R3) and the dense record index key = rank*T + (step - step_base).
+__device__ __forceinline__ bool argus_event_key(const argus_dims& D, uint32_t rank, uint32_t step,
+                                                uint32_t sig, uint32_t phase, int64_t start,
+                                                int64_t end, uint32_t& key) {
+  uint32_t t = step - D.step_base;  // wraps to >= T when step < step_base (T*R < 2^31)
+  bool ok = (rank < D.R) & (t < D.T) & (sig < D.S) & (phase < D.P) & (start >= 0) & (end >= start);
+  key = rank * D.T + t;
+  return ok;
+}
+
+// One event straight into a LIVE record with L2 atomics (global-table path, and the overflow path
+// of the segmented kernel).  min/max and span bounds are tested first: after the first few events
+// of a cell they rarely improve, so most events cost 3 reductions (count, sum, hist) + 1 (span n).
+__device__ __forceinline__ void argus_global_accumulate(uint8_t* rec, const argus_dims& D,
+                                                        uint32_t sig, uint32_t phase, int64_t start,
+                                                        int64_t end) {
+  uint64_t d = (uint64_t)(end - start);
+  argus_cell* c = reinterpret_cast<argus_cell*>(rec + D.cell_off) + sig;
+  atomicAdd(reinterpret_cast<unsigned long long*>(&c->count), 1ull);
+  atomicAdd(reinterpret_cast<unsigned long long*>(&c->sum_ns), (unsigned long long)d);
+  if (d < *reinterpret_cast<volatile uint64_t*>(&c->min_ns))
+    atomicMin(reinterpret_cast<unsigned long long*>(&c->min_ns), (unsigned long long)d);
+  if (d > *reinterpret_cast<volatile uint64_t*>(&c->max_ns))
+    atomicMax(reinterpret_cast<unsigned long long*>(&c->max_ns), (unsigned long long)d);
+  atomicAdd(&c->hist[argus_bucket64(d)], 1u);
+  argus_span* sp = reinterpret_cast<argus_span*>(rec + D.span_off) + phase;
+  if (start < *reinterpret_cast<volatile int64_t*>(&sp->min_start_ns))
+    atomicMin(reinterpret_cast<long long*>(&sp->min_start_ns), (long long)start);
+  if (end > *reinterpret_cast<volatile int64_t*>(&sp->max_end_ns))
+    atomicMax(reinterpret_cast<long long*>(&sp->max_end_ns), (long long)end);
+  atomicAdd(reinterpret_cast<unsigned long long*>(&sp->n_events), 1ull);
+}
+
+// Identity bytes of the 16-byte chunk `c` of a record's span+cell area (R7).
+// Span area: chunks of argus_span {min_start INT64_MAX, max_end INT64_MIN | span 0, n 0}.
+// Cell area: 10 chunks per cell: {count 0, sum 0} {min UINT64_MAX, max 0} then 8 zero hist chunks.
+__device__ __forceinline__ uint4 argus_identity_chunk(const argus_dims& D, uint32_t chunk) {
+  const uint32_t span_chunks = 2u * (D.P + 1u);
+  if (chunk < span_chunks) {
+    if (chunk & 1u) return make_uint4(0u, 0u, 0u, 0u);
+    return make_uint4(0xFFFFFFFFu, 0x7FFFFFFFu, 0u, 0x80000000u);
+  }
+  uint32_t part = (chunk - span_chunks) % 10u;
+  if (part == 1u) return make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u);
+  return make_uint4(0u, 0u, 0u, 0u);
+}
+
+#endif  // __CUDACC__

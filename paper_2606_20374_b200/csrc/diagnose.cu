@@ -1,0 +1,235 @@
+// diagnose.cu — cross-rank median/MAD selection kernel (NS (4): "per (step, sig), the exact median
+// and MAD over ranks of the u64 summed duration and flags a rank when |x - median| > 3*MAD, all
+// in integer arithmetic"; the paper's comparison of "the same kernel across different ranks",
+// PAPER.md:228).  R15: the same rule runs on the phase spans and on the whole-iteration span.
+//
+// One CTA per series (step t, family member f: sig s < S, or span k = f - S <= P).  The R values
+// live in registers (up to 16 per thread); order statistics come from an exact MSD radix select:
+// a block min/max finds the highest bit in which the candidates differ, then 8-bit digit
+// histograms in shared memory narrow the candidate set until one value remains.  No sort, no
+// sampling, no floating point.
+#include "argus_internal.cuh"
+
+namespace {
+
+constexpr int EPT = 16;
+constexpr uint32_t FULL = 0xFFFFFFFFu;
+
+struct SelSmem {
+  uint32_t hist[256];
+  unsigned long long red_a[32];
+  unsigned long long red_b[32];
+  unsigned long long bcast[2];
+  uint32_t pick_digit, pick_before, pick_count;
+};
+
+template <int NT>
+__device__ __forceinline__ void block_minmax(unsigned long long mn, unsigned long long mx, SelSmem& sm,
+                                             unsigned long long& omn, unsigned long long& omx) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    unsigned long long a = __shfl_xor_sync(FULL, mn, o), b = __shfl_xor_sync(FULL, mx, o);
+    mn = a < mn ? a : mn;
+    mx = b > mx ? b : mx;
+  }
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  __syncthreads();
+  if (lane == 0) { sm.red_a[w] = mn; sm.red_b[w] = mx; }
+  __syncthreads();
+  mn = lane < NT / 32 ? sm.red_a[lane] : ~0ull;
+  mx = lane < NT / 32 ? sm.red_b[lane] : 0ull;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    unsigned long long a = __shfl_xor_sync(FULL, mn, o), b = __shfl_xor_sync(FULL, mx, o);
+    mn = a < mn ? a : mn;
+    mx = b > mx ? b : mx;
+  }
+  omn = mn; omx = mx;
+}
+
+template <int NT>
+__device__ __forceinline__ void block_sum2(uint32_t a, uint32_t b, SelSmem& sm, uint32_t& oa, uint32_t& ob) {
+  a = __reduce_add_sync(FULL, a);
+  b = __reduce_add_sync(FULL, b);
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  __syncthreads();
+  if (lane == 0) { sm.red_a[w] = a; sm.red_b[w] = b; }
+  __syncthreads();
+  a = lane < NT / 32 ? (uint32_t)sm.red_a[lane] : 0u;
+  b = lane < NT / 32 ? (uint32_t)sm.red_b[lane] : 0u;
+  oa = __reduce_add_sync(FULL, a);
+  ob = __reduce_add_sync(FULL, b);
+}
+
+// k-th smallest (0-based) of the block's values v[j] (element index j*NT + tid < R).  Exact.
+template <int NT>
+__device__ unsigned long long block_select(const unsigned long long (&v)[EPT], uint32_t R, uint32_t k,
+                                           SelSmem& sm) {
+  const int tid = threadIdx.x;
+  unsigned long long mn = ~0ull, mx = 0ull;
+#pragma unroll
+  for (int j = 0; j < EPT; ++j)
+    if ((uint32_t)(j * NT + tid) < R) { mn = v[j] < mn ? v[j] : mn; mx = v[j] > mx ? v[j] : mx; }
+  block_minmax<NT>(mn, mx, sm, mn, mx);
+  if (mn == mx) return mn;
+  int top = 63 - __clzll((long long)(mn ^ mx));          // highest bit where candidates differ
+  unsigned long long prefix = (top == 63) ? 0ull : (mn >> (top + 1)) << (top + 1);
+  unsigned long long pmask = (top == 63) ? 0ull : (~0ull << (top + 1));  // bits already fixed
+  int hi_bit = top;
+  for (;;) {
+    const int shift = hi_bit >= 7 ? hi_bit - 7 : 0;
+    const uint32_t dmask = (uint32_t)((1ull << (hi_bit - shift + 1)) - 1ull);
+    __syncthreads();
+    sm.hist[tid & 255] = 0u;
+    if (NT < 256) for (int i = tid; i < 256; i += NT) sm.hist[i] = 0u;
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < EPT; ++j)
+      if ((uint32_t)(j * NT + tid) < R && (v[j] & pmask) == prefix)
+        atomicAdd(&sm.hist[(uint32_t)(v[j] >> shift) & dmask], 1u);
+    __syncthreads();
+    if (tid < 32) {
+      // warp 0: 8 bins per lane, inclusive scan across lanes, pick the bin holding rank k
+      uint32_t c[8], s = 0;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { c[i] = sm.hist[tid * 8 + i]; s += c[i]; }
+      uint32_t inc = s;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        uint32_t t = __shfl_up_sync(FULL, inc, o);
+        if (tid >= o) inc += t;
+      }
+      uint32_t before = inc - s;
+      if (k >= before && k < inc) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          if (k >= before && k < before + c[i]) {
+            sm.pick_digit = tid * 8 + i; sm.pick_before = before; sm.pick_count = c[i];
+          }
+          before += c[i];
+        }
+      }
+    }
+    __syncthreads();
+    const uint32_t digit = sm.pick_digit, cnt = sm.pick_count;
+    k -= sm.pick_before;
+    prefix |= (unsigned long long)digit << shift;
+    pmask |= (unsigned long long)dmask << shift;
+    if (shift == 0) return prefix;
+    if (cnt == 1u) {
+      // a single candidate is left: whoever holds it publishes it
+#pragma unroll
+      for (int j = 0; j < EPT; ++j)
+        if ((uint32_t)(j * NT + tid) < R && (v[j] & pmask) == prefix) sm.bcast[0] = v[j];
+      __syncthreads();
+      return sm.bcast[0];
+    }
+    hi_bit = shift - 1;
+  }
+}
+
+// median (R10) of the block's values: lo = v_(k), hi = v_(k+1 if R even), med = lo + (hi-lo)/2
+template <int NT>
+__device__ unsigned long long block_median(const unsigned long long (&v)[EPT], uint32_t R, SelSmem& sm) {
+  const int tid = threadIdx.x;
+  const uint32_t k = (R - 1) / 2;
+  const unsigned long long lo = block_select<NT>(v, R, k, sm);
+  if ((R & 1u) != 0u) return lo;
+  // hi = v[R/2] = v[k+1]: equals lo when at least k+2 values are <= lo, else the smallest value > lo
+  uint32_t le = 0;
+  unsigned long long gt_min = ~0ull;
+#pragma unroll
+  for (int j = 0; j < EPT; ++j)
+    if ((uint32_t)(j * NT + tid) < R) {
+      if (v[j] <= lo) ++le;
+      else gt_min = v[j] < gt_min ? v[j] : gt_min;
+    }
+  uint32_t le_all, dummy;
+  block_sum2<NT>(le, 0u, sm, le_all, dummy);
+  unsigned long long mn, mx;
+  block_minmax<NT>(gt_min, 0ull, sm, mn, mx);
+  const unsigned long long hi = (le_all >= k + 2u) ? lo : mn;
+  return lo + (hi - lo) / 2ull;
+}
+
+template <int NT>
+__global__ void __launch_bounds__(NT)
+diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_out out) {
+  __shared__ SelSmem sm;
+  const int tid = threadIdx.x;
+  const uint32_t F = D.S + D.P + 1u;
+  const uint32_t t = blockIdx.x / F, f = blockIdx.x % F;
+  const bool is_sig = f < D.S;
+  const uint32_t R = D.R;
+  if (is_sig ? (out.sig_stats == nullptr && out.sig_flags == nullptr && out.rank_score == nullptr)
+             : (out.span_stats == nullptr && out.span_flags == nullptr && out.step_anomalous == nullptr))
+    return;
+
+  // ---- gather x[r] over ranks (a6) ----------------------------------------------------------
+  unsigned long long x[EPT];
+  const size_t off = is_sig ? (size_t)D.cell_off + (size_t)f * sizeof(argus_cell)
+                            : (size_t)D.span_off + (size_t)(f - D.S) * sizeof(argus_span) + 16u;
+#pragma unroll
+  for (int j = 0; j < EPT; ++j) {
+    const uint32_t r = (uint32_t)(j * NT + tid);
+    x[j] = 0ull;
+    if (r < R) {
+      const ulonglong2 q = __ldg(reinterpret_cast<const ulonglong2*>(
+          records + ((size_t)r * D.T + t) * D.rec_bytes + off));
+      // cell: {count, sum} -> sum if count (R11: empty = 0);  span: {span_ns, n_events} -> span_ns
+      x[j] = is_sig ? (q.x ? q.y : 0ull) : q.x;
+    }
+  }
+  // ---- a7 median, a8 MAD ----------------------------------------------------------------------
+  const unsigned long long med = block_median<NT>(x, R, sm);
+  unsigned long long dev[EPT];
+#pragma unroll
+  for (int j = 0; j < EPT; ++j) dev[j] = x[j] >= med ? x[j] - med : med - x[j];
+  const unsigned long long mad = block_median<NT>(dev, R, sm);
+  const unsigned long long thr = mad > 0xFFFFFFFFFFFFFFFFull / 3ull ? 0xFFFFFFFFFFFFFFFFull : 3ull * mad;  // R12
+  // ---- flags + roll-ups -------------------------------------------------------------------------
+  uint8_t* fl = is_sig ? out.sig_flags : out.span_flags;
+  const size_t series = is_sig ? (size_t)t * D.S + f : (size_t)t * (D.P + 1u) + (f - D.S);
+  uint32_t nh = 0, nl = 0;
+#pragma unroll
+  for (int j = 0; j < EPT; ++j) {
+    const uint32_t r = (uint32_t)(j * NT + tid);
+    if (r < R) {
+      uint8_t g = ARGUS_FLAG_NONE;
+      if (dev[j] > thr) g = x[j] > med ? ARGUS_FLAG_HIGH : ARGUS_FLAG_LOW;   // R13, R14
+      nh += g == ARGUS_FLAG_HIGH;
+      nl += g == ARGUS_FLAG_LOW;
+      if (fl) fl[series * R + r] = g;
+      if (is_sig && out.rank_score && g == ARGUS_FLAG_HIGH) atomicAdd(&out.rank_score[(size_t)t * R + r], 1u);
+    }
+  }
+  uint32_t NH, NL;
+  block_sum2<NT>(nh, nl, sm, NH, NL);
+  if (tid == 0) {
+    argus_series_stat st;
+    st.median = med; st.mad = mad; st.n_high = NH; st.n_low = NL; st.reserved = 0;
+    if (is_sig) { if (out.sig_stats) out.sig_stats[series] = st; }
+    else {
+      if (out.span_stats) out.span_stats[series] = st;
+      if (f - D.S == D.P && out.step_anomalous) out.step_anomalous[t] = NH;
+    }
+  }
+}
+
+}  // namespace
+
+cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
+                                  cudaStream_t s) {
+  const argus_dims& D = ctx->dims;
+  if (o->rank_score) {
+    cudaError_t e = cudaMemsetAsync(o->rank_score, 0, (size_t)D.T * D.R * sizeof(uint32_t), s);
+    if (e != cudaSuccess) return e;
+  }
+  const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);
+  if (blocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
+  const uint8_t* rec = static_cast<const uint8_t*>(d_records);
+  if (D.R <= 64u * EPT) diagnose_kernel<64><<<(unsigned)blocks, 64, 0, s>>>(rec, D, *o);
+  else if (D.R <= 256u * EPT) diagnose_kernel<256><<<(unsigned)blocks, 256, 0, s>>>(rec, D, *o);
+  else diagnose_kernel<1024><<<(unsigned)blocks, 1024, 0, s>>>(rec, D, *o);
+  return cudaGetLastError();
+}

@@ -1,0 +1,175 @@
+"""-m gpu parity tests: the CUDA path through the C ABI vs the CPU oracle, bit-exact (all work is
+integer), on the same seeded bytes.  Sizes the oracle finishes in seconds, spanning several tiles
+and ragged tails; the edge cases of DESIGN.md §3."""
+import dataclasses
+import random
+
+import numpy as np
+import pytest
+
+from gpu_util import assert_parity, run_gpu
+from helpers import check_handworked, make_events, parse_handworked, parse_series_cases
+from paper_2606_20374_b200.workload import EVENT_DTYPE, build_workload, scaled
+
+pytestmark = pytest.mark.gpu
+
+PATH_SEG, PATH_GLOBAL = 1, 2
+
+
+def _dims(spec):
+    return spec.n_ranks, spec.n_steps, spec.n_sigs, spec.n_phases, spec.step_base
+
+
+def test_handworked_golden_gpu():
+    from paper_2606_20374_b200 import argus as A
+    g = parse_handworked()
+    for path in (PATH_SEG, PATH_GLOBAL):
+        rec, diag, stats, spans = run_gpu(g["events"], 3, 1, 2, 2, 0, path=path)
+        ctx = A.Argus(3, 1, 2, 2, 0)
+        hdr, sp, ce = ctx.split_records(rec)
+        check_handworked(g, ce, sp, stats[0], stats[1], diag)
+        assert (sp == spans).all()
+        assert list(hdr["n_events"].reshape(-1)) == [3, 2, 2]
+        assert list(hdr["iter_ns"].reshape(-1)) == [3148, 3200, 10000]
+        ctx.close()
+
+
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+def test_tiny_parity(path):
+    wl = build_workload("tiny")
+    ev = wl.expand_host()
+    rec, diag, o = assert_parity(ev, *_dims(wl.spec), path=path)
+    assert (diag["sig_flags"][:, 17, 5] == 1).all() and diag["span_flags"][2, 1, 3] == 1
+
+
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+def test_tiny_chunked_mid_rank_step(path):
+    wl = build_workload("tiny")
+    ev = wl.expand_host()
+    cuts = [0, 1, 777, 2000, 2001, 31999, 32000, 50000, ev.size]
+    assert_parity(ev, *_dims(wl.spec), path=path, cuts=cuts)
+
+
+def test_tiny_many_small_ctas():
+    # rank-steps cut by CTA boundaries: the claim/merge protocol of the flush
+    wl = build_workload("tiny")
+    ev = wl.expand_host()
+    for grid in (1, 3, 64, 1000):
+        assert_parity(ev, *_dims(wl.spec), path=PATH_SEG, grid=grid)
+
+
+def test_violated_sorted_hint_still_exact():
+    wl = build_workload(scaled("tiny", n_ranks=4, n_steps=2, n_events=600))
+    ev = wl.expand_host()
+    rng = np.random.default_rng(3)
+    assert_parity(ev[rng.permutation(ev.size)], *_dims(wl.spec), path=PATH_SEG)
+
+
+def _random_events(rnd, n, R, T, S, P, base, big):
+    rows = []
+    for _ in range(n):
+        r = rnd.randrange(R + (1 if rnd.random() < 0.02 else 0))
+        st = base + rnd.randrange(-1 if (base and rnd.random() < 0.02) else 0, T + (1 if rnd.random() < 0.02 else 0))
+        s = rnd.randrange(S + (1 if rnd.random() < 0.02 else 0))
+        ph = rnd.randrange(P + (1 if rnd.random() < 0.02 else 0))
+        a = rnd.randrange(0, 10**9)
+        if rnd.random() < 0.01:
+            a = -rnd.randrange(1, 100)
+        mode = rnd.random()
+        if mode < 0.02:
+            d = -rnd.randrange(1, 1000)
+        elif mode < 0.06:
+            d = rnd.choice([0, 1, 2, 3])
+        elif big and mode < 0.3:
+            d = rnd.getrandbits(rnd.randint(1, 62))     # many buckets per sig, durations >= 2^32
+        else:
+            d = int(rnd.lognormvariate(10, 1.5))
+        rows.append((r, st, s, rnd.randrange(65536), ph, a, min(a + d, 2**63 - 1)))
+    rows.sort(key=lambda x: (x[0], x[1]))
+    return make_events(rows)
+
+
+@pytest.mark.parametrize("seed,dims,big", [(1, (3, 2, 5, 2, 0), False), (2, (8, 3, 16, 4, 10), True),
+                                           (3, (1, 1, 1, 1, 0), True), (4, (5, 1, 7, 3, 1000), True),
+                                           (5, (2, 2, 3, 64, 5), True)])
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+def test_random_with_invalid_and_overflow(seed, dims, big, path):
+    R, T, S, P, base = dims
+    ev = _random_events(random.Random(seed), 6000, R, T, S, P, base, big)
+    rec, diag, o = assert_parity(ev, R, T, S, P, base, path=path)
+    assert o.n_invalid > 0
+
+
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+def test_empty_input(path):
+    ev = np.zeros(0, dtype=EVENT_DTYPE)
+    assert_parity(ev, 4, 2, 9, 3, 0, path=path)
+
+
+def test_sum_wrap_and_clamp_bucket():
+    big = 2**63 - 1
+    ev = make_events([(0, 0, 0, 0, 0, 0, big)] * 5 + [(1, 0, 1, 0, 0, 5, 5)])
+    for path in (PATH_SEG, PATH_GLOBAL):
+        assert_parity(ev, 2, 1, 2, 1, 0, path=path)
+
+
+def test_hot_single_sig_carry():
+    # one sig, one bucket, durations near 2^32: the u32 sum_lo carries constantly
+    n = 50000
+    ev = np.zeros(n, dtype=EVENT_DTYPE)
+    ev["start_ns"] = np.arange(n)
+    ev["end_ns"] = ev["start_ns"] + (2**32 - 1 - (np.arange(n) % 7))
+    assert_parity(ev, 1, 1, 1, 1, 0, path=PATH_SEG)
+
+
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+def test_mid_scaled(path):
+    wl = build_workload(scaled("mid", n_ranks=48, n_steps=3))
+    ev = wl.expand_host()
+    assert_parity(ev, *_dims(wl.spec), path=path)
+
+
+def test_production_scaled_large_S():
+    # S = 4096 (the compact table fills the CTA's shared memory), 16 phases, 8 streams, ragged N
+    wl = build_workload(scaled("production", n_ranks=24, n_events=100_003))
+    ev = wl.expand_host()
+    assert_parity(ev, *_dims(wl.spec), path=PATH_SEG)
+
+
+def test_unsorted_scaled():
+    wl = build_workload(scaled("unsorted", n_ranks=64, n_events=20000))
+    ev = wl.expand_host()
+    assert_parity(ev, *_dims(wl.spec), sorted_hint=False)
+
+
+def test_odd_rank_counts_select():
+    # R = 1, 2, 3, 9, 257, 4097 (odd/even medians, > 4096 ranks uses the 1024-thread select)
+    rnd = random.Random(11)
+    for R in (1, 2, 3, 9, 257, 4097):
+        rows = []
+        for r in range(R):
+            for s in range(3):
+                if rnd.random() < 0.9:
+                    rows.append((r, 0, s, 0, s % 2, 1000 * r, 1000 * r + rnd.randrange(1, 10**6) * (50 if rnd.random() < 0.02 else 1)))
+        assert_parity(make_events(rows), R, 1, 3, 2, 0, path=PATH_SEG)
+
+
+def test_series_closed_forms_gpu():
+    # golden series through the whole path: one event per rank with duration x (x < 2^63)
+    for x, med, mad, fl in parse_series_cases():
+        if max(x) >= 2**63:
+            continue
+        ev = make_events([(r, 0, 0, 0, 0, 0, v) for r, v in enumerate(x)])
+        rec, diag, stats, _ = run_gpu(ev, len(x), 1, 1, 1, 0)
+        st = diag["sig_stats"][0, 0]
+        assert (int(st["median"]), int(st["mad"])) == (med, mad), x
+        assert list(diag["sig_flags"][0, 0]) == fl, x
+
+
+def test_device_expander_matches_host():
+    import torch
+    for name, kw in (("tiny", {}), ("mid", dict(n_ranks=8, n_steps=2)), ("unsorted", dict(n_ranks=8, n_events=3000))):
+        wl = build_workload(scaled(name, **kw))
+        h = wl.expand_host().view(np.uint8).reshape(-1)
+        d = wl.expand_device().cpu().numpy()
+        assert (h == d).all(), name
