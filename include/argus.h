@@ -198,6 +198,7 @@ int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid);
 /* Tuning knobs for measurement (not needed for correctness): which = ARGUS_TUNE_*.  */
 #define ARGUS_TUNE_GRID_CTAS   1  /* persistent CTAs of the segmented kernel (0 = #SMs)  */
 #define ARGUS_TUNE_FORCE_PATH  2  /* 0 = by flags, 1 = segmented, 2 = global-table        */
+#define ARGUS_TUNE_SEG_VARIANT 3  /* thread/unroll geometry of the segmented kernel (0 = default) */
 int argus_tune(argus_ctx* ctx, int which, int64_t value);
 
 const char* argus_strerror(int code);

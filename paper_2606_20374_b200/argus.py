@@ -14,7 +14,7 @@ from ._build import build_argus
 
 OK, EINVAL, ECUDA, ESIZE, ESTATE, ENOMEM = 0, -1, -2, -3, -4, -5
 FLAG_SORTED = 0x1
-TUNE_GRID_CTAS, TUNE_FORCE_PATH = 1, 2
+TUNE_GRID_CTAS, TUNE_FORCE_PATH, TUNE_SEG_VARIANT = 1, 2, 3
 PATH_AUTO, PATH_SEGMENTED, PATH_GLOBAL = 0, 1, 2
 
 EVENT_DTYPE = np.dtype(

@@ -25,7 +25,7 @@ __global__ void materialise_kernel(uint8_t* records, uint32_t* state, argus_dims
 __global__ void __launch_bounds__(256)
 aggregate_global_kernel(const uint4* __restrict__ ev, uint64_t n, uint8_t* records,
                         unsigned long long* counters, argus_dims D) {
-  uint32_t n_valid = 0, n_invalid = 0;
+  uint32_t n_valid = 0, n_invalid = 0;   // counters[0] counts events SEEN, counters[1] rejected
   const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
   const int lane = threadIdx.x & 31;
   // lane pairs fetch the two 16-byte halves of an event as ONE coalesced 512-byte warp access per
@@ -49,12 +49,12 @@ aggregate_global_kernel(const uint4* __restrict__ ev, uint64_t n, uint8_t* recor
     const uint4 hi = odd ? b : got;
     const uint64_t idx = base + (odd ? 16 + (lane >> 1) : (lane >> 1));
     if (idx < n) {
+      ++n_valid;
       const uint32_t phase = lo.w >> 16;
       const long long start = (long long)(((unsigned long long)hi.y << 32) | hi.x);
       const long long end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
       uint32_t key;
       if (argus_event_key(D, lo.x, lo.y, lo.z, phase, start, end, key)) {
-        ++n_valid;
         argus_global_accumulate(records + (size_t)key * D.rec_bytes, D, lo.z, phase, start, end);
       } else {
         ++n_invalid;

@@ -4,29 +4,33 @@
 // reductions where a block spans rank-step boundaries, and flush to global in one pass").
 //
 // One persistent CTA per SM walks a contiguous span of the event buffer.  Events arrive through a
-// ring of 8 KB stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx).  The
-// CTA keeps ONE (rank, step) table in shared memory at a time, in a compact 32-byte cell per sig
-// (DESIGN.md §6.1): four tagged histogram slots {bucket+1 : 6 bits | count : 26 bits}, a 64-bit
-// sum split into two u32 words with carry, ~min and max as u32.  Only native 32-bit shared atomics
-// are used (64-bit shared atomics compile to CAS loops on sm_100a).  An event the compact cell
-// cannot take (duration >= 2^32 ns, or a fifth distinct bucket of one sig) goes straight to the
-// global record with L2 atomics.  When the (rank, step) key changes the table is flushed: the
-// first CTA to reach a record claims it and writes the whole 160-byte cells with coalesced
-// 128-bit stores (no read-modify-write, no separate identity fill); any later contribution to the
-// same record merges with L2 reductions.  Correct for ANY event order; fast when events are
-// grouped by (rank, step) (R18).
+// ring of 8 KB stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx, L2
+// evict-first).  Each thread takes EPT events per iteration into registers; the stages are
+// refilled right after that load phase, so the whole ring is in flight while the CTA accumulates.
+// The CTA keeps ONE (rank, step) table in shared memory at a time, 32 bytes per sig, laid out as
+// structure-of-arrays so that random sigs spread over all 32 banks:
+//   slots[S]  uint4: four tagged histogram slots {bucket+1 : 6 bits | count : 26 bits}; the word
+//                    a slot lives in is XOR-swizzled with sig bits 3-4
+//   sum_lo[S], sum_hi[S] u32: the 64-bit sum with an explicit carry
+//   mm[S]     uint2: {~min, max} as u32
+// Only native 32-bit shared atomics are used (64-bit shared atomics are CAS loops on sm_100a).
+// An event the compact cell cannot take (duration >= 2^32 ns, or a fifth distinct bucket of one
+// sig) goes straight to the global record with L2 atomics.  When the (rank, step) key changes the
+// table is flushed: the first CTA to reach a record claims it and writes the whole 160-byte cells
+// with coalesced 128-bit stores (no read-modify-write, no separate identity fill); any later
+// contribution to the same record merges with L2 reductions.  Correct for ANY event order; fast
+// when events are grouped by (rank, step) (R18).
 #include "argus_internal.cuh"
 
 namespace {
 
-constexpr int NT = 1024;             // threads per CTA
 constexpr int SUB = 256;             // events per TMA stage (8 KB)
-constexpr int G = NT / SUB;          // stages consumed per iteration
-constexpr int MAXK = 20;             // ring stages (bounded by shared memory at launch)
+constexpr int MAXK = 24;             // ring stages (bounded by shared memory at launch)
 constexpr uint32_t KEY_NONE = 0xFFFFFFFFu;
 constexpr uint32_t FULL = 0xFFFFFFFFu;
-constexpr int HDR_BYTES = 256;
-constexpr int SPAN_BYTES = ARGUS_MAX_PHASES * 32;
+constexpr uint32_t HDR_BYTES = 256;
+constexpr uint32_t SPAN_BYTES = ARGUS_MAX_PHASES * 32;
+constexpr uint32_t TAB_OFF = HDR_BYTES + SPAN_BYTES;   // compact table starts here
 
 struct SpanAcc {                      // shared-memory span accumulator of one phase (32 B)
   long long mn, mx;
@@ -37,11 +41,29 @@ struct SpanAcc {                      // shared-memory span accumulator of one p
 struct Hdr {
   unsigned long long bars[MAXK];      // mbarriers, one per stage
   uint32_t cur_key;
-  uint32_t flags;                     // bit 0: some event of this iteration needs the global path
+  uint32_t flags;                     // != 0: some event of this iteration needs the global path
   uint32_t next_idx;                  // lowest pending event index (key switch)
   uint32_t mode;                      // state word seen by the flush claim
 };
 static_assert(sizeof(Hdr) <= HDR_BYTES, "header");
+
+extern __shared__ __align__(128) uint8_t smem[];
+
+// The compact table of one (rank, step), addressed by 32-bit offsets from the dynamic shared
+// window: slots[S] uint4 | sum_lo[S] u32 | sum_hi[S] u32 | mm[S] uint2 {~min, max}.
+struct Table {
+  uint32_t S;
+  __device__ __forceinline__ uint4* slots(uint32_t sig) const { return reinterpret_cast<uint4*>(smem + TAB_OFF) + sig; }
+  __device__ __forceinline__ uint32_t* slot_words(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF) + 4u * sig; }
+  __device__ __forceinline__ uint32_t* sum_lo(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF + 16u * S) + sig; }
+  __device__ __forceinline__ uint32_t* sum_hi(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF + 20u * S) + sig; }
+  __device__ __forceinline__ uint2* mm(uint32_t sig) const { return reinterpret_cast<uint2*>(smem + TAB_OFF + 24u * S) + sig; }
+};
+__device__ __forceinline__ Hdr* hdr() { return reinterpret_cast<Hdr*>(smem); }
+__device__ __forceinline__ SpanAcc* span_tab() { return reinterpret_cast<SpanAcc*>(smem + HDR_BYTES); }
+__host__ __device__ __forceinline__ uint32_t stage_off(uint32_t S) {
+  return (TAB_OFF + 32u * ((S + 3u) & ~3u) + 127u) & ~127u;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
@@ -54,10 +76,11 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
                : "memory");
 }
 __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint32_t bytes,
-                                            uint32_t bar) {
+                                            uint32_t bar, uint64_t policy) {
   asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
-      "l"(src), "r"(bytes), "r"(bar)
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1], %2, [%3], %4;" ::"r"(dst),
+      "l"(src), "r"(bytes), "r"(bar), "l"(policy)
       : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
@@ -101,76 +124,69 @@ struct WarpSpan {
     phase = KEY_NONE; n = 0; mn = INT64_MAX; mx = INT64_MIN;
   }
   // all 32 lanes call
-  __device__ __forceinline__ void flush(SpanAcc* spans, int lane) {
+  __device__ __forceinline__ void flush(int lane) {
     if (phase != KEY_NONE) {
       long long a = warp_min_i64(mn), b = warp_max_i64(mx);
       uint32_t c = __reduce_add_sync(FULL, n);
       if (lane == 0 && c) {
-        atomicMin(&spans[phase].mn, a);
-        atomicMax(&spans[phase].mx, b);
-        atomicAdd(&spans[phase].n, (unsigned long long)c);
+        SpanAcc* sp = span_tab() + phase;
+        atomicMin(&sp->mn, a);
+        atomicMax(&sp->mx, b);
+        atomicAdd(&sp->n, (unsigned long long)c);
       }
     }
     reset();
   }
 };
 
-struct Ctx {
-  Hdr* H;
-  SpanAcc* spans;
-  uint4* table;  // 2 uint4 per sig: {slot0..3} {sum_lo, sum_hi, ~min, max}
+struct Glob {             // global-memory side of the kernel
   uint8_t* records;
   uint32_t* state;
   argus_dims D;
 };
 
-// Fold one accepted event into the compact table.  Returns false if it needs the global path.
-__device__ __forceinline__ bool cell_accumulate(uint4* table, uint32_t sig, uint64_t d) {
-  if (d >> 32) return false;
-  const uint32_t d32 = (uint32_t)d;
-  const uint32_t tag = (31u - (uint32_t)__clz((int)(d32 | 1u))) + 1u;  // bucket + 1, 1..32
-  uint32_t* cell = reinterpret_cast<uint32_t*>(table + 2 * sig);
-  const uint4 s = *reinterpret_cast<const uint4*>(cell);
-  int j = -1;
-  if ((s.x & 63u) == tag) j = 0;
-  else if ((s.y & 63u) == tag) j = 1;
-  else if ((s.z & 63u) == tag) j = 2;
-  else if ((s.w & 63u) == tag) j = 3;
-  if (j >= 0) {
-    atomicAdd(cell + j, 64u);
-  } else {
-    // claim a slot (first events of a sig in this rank-step); slots fill in order and are never
-    // released before the flush, so a tag lives in at most one slot
-    bool done = false;
-#pragma unroll 1
-    for (int k = 0; k < 4 && !done; ++k) {
-      uint32_t v = *reinterpret_cast<volatile uint32_t*>(cell + k);
-      if (v == 0u) {
-        v = atomicCAS(cell + k, 0u, tag | 64u);
-        if (v == 0u) { done = true; break; }
-      }
-      if ((v & 63u) == tag) { atomicAdd(cell + k, 64u); done = true; }
-    }
-    if (!done) return false;
+// Histogram part of one event: bump the slot tagged bucket+1, claiming one if needed.
+// `s` is a (possibly stale) snapshot of the sig's four slot words.  Returns false if all four
+// slots hold other buckets.
+__device__ __forceinline__ bool slot_update(const Table& tb, uint32_t sig, uint32_t tag, const uint4& s) {
+  uint32_t* w = tb.slot_words(sig);
+  int p = -1;
+  if ((s.x & 63u) == tag) p = 0;
+  else if ((s.y & 63u) == tag) p = 1;
+  else if ((s.z & 63u) == tag) p = 2;
+  else if ((s.w & 63u) == tag) p = 3;
+  if (p >= 0) {
+    atomicAdd(w + p, 64u);
+    return true;
   }
-  const uint32_t old = atomicAdd(cell + 4, d32);
-  if (old + d32 < old) atomicAdd(cell + 5, 1u);
-  const uint2 mm = *reinterpret_cast<const uint2*>(cell + 6);
-  if (~d32 > mm.x) atomicMax(cell + 6, ~d32);
-  if (d32 > mm.y) atomicMax(cell + 7, d32);
-  return true;
+  // claim (first events of a bucket in this rank-step).  Slots are claimed in a fixed per-sig
+  // order (logical j -> word j ^ swz) and never released before the flush, so a tag lives in at
+  // most one slot.  The swizzle spreads the first-claimed (hottest) slot over all banks.
+  const int swz = (int)((sig >> 3) & 3u);
+#pragma unroll 1
+  for (int j = 0; j < 4; ++j) {
+    uint32_t* q = w + (j ^ swz);
+    uint32_t v = *reinterpret_cast<volatile uint32_t*>(q);
+    if (v == 0u) {
+      v = atomicCAS(q, 0u, tag | 64u);
+      if (v == 0u) return true;
+    }
+    if ((v & 63u) == tag) { atomicAdd(q, 64u); return true; }
+  }
+  return false;
 }
 
 // 16-byte chunk `part` (0..9) of the 160-byte argus_cell decoded from a compact cell.
-__device__ __forceinline__ uint4 cell_chunk(const uint4 s, const uint4 m, uint32_t part) {
+__device__ __forceinline__ uint4 cell_chunk(const uint4 s, uint32_t sum_lo, uint32_t sum_hi,
+                                            const uint2 m, uint32_t part) {
   const uint32_t c0 = s.x >> 6, c1 = s.y >> 6, c2 = s.z >> 6, c3 = s.w >> 6;
   if (part == 0u) {
     unsigned long long cnt = (unsigned long long)c0 + c1 + c2 + c3;
-    return make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), m.x, m.y);
+    return make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), sum_lo, sum_hi);
   }
   if (part == 1u) {
     if ((c0 | c1 | c2 | c3) == 0u) return make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u);
-    return make_uint4(~m.z, 0u, m.w, 0u);
+    return make_uint4(~m.x, 0u, m.y, 0u);
   }
   const uint32_t b0 = 4u * (part - 2u) + 1u;  // tag of the chunk's first bucket
   const uint32_t t0 = s.x & 63u, t1 = s.y & 63u, t2 = s.z & 63u, t3 = s.w & 63u;
@@ -182,25 +198,29 @@ __device__ __forceinline__ uint4 cell_chunk(const uint4 s, const uint4 m, uint32
   return v;
 }
 
-// Flush the shared table of record `key` to global memory and clear it.  All threads call.
-// The caller has flushed its WarpSpan first.
-__device__ __noinline__ void flush_table(const Ctx& c, uint32_t key) {
+// Flush the shared table of record `key` to global memory and clear it.  All threads call; the
+// caller has flushed its WarpSpan first.
+template <int NT>
+__device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
   const int tid = threadIdx.x;
-  const argus_dims& D = c.D;
+  const argus_dims& D = g.D;
+  const Table tb{D.S};
+  Hdr* H = hdr();
+  SpanAcc* spans = span_tab();
   __syncthreads();
   if (tid == 0) {
-    uint32_t old = atomicCAS(&c.state[key], ARGUS_ST_LAZY, ARGUS_ST_BUSY);
+    uint32_t old = atomicCAS(&g.state[key], ARGUS_ST_LAZY, ARGUS_ST_BUSY);
     if (old == ARGUS_ST_BUSY) {
       // another (resident, running) CTA is writing this record: wait for it, then merge
-      while (atomicAdd(&c.state[key], 0u) != ARGUS_ST_LIVE) __nanosleep(128);
+      while (atomicAdd(&g.state[key], 0u) != ARGUS_ST_LIVE) __nanosleep(128);
       __threadfence();
       old = ARGUS_ST_LIVE;
     }
-    c.H->mode = old;
+    H->mode = old;
   }
   __syncthreads();
-  const uint32_t mode = c.H->mode;
-  uint8_t* rec = c.records + (size_t)key * D.rec_bytes;
+  const uint32_t mode = H->mode;
+  uint8_t* rec = g.records + (size_t)key * D.rec_bytes;
   if (mode == ARGUS_ST_LAZY) {
     // we own the record: write spans + cells once, coalesced 16-byte chunks
     uint4* dst = reinterpret_cast<uint4*>(rec + D.span_off);
@@ -210,8 +230,8 @@ __device__ __noinline__ void flush_table(const Ctx& c, uint32_t key) {
       uint4 v;
       if (ch < span_chunks) {
         const uint32_t k = ch >> 1;
-        if (k < D.P && c.spans[k].n != 0ull) {
-          const SpanAcc a = c.spans[k];
+        if (k < D.P && spans[k].n != 0ull) {
+          const SpanAcc a = spans[k];
           v = (ch & 1u) ? make_uint4(0u, 0u, (uint32_t)a.n, (uint32_t)(a.n >> 32))
                         : make_uint4((uint32_t)a.mn, (uint32_t)((unsigned long long)a.mn >> 32),
                                      (uint32_t)a.mx, (uint32_t)((unsigned long long)a.mx >> 32));
@@ -221,18 +241,19 @@ __device__ __noinline__ void flush_table(const Ctx& c, uint32_t key) {
       } else {
         const uint32_t cc = ch - span_chunks;
         const uint32_t sig = cc / 10u, part = cc - sig * 10u;
-        v = cell_chunk(c.table[2 * sig], c.table[2 * sig + 1], part);
+        v = cell_chunk(*tb.slots(sig), *tb.sum_lo(sig), *tb.sum_hi(sig), *tb.mm(sig), part);
       }
-      dst[ch] = v;
+      __stcs(dst + ch, v);
     }
     __threadfence();
     __syncthreads();
-    if (tid == 0) atomicExch(&c.state[key], ARGUS_ST_LIVE);
+    if (tid == 0) atomicExch(&g.state[key], ARGUS_ST_LIVE);
   } else {
     // merge into a live record with L2 reductions (non-empty fields only)
     argus_cell* cells = reinterpret_cast<argus_cell*>(rec + D.cell_off);
     for (uint32_t sig = tid; sig < D.S; sig += NT) {
-      const uint4 s = c.table[2 * sig], m = c.table[2 * sig + 1];
+      const uint4 s = *tb.slots(sig);
+      const uint2 m = *tb.mm(sig);
       const uint32_t sl[4] = {s.x, s.y, s.z, s.w};
       unsigned long long cnt = 0;
 #pragma unroll
@@ -246,16 +267,16 @@ __device__ __noinline__ void flush_table(const Ctx& c, uint32_t key) {
       if (cnt) {
         atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].count), cnt);
         atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].sum_ns),
-                  ((unsigned long long)m.y << 32) | m.x);
+                  ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig));
         atomicMin(reinterpret_cast<unsigned long long*>(&cells[sig].min_ns),
-                  (unsigned long long)(~m.z));
+                  (unsigned long long)(~m.x));
         atomicMax(reinterpret_cast<unsigned long long*>(&cells[sig].max_ns),
-                  (unsigned long long)m.w);
+                  (unsigned long long)m.y);
       }
     }
     argus_span* sp = reinterpret_cast<argus_span*>(rec + D.span_off);
     for (uint32_t k = tid; k < D.P; k += NT) {
-      const SpanAcc a = c.spans[k];
+      const SpanAcc a = spans[k];
       if (a.n) {
         atomicMin(reinterpret_cast<long long*>(&sp[k].min_start_ns), a.mn);
         atomicMax(reinterpret_cast<long long*>(&sp[k].max_end_ns), a.mx);
@@ -264,23 +285,26 @@ __device__ __noinline__ void flush_table(const Ctx& c, uint32_t key) {
     }
   }
   __syncthreads();
-  for (uint32_t i = tid; i < 2u * D.S; i += NT) c.table[i] = make_uint4(0u, 0u, 0u, 0u);
+  uint4* all = tb.slots(0);           // slots, sum_lo, sum_hi, mm are contiguous: 2*S uint4
+  for (uint32_t i = tid; i < 2u * D.S; i += NT) all[i] = make_uint4(0u, 0u, 0u, 0u);
   for (uint32_t k = tid; k < D.P; k += NT) {
-    c.spans[k].mn = INT64_MAX; c.spans[k].mx = INT64_MIN; c.spans[k].n = 0ull; c.spans[k].pad = 0ull;
+    spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
   }
   __syncthreads();
 }
 
+template <int NT, int EPT>
 __global__ void __launch_bounds__(NT, 1)
 aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta, uint8_t* records,
                      uint32_t* state, unsigned long long* counters, argus_dims D, int K) {
-  extern __shared__ __align__(128) uint8_t smem[];
-  Ctx c;
-  c.H = reinterpret_cast<Hdr*>(smem);
-  c.spans = reinterpret_cast<SpanAcc*>(smem + HDR_BYTES);
-  c.table = reinterpret_cast<uint4*>(smem + HDR_BYTES + SPAN_BYTES);
-  c.records = records; c.state = state; c.D = D;
-  uint8_t* stages = smem + ((HDR_BYTES + SPAN_BYTES + 32u * D.S + 127u) & ~127u);
+  constexpr int G = EPT * NT / SUB;    // stages consumed per iteration
+  constexpr int WPS = NT / SUB;        // stage groups per event slot (threads / stage size)
+  static_assert(NT % SUB == 0 && G >= 1, "geometry");
+  Glob gl;
+  gl.records = records; gl.state = state; gl.D = D;
+  const Table tb{D.S};
+  Hdr* H = hdr();
+  const uint32_t stages = stage_off(D.S);     // byte offset of the stage ring in smem
 
   const int tid = threadIdx.x, lane = tid & 31;
   const uint64_t e0 = (uint64_t)blockIdx.x * per_cta;
@@ -288,168 +312,246 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   const uint64_t e1 = (e0 + per_cta < n) ? e0 + per_cta : n;
   const uint32_t n_ev = (uint32_t)(e1 - e0);
   const uint32_t n_sub = (n_ev + SUB - 1) / SUB;
-  const uint32_t n_iter = (n_ev + NT - 1) / NT;
+  const uint32_t n_iter = (n_ev + EPT * NT - 1) / (EPT * NT);
   const uint4* src = ev + 2 * e0;
 
   if (tid == 0) {
-    for (int k = 0; k < K; ++k) mbar_init(smem_u32(&c.H->bars[k]), 1u);
-    c.H->cur_key = KEY_NONE; c.H->flags = 0u; c.H->next_idx = KEY_NONE; c.H->mode = 0u;
+    for (int k = 0; k < K; ++k) mbar_init(smem_u32(&H->bars[k]), 1u);
+    H->cur_key = KEY_NONE; H->flags = 0u; H->next_idx = KEY_NONE; H->mode = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  for (uint32_t i = tid; i < 2u * D.S; i += NT) c.table[i] = make_uint4(0u, 0u, 0u, 0u);
-  for (uint32_t k = tid; k < ARGUS_MAX_PHASES; k += NT) {
-    c.spans[k].mn = INT64_MAX; c.spans[k].mx = INT64_MIN; c.spans[k].n = 0ull; c.spans[k].pad = 0ull;
+  {
+    uint4* all = tb.slots(0);
+    for (uint32_t i = tid; i < 2u * D.S; i += NT) all[i] = make_uint4(0u, 0u, 0u, 0u);
+    SpanAcc* spans = span_tab();
+    for (uint32_t k = tid; k < ARGUS_MAX_PHASES; k += NT) {
+      spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
+    }
   }
   __syncthreads();
 
-  auto issue = [&](uint32_t s) {  // thread 0 only
-    const uint32_t slot = s % (uint32_t)K;
+  uint64_t policy = 0;
+  if (tid == 0) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+  auto issue = [&](uint32_t s, uint32_t slot) {  // thread 0 only: stage s into ring slot `slot`
     const uint32_t cnt = (n_ev - s * SUB < (uint32_t)SUB) ? n_ev - s * SUB : (uint32_t)SUB;
-    const uint32_t bar = smem_u32(&c.H->bars[slot]);
+    const uint32_t bar = smem_u32(&H->bars[slot]);
     mbar_expect_tx(bar, cnt * 32u);
-    tma_load_1d(smem_u32(stages + (size_t)slot * SUB * 32), src + 2 * (size_t)s * SUB, cnt * 32u, bar);
+    tma_load_1d(smem_u32(smem + stages + slot * (SUB * 32u)), src + 2 * (size_t)s * SUB, cnt * 32u, bar, policy);
   };
   if (tid == 0)
-    for (uint32_t s = 0; s < (uint32_t)K && s < n_sub; ++s) issue(s);
+    for (uint32_t s = 0; s < (uint32_t)K && s < n_sub; ++s) issue(s, s);
 
   WarpSpan ws;
   ws.reset();
   uint32_t cur_key = KEY_NONE;
-  uint32_t n_valid = 0, n_invalid = 0;
+  uint32_t n_invalid = 0;
+  // ring position of stage it*G + tid/SUB (this thread's first stage); the others follow at +WPS
+  uint32_t slot0 = (uint32_t)(tid / SUB) % (uint32_t)K, par0 = 0;
+  uint32_t base_slot = 0;
 
   for (uint32_t it = 0; it < n_iter; ++it) {
-    const uint32_t s = it * G + (uint32_t)(tid / SUB);
-    const uint32_t idx = it * NT + (uint32_t)tid;
-    const bool active = idx < n_ev;
-    uint32_t rank = 0, step = 0, sig = 0, phase = 0, key = KEY_NONE;
-    long long start = 0, end = 0;
-    bool pending = false;
-    if (s < n_sub) {
-      mbar_wait(smem_u32(&c.H->bars[s % (uint32_t)K]), (s / (uint32_t)K) & 1u);
-      if (active) {
-        // lanes 0-3,8-11,.. read the first half first, the others the second: conflict-free LDS.128
-        const uint4* p = reinterpret_cast<const uint4*>(stages + (size_t)(s % (uint32_t)K) * SUB * 32) +
-                         2 * (tid % SUB);
-        const int h = (lane >> 2) & 1;
-        const uint4 a = p[h], b = p[h ^ 1];
-        const uint4 lo = h ? b : a, hi = h ? a : b;
-        rank = lo.x; step = lo.y; sig = lo.z; phase = lo.w >> 16;
-        start = (long long)(((unsigned long long)hi.y << 32) | hi.x);
-        end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
-        pending = argus_event_key(D, rank, step, sig, phase, start, end, key);
-        if (pending) ++n_valid; else ++n_invalid;
+    // ---- load phase: EPT events per thread, stage -> registers ---------------------------------
+    uint32_t sig[EPT], phase[EPT], key[EPT];
+    long long start[EPT], end[EPT];
+    bool pending[EPT];
+    {
+      uint32_t sl = slot0, pr = par0;
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        const uint32_t s = it * G + (uint32_t)(e * WPS + tid / SUB);
+        const uint32_t idx = it * (EPT * NT) + (uint32_t)(e * NT + tid);
+        pending[e] = false; sig[e] = 0; phase[e] = 0; key[e] = KEY_NONE; start[e] = 0; end[e] = 0;
+        if (s < n_sub) {
+          mbar_wait(smem_u32(&H->bars[sl]), pr);
+          if (idx < n_ev) {
+            // lanes 0-3,8-11,.. read the first half first, the others the second: conflict-free LDS.128
+            const uint4* p = reinterpret_cast<const uint4*>(smem + stages + sl * (SUB * 32u)) + 2 * (tid % SUB);
+            const int h = (lane >> 2) & 1;
+            const uint4 a = p[h], b = p[h ^ 1];
+            const uint4 lo = h ? b : a, hi = h ? a : b;
+            sig[e] = lo.z; phase[e] = lo.w >> 16;
+            start[e] = (long long)(((unsigned long long)hi.y << 32) | hi.x);
+            end[e] = (long long)(((unsigned long long)hi.w << 32) | hi.z);
+            pending[e] = argus_event_key(D, lo.x, lo.y, lo.z, phase[e], start[e], end[e], key[e]);
+            n_invalid += pending[e] ? 0u : 1u;
+          }
+        }
+        sl += WPS; if (sl >= (uint32_t)K) { sl -= (uint32_t)K; pr ^= 1u; }
+      }
+      slot0 = sl; par0 = pr;     // EPT*WPS = G stages further
+    }
+    __syncthreads();   // every thread holds its events: the G stages can be refilled right away
+    if (tid == 0) {
+      uint32_t sl = base_slot;
+#pragma unroll 1
+      for (uint32_t g = 0; g < (uint32_t)G; ++g) {
+        const uint32_t sn = it * G + (uint32_t)K + g;
+        if (sn < n_sub) issue(sn, sl);
+        if (++sl == (uint32_t)K) sl = 0;
       }
     }
-    bool ovf = false;
+    base_slot += G; if (base_slot >= (uint32_t)K) base_slot -= (uint32_t)K;
+
+    uint32_t ovf_mask = 0;
     for (;;) {
-      const bool accept = pending && key == cur_key;
-      // ---- spans: warp-uniform fast path in registers, else per-phase ballot groups -----------
-      const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
-      if (__all_sync(FULL, accept && phase == ph0)) {
-        if (ws.phase != ph0) { ws.flush(c.spans, lane); ws.phase = ph0; }
-        ws.mn = start < ws.mn ? start : ws.mn;
-        ws.mx = end > ws.mx ? end : ws.mx;
-        ws.n++;
-      } else {
-        uint32_t todo = __ballot_sync(FULL, accept);
-        while (todo) {
-          const int leader = __ffs((int)todo) - 1;
-          const uint32_t ph = __shfl_sync(FULL, phase, leader);
-          const bool mine = accept && phase == ph;
-          const uint32_t grp = __ballot_sync(FULL, mine);
-          const long long a = warp_min_i64(mine ? start : INT64_MAX);
-          const long long b = warp_max_i64(mine ? end : INT64_MIN);
-          if (lane == leader) {
-            atomicMin(&c.spans[ph].mn, a);
-            atomicMax(&c.spans[ph].mx, b);
-            atomicAdd(&c.spans[ph].n, (unsigned long long)__popc(grp));
+      bool accept[EPT];
+      uint4 snap[EPT];
+      uint2 mmv[EPT];
+      // ---- table loads for all accepted events first (ILP), then the atomics ---------------------
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        accept[e] = pending[e] && key[e] == cur_key;
+        if (accept[e]) { snap[e] = *tb.slots(sig[e]); mmv[e] = *tb.mm(sig[e]); }
+      }
+      // ---- spans: warp-uniform fast path in registers, else per-phase ballot groups ---------------
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        const uint32_t ph0 = __shfl_sync(FULL, phase[e], 0);
+        if (__all_sync(FULL, accept[e] && phase[e] == ph0)) {
+          if (ws.phase != ph0) { ws.flush(lane); ws.phase = ph0; }
+          ws.mn = start[e] < ws.mn ? start[e] : ws.mn;
+          ws.mx = end[e] > ws.mx ? end[e] : ws.mx;
+          ws.n++;
+        } else {
+          uint32_t todo = __ballot_sync(FULL, accept[e]);
+          while (todo) {
+            const int leader = __ffs((int)todo) - 1;
+            const uint32_t ph = __shfl_sync(FULL, phase[e], leader);
+            const bool mine = accept[e] && phase[e] == ph;
+            const uint32_t grp = __ballot_sync(FULL, mine);
+            const long long a = warp_min_i64(mine ? start[e] : INT64_MAX);
+            const long long b = warp_max_i64(mine ? end[e] : INT64_MIN);
+            if (lane == leader) {
+              SpanAcc* sp = span_tab() + ph;
+              atomicMin(&sp->mn, a);
+              atomicMax(&sp->mx, b);
+              atomicAdd(&sp->n, (unsigned long long)__popc(grp));
+            }
+            todo &= ~grp;
           }
-          todo &= ~grp;
         }
       }
-      // ---- cells -----------------------------------------------------------------------------
-      if (accept) {
-        if (!cell_accumulate(c.table, sig, (uint64_t)(end - start))) {
-          ovf = true;
-          c.H->flags = 1u;
+      // ---- cells ------------------------------------------------------------------------------------
+      uint32_t d32[EPT], old[EPT];
+      bool fits[EPT];
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        const unsigned long long d = (unsigned long long)(end[e] - start[e]);
+        d32[e] = (uint32_t)d;
+        fits[e] = accept[e] && (d >> 32) == 0ull;
+        if (fits[e]) {
+          const uint32_t tag = (31u - (uint32_t)__clz((int)(d32[e] | 1u))) + 1u;  // bucket + 1
+          fits[e] = slot_update(tb, sig[e], tag, snap[e]);
         }
-        pending = false;
+        if (accept[e] && !fits[e]) { ovf_mask |= 1u << e; H->flags = 1u; }
       }
-      const int any_pending = __syncthreads_or(pending ? 1 : 0);
-      if (c.H->flags) {  // uniform: written before the barrier
+#pragma unroll
+      for (int e = 0; e < EPT; ++e)
+        if (fits[e]) old[e] = atomicAdd(tb.sum_lo(sig[e]), d32[e]);
+#pragma unroll
+      for (int e = 0; e < EPT; ++e)
+        if (fits[e]) {
+          if (~d32[e] > mmv[e].x) atomicMax(&tb.mm(sig[e])->x, ~d32[e]);
+          if (d32[e] > mmv[e].y) atomicMax(&tb.mm(sig[e])->y, d32[e]);
+        }
+      bool pend = false;
+#pragma unroll
+      for (int e = 0; e < EPT; ++e) {
+        if (fits[e] && old[e] + d32[e] < old[e]) atomicAdd(tb.sum_hi(sig[e]), 1u);
+        if (accept[e]) pending[e] = false;
+        pend |= pending[e];
+      }
+      const int any_pending = __syncthreads_or(pend ? 1 : 0);
+      if (H->flags) {  // uniform: written before the barrier
         // rare: some event does not fit the compact cell -> make the record live, then L2 atomics
-        { ws.flush(c.spans, lane); flush_table(c, cur_key); }
-        if (ovf) {
-          // the span part was already folded above; only the cell goes the global way
-          uint8_t* rec = records + (size_t)cur_key * D.rec_bytes;
-          const uint64_t d = (uint64_t)(end - start);
-          argus_cell* cl = reinterpret_cast<argus_cell*>(rec + D.cell_off) + sig;
-          atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
-          atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), (unsigned long long)d);
-          atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), (unsigned long long)d);
-          atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), (unsigned long long)d);
-          atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
-          ovf = false;
-        }
-        if (tid == 0) c.H->flags = 0u;
+        ws.flush(lane);
+        flush_table<NT>(gl, cur_key);
+#pragma unroll
+        for (int e = 0; e < EPT; ++e)
+          if (ovf_mask & (1u << e)) {
+            // the span part was already folded above; only the cell goes the global way
+            uint8_t* rec = records + (size_t)cur_key * D.rec_bytes;
+            const uint64_t d = (uint64_t)(end[e] - start[e]);
+            argus_cell* cl = reinterpret_cast<argus_cell*>(rec + D.cell_off) + sig[e];
+            atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
+            atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), (unsigned long long)d);
+            atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), (unsigned long long)d);
+            atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), (unsigned long long)d);
+            atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
+          }
+        ovf_mask = 0;
+        if (tid == 0) H->flags = 0u;
         __syncthreads();
       }
       if (!any_pending) break;
-      // ---- key switch: flush the finished record, adopt the key of the first pending event -----
-      if (cur_key != KEY_NONE) { ws.flush(c.spans, lane); flush_table(c, cur_key); }
-      if (pending) atomicMin(&c.H->next_idx, (uint32_t)tid);
+      // ---- key switch: flush the finished record, adopt the key of the first pending event --------
+      if (cur_key != KEY_NONE) { ws.flush(lane); flush_table<NT>(gl, cur_key); }
+#pragma unroll
+      for (int e = EPT - 1; e >= 0; --e)
+        if (pending[e]) atomicMin(&H->next_idx, (uint32_t)(e * NT + tid));
       __syncthreads();
-      if ((uint32_t)tid == c.H->next_idx) c.H->cur_key = key;
+      {
+        const uint32_t pick = H->next_idx;
+#pragma unroll
+        for (int e = 0; e < EPT; ++e)
+          if ((uint32_t)(e * NT + tid) == pick) H->cur_key = key[e];
+      }
       __syncthreads();
-      cur_key = c.H->cur_key;
-      if (tid == 0) c.H->next_idx = KEY_NONE;
+      cur_key = H->cur_key;
+      if (tid == 0) H->next_idx = KEY_NONE;
       // (next_idx is next read after at least one more barrier)
     }
-    // every thread is past its reads of this iteration's stages: refill them
-    if (tid == 0) {
-      for (uint32_t g = 0; g < (uint32_t)G; ++g) {
-        const uint32_t sn = it * G + (uint32_t)K + g;
-        if (sn < n_sub) issue(sn);
-      }
-    }
   }
-  if (cur_key != KEY_NONE) { ws.flush(c.spans, lane); flush_table(c, cur_key); }
+  if (cur_key != KEY_NONE) { ws.flush(lane); flush_table<NT>(gl, cur_key); }
 
-  n_valid = __reduce_add_sync(FULL, n_valid);
   n_invalid = __reduce_add_sync(FULL, n_invalid);
-  if (lane == 0) {
-    if (n_valid) atomicAdd(&counters[0], (unsigned long long)n_valid);
-    if (n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
-  }
+  if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
+  if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // valid = seen - invalid (host)
 }
 
-size_t seg_fixed_smem(uint32_t S) { return (HDR_BYTES + SPAN_BYTES + 32u * (size_t)S + 127u) & ~(size_t)127u; }
+template <int NT, int EPT>
+cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records,
+                           cudaStream_t s) {
+  constexpr int G = EPT * NT / SUB;
+  const size_t fixed = stage_off(ctx->dims.S);
+  int K = (int)(((size_t)ctx->max_smem_optin - fixed) / ((size_t)SUB * 32));
+  if (K > MAXK) K = MAXK;
+  if (K < G) return cudaErrorInvalidConfiguration;
+  const size_t smem_bytes = fixed + (size_t)K * SUB * 32;
+  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<NT, EPT>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+  if (e != cudaSuccess) return e;
+  int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count;
+  // a CTA's slot counters hold 26 bits between flushes: bound the span of one CTA
+  const uint64_t tile = (uint64_t)EPT * NT;
+  const uint64_t cap = (1ull << 26) - tile;
+  uint64_t per_cta = (n + grid - 1) / grid;
+  if (per_cta > cap) per_cta = cap;
+  per_cta = (per_cta + tile - 1) / tile * tile;
+  const uint64_t ctas = (n + per_cta - 1) / per_cta;
+  aggregate_seg_kernel<NT, EPT><<<(unsigned)ctas, NT, smem_bytes, s>>>(
+      reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
+      ctx->d_counters, ctx->dims, K);
+  return cudaGetLastError();
+}
 
 }  // namespace
 
 bool argus_seg_supported(const argus_ctx* ctx) {
-  return seg_fixed_smem(ctx->dims.S) + (size_t)(G + 1) * SUB * 32 <= (size_t)ctx->max_smem_optin;
+  // the smallest variant consumes 4 stages (32 KB) per iteration
+  return (size_t)stage_off(ctx->dims.S) + (size_t)8 * SUB * 32 <= (size_t)ctx->max_smem_optin;
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
                                        void* d_records, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
-  const size_t fixed = seg_fixed_smem(ctx->dims.S);
-  int K = (int)(((size_t)ctx->max_smem_optin - fixed) / ((size_t)SUB * 32));
-  if (K > MAXK) K = MAXK;
-  const size_t smem = fixed + (size_t)K * SUB * 32;
-  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel,
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
-  int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count;
-  // a CTA's slot counters hold 26 bits between flushes: bound the span of one CTA
-  const uint64_t cap = (1ull << 26) - NT;
-  uint64_t per_cta = (n + grid - 1) / grid;
-  if (per_cta > cap) per_cta = cap;
-  per_cta = (per_cta + NT - 1) / NT * NT;
-  const uint64_t ctas = (n + per_cta - 1) / per_cta;
-  aggregate_seg_kernel<<<(unsigned)ctas, NT, smem, s>>>(
-      reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
-      ctx->d_counters, ctx->dims, K);
-  return cudaGetLastError();
+  switch (ctx->tune_variant) {
+    case 1: return launch_variant<1024, 1>(ctx, ev, n, d_records, s);
+    case 2: return launch_variant<1024, 2>(ctx, ev, n, d_records, s);
+    case 3: return launch_variant<512, 2>(ctx, ev, n, d_records, s);
+    case 5: return launch_variant<256, 8>(ctx, ev, n, d_records, s);
+    case 6: return launch_variant<768, 2>(ctx, ev, n, d_records, s);
+    case 4:
+    default: return launch_variant<512, 4>(ctx, ev, n, d_records, s);
+  }
 }

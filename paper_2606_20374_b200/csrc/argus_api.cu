@@ -217,6 +217,7 @@ extern "C" int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invali
   CU(ctx, cudaStreamSynchronize(ctx->last_stream));
   unsigned long long h[2] = {0, 0};
   CU(ctx, cudaMemcpy(h, ctx->d_counters, sizeof h, cudaMemcpyDeviceToHost));
+  h[0] -= h[1];  // kernels count events seen and events rejected
   if (n_valid) *n_valid = h[0];
   if (n_invalid) *n_invalid = h[1];
   return ARGUS_OK;
@@ -228,6 +229,9 @@ extern "C" int argus_tune(argus_ctx* ctx, int which, int64_t value) {
     case ARGUS_TUNE_GRID_CTAS:
       if (value < 0 || value > 65535) return ARGUS_EINVAL;
       ctx->tune_grid = (int)value;
+      return ARGUS_OK;
+    case ARGUS_TUNE_SEG_VARIANT:
+      ctx->tune_variant = (int)value;
       return ARGUS_OK;
     case ARGUS_TUNE_FORCE_PATH:
       if (value < 0 || value > 2) return ARGUS_EINVAL;

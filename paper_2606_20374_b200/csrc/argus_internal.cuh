@@ -38,6 +38,7 @@ struct argus_ctx {
   int last_cuda_error;
   int tune_grid;
   int tune_path;
+  int tune_variant;
 };
 
 // kernels' host-side launchers (each returns cudaError_t of the launch)
