@@ -24,11 +24,10 @@
 
 namespace {
 
-constexpr int SUB = 256;             // events per TMA stage (8 KB)
-constexpr int MAXK = 24;             // ring stages (bounded by shared memory at launch)
+constexpr int MAXK = 48;             // ring stages (bounded by shared memory at launch)
 constexpr uint32_t KEY_NONE = 0xFFFFFFFFu;
 constexpr uint32_t FULL = 0xFFFFFFFFu;
-constexpr uint32_t HDR_BYTES = 256;
+constexpr uint32_t HDR_BYTES = 1024;
 constexpr uint32_t SPAN_BYTES = ARGUS_MAX_PHASES * 32;
 constexpr uint32_t TAB_OFF = HDR_BYTES + SPAN_BYTES;   // compact table starts here
 
@@ -39,11 +38,14 @@ struct SpanAcc {                      // shared-memory span accumulator of one p
 };
 
 struct Hdr {
-  unsigned long long bars[MAXK];      // mbarriers, one per stage
-  uint32_t cur_key;
-  uint32_t flags;                     // != 0: some event of this iteration needs the global path
-  uint32_t next_idx;                  // lowest pending event index (key switch)
+  unsigned long long full[MAXK];      // mbarriers: stage filled by TMA (tx bytes)
+  unsigned long long empty[MAXK];     // mbarriers: stage read by all its consumer warps
+  uint32_t cur_key;                   // key adopted at the rendezvous
+  uint32_t pad0;
+  uint32_t next_idx;                  // lowest pending event index
   uint32_t mode;                      // state word seen by the flush claim
+  uint32_t n_finished;                // consumer warps that ran out of events
+  uint32_t decision;                  // outcome of the current rendezvous
 };
 static_assert(sizeof(Hdr) <= HDR_BYTES, "header");
 
@@ -95,6 +97,20 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
       "}" ::"r"(bar),
       "r"(parity)
       : "memory");
+}
+
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+      "selp.u32 %0, 1, 0, P1;\n"
+      "}"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return ok != 0u;
 }
 
 __device__ __forceinline__ long long warp_min_i64(long long v) {
@@ -198,16 +214,23 @@ __device__ __forceinline__ uint4 cell_chunk(const uint4 s, uint32_t sum_lo, uint
   return v;
 }
 
-// Flush the shared table of record `key` to global memory and clear it.  All threads call; the
-// caller has flushed its WarpSpan first.
-template <int NT>
+__device__ __forceinline__ void bar_consumers(int n) {   // named barrier 1: consumer warps only
+  asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+// Flush the shared table of record `key` to global memory and clear it.  All NC consumer threads
+// call (tid < NC); each warp has flushed its WarpSpan first.  Ends with a consumer barrier.
+template <int NC>
 __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
   const int tid = threadIdx.x;
   const argus_dims& D = g.D;
   const Table tb{D.S};
   Hdr* H = hdr();
   SpanAcc* spans = span_tab();
-  __syncthreads();
+  bar_consumers(NC);
   if (tid == 0) {
     uint32_t old = atomicCAS(&g.state[key], ARGUS_ST_LAZY, ARGUS_ST_BUSY);
     if (old == ARGUS_ST_BUSY) {
@@ -218,7 +241,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
     }
     H->mode = old;
   }
-  __syncthreads();
+  bar_consumers(NC);
   const uint32_t mode = H->mode;
   uint8_t* rec = g.records + (size_t)key * D.rec_bytes;
   if (mode == ARGUS_ST_LAZY) {
@@ -226,7 +249,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
     uint4* dst = reinterpret_cast<uint4*>(rec + D.span_off);
     const uint32_t span_chunks = 2u * (D.P + 1u);
     const uint32_t n_chunks = span_chunks + 10u * D.S;
-    for (uint32_t ch = tid; ch < n_chunks; ch += NT) {
+    for (uint32_t ch = tid; ch < n_chunks; ch += NC) {
       uint4 v;
       if (ch < span_chunks) {
         const uint32_t k = ch >> 1;
@@ -246,12 +269,12 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
       __stcs(dst + ch, v);
     }
     __threadfence();
-    __syncthreads();
+    bar_consumers(NC);
     if (tid == 0) atomicExch(&g.state[key], ARGUS_ST_LIVE);
   } else {
     // merge into a live record with L2 reductions (non-empty fields only)
     argus_cell* cells = reinterpret_cast<argus_cell*>(rec + D.cell_off);
-    for (uint32_t sig = tid; sig < D.S; sig += NT) {
+    for (uint32_t sig = tid; sig < D.S; sig += NC) {
       const uint4 s = *tb.slots(sig);
       const uint2 m = *tb.mm(sig);
       const uint32_t sl[4] = {s.x, s.y, s.z, s.w};
@@ -275,7 +298,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
       }
     }
     argus_span* sp = reinterpret_cast<argus_span*>(rec + D.span_off);
-    for (uint32_t k = tid; k < D.P; k += NT) {
+    for (uint32_t k = tid; k < D.P; k += NC) {
       const SpanAcc a = spans[k];
       if (a.n) {
         atomicMin(reinterpret_cast<long long*>(&sp[k].min_start_ns), a.mn);
@@ -284,252 +307,271 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
       }
     }
   }
-  __syncthreads();
+  bar_consumers(NC);
   uint4* all = tb.slots(0);           // slots, sum_lo, sum_hi, mm are contiguous: 2*S uint4
-  for (uint32_t i = tid; i < 2u * D.S; i += NT) all[i] = make_uint4(0u, 0u, 0u, 0u);
-  for (uint32_t k = tid; k < D.P; k += NT) {
+  for (uint32_t i = tid; i < 2u * D.S; i += NC) all[i] = make_uint4(0u, 0u, 0u, 0u);
+  for (uint32_t k = tid; k < D.P; k += NC) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
   }
-  __syncthreads();
+  bar_consumers(NC);
 }
 
-template <int NT, int EPT>
-__global__ void __launch_bounds__(NT, 1)
+// Rendezvous of all consumer warps (the only CTA-wide synchronisation of the steady state, taken
+// once per (rank, step) boundary on grouped input).  A warp comes here when it holds an event it
+// cannot fold: another key than the table's, or an event that needs the global path while the
+// record is not live yet.  Warps that see H->park_flag, or have run out of events, join.  Then the
+// table is flushed and the key of the lowest pending event becomes current.  Returns true when no
+// warp has anything left (the last table has been flushed).
+// Result packed as {cur_key : 32 | live : 1 | all_done : 1} (by value: keeps the caller's state in registers).
+constexpr unsigned long long PARK_LIVE = 1ull << 32, PARK_DONE = 1ull << 33;
+constexpr uint32_t DEC_SWITCH = 0u, DEC_SPURIOUS = 1u, DEC_DONE = 2u;
+template <int NC>
+__device__ __noinline__ unsigned long long park(const Glob& gl, bool pending, uint32_t key,
+                                                uint32_t my_idx, uint32_t cur_key, uint32_t live) {
+  Hdr* H = hdr();
+  const int tid = threadIdx.x;
+  // a pending event's index is the rendezvous request: every warp whose position in the stream is
+  // beyond H->next_idx comes here instead of going on (finished warps just wait here)
+  if (pending) atomicMin(&H->next_idx, my_idx);
+  bar_consumers(NC);
+  const uint32_t pick = *reinterpret_cast<volatile uint32_t*>(&H->next_idx);
+  if (tid == 0) {
+    const uint32_t fin = *reinterpret_cast<volatile uint32_t*>(&H->n_finished);
+    H->decision = pick != KEY_NONE ? DEC_SWITCH : (fin == (uint32_t)(NC / 32) ? DEC_DONE : DEC_SPURIOUS);
+  }
+  if (pending && my_idx == pick) H->cur_key = key;
+  bar_consumers(NC);
+  const uint32_t dec = *reinterpret_cast<volatile uint32_t*>(&H->decision);
+  const uint32_t nk = *reinterpret_cast<volatile uint32_t*>(&H->cur_key);
+  if (dec == DEC_SPURIOUS) {            // nobody holds a pending event, but not every warp is done
+    bar_consumers(NC);
+    return (unsigned long long)cur_key | (live ? PARK_LIVE : 0ull);
+  }
+  if (dec == DEC_DONE) {
+    if (cur_key != KEY_NONE) flush_table<NC>(gl, cur_key);
+    return PARK_DONE | cur_key;
+  }
+  if (cur_key != KEY_NONE) flush_table<NC>(gl, cur_key);   // begins and ends with a consumer barrier
+  else bar_consumers(NC);
+  if (tid == 0) H->next_idx = KEY_NONE;
+  bar_consumers(NC);
+  if (nk == cur_key) live = 1u;          // an overflow event asked for a live record
+  else { cur_key = nk; live = 0u; }
+  return (unsigned long long)cur_key | (live ? PARK_LIVE : 0ull);
+}
+
+// CW consumer warps + 1 producer warp.  Stage = WPSTG warps' worth of events (WPSTG KB).
+template <int CW, int WPSTG>
+__global__ void __launch_bounds__((CW + 1) * 32, 1)
 aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta, uint8_t* records,
                      uint32_t* state, unsigned long long* counters, argus_dims D, int K) {
-  constexpr int G = EPT * NT / SUB;    // stages consumed per iteration
-  constexpr int WPS = NT / SUB;        // stage groups per event slot (threads / stage size)
-  static_assert(NT % SUB == 0 && G >= 1, "geometry");
+  constexpr int NC = CW * 32;            // consumer threads
+  constexpr int SUBE = WPSTG * 32;       // events per stage
+  constexpr int SPI = CW / WPSTG;        // stages per iteration
+  static_assert(CW % WPSTG == 0, "geometry");
   Glob gl;
   gl.records = records; gl.state = state; gl.D = D;
   const Table tb{D.S};
   Hdr* H = hdr();
   const uint32_t stages = stage_off(D.S);     // byte offset of the stage ring in smem
 
-  const int tid = threadIdx.x, lane = tid & 31;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint64_t e0 = (uint64_t)blockIdx.x * per_cta;
   if (e0 >= n) return;
   const uint64_t e1 = (e0 + per_cta < n) ? e0 + per_cta : n;
   const uint32_t n_ev = (uint32_t)(e1 - e0);
-  const uint32_t n_sub = (n_ev + SUB - 1) / SUB;
-  const uint32_t n_iter = (n_ev + EPT * NT - 1) / (EPT * NT);
+  const uint32_t n_sub = (n_ev + SUBE - 1) / SUBE;
+  const uint32_t n_iter = (n_ev + NC - 1) / NC;
   const uint4* src = ev + 2 * e0;
 
   if (tid == 0) {
-    for (int k = 0; k < K; ++k) mbar_init(smem_u32(&H->bars[k]), 1u);
-    H->cur_key = KEY_NONE; H->flags = 0u; H->next_idx = KEY_NONE; H->mode = 0u;
+    for (int k = 0; k < K; ++k) {
+      mbar_init(smem_u32(&H->full[k]), 1u);
+      mbar_init(smem_u32(&H->empty[k]), (uint32_t)WPSTG);
+    }
+    H->cur_key = KEY_NONE; H->pad0 = 0u; H->next_idx = KEY_NONE; H->mode = 0u;
+    H->n_finished = 0u; H->decision = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   {
     uint4* all = tb.slots(0);
-    for (uint32_t i = tid; i < 2u * D.S; i += NT) all[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (uint32_t i = tid; i < 2u * D.S; i += (CW + 1) * 32) all[i] = make_uint4(0u, 0u, 0u, 0u);
     SpanAcc* spans = span_tab();
-    for (uint32_t k = tid; k < ARGUS_MAX_PHASES; k += NT) {
+    for (uint32_t k = tid; k < ARGUS_MAX_PHASES; k += (CW + 1) * 32) {
       spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
     }
   }
   __syncthreads();
 
-  uint64_t policy = 0;
-  if (tid == 0) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
-  auto issue = [&](uint32_t s, uint32_t slot) {  // thread 0 only: stage s into ring slot `slot`
-    const uint32_t cnt = (n_ev - s * SUB < (uint32_t)SUB) ? n_ev - s * SUB : (uint32_t)SUB;
-    const uint32_t bar = smem_u32(&H->bars[slot]);
-    mbar_expect_tx(bar, cnt * 32u);
-    tma_load_1d(smem_u32(smem + stages + slot * (SUB * 32u)), src + 2 * (size_t)s * SUB, cnt * 32u, bar, policy);
-  };
-  if (tid == 0)
-    for (uint32_t s = 0; s < (uint32_t)K && s < n_sub; ++s) issue(s, s);
+  if (warp == CW) {
+    // ---- producer warp: one lane streams the CTA's span through the ring with TMA bulk copies ----
+    if (lane == 0) {
+      uint64_t policy;
+      asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
+      uint32_t slot = 0, round = 0;
+      for (uint32_t s = 0; s < n_sub; ++s) {
+        if (round) mbar_wait(smem_u32(&H->empty[slot]), (round - 1u) & 1u);
+        const uint32_t cnt = (n_ev - s * SUBE < (uint32_t)SUBE) ? n_ev - s * SUBE : (uint32_t)SUBE;
+        const uint32_t bar = smem_u32(&H->full[slot]);
+        mbar_expect_tx(bar, cnt * 32u);
+        tma_load_1d(smem_u32(smem + stages + slot * (SUBE * 32u)), src + 2 * (size_t)s * SUBE,
+                    cnt * 32u, bar, policy);
+        if (++slot == (uint32_t)K) { slot = 0; ++round; }
+      }
+    }
+    return;
+  }
 
+  // ---- consumer warps -----------------------------------------------------------------------------
   WarpSpan ws;
   ws.reset();
-  uint32_t cur_key = KEY_NONE;
+  uint32_t cur_key = KEY_NONE, live = 0u;
   uint32_t n_invalid = 0;
-  // ring position of stage it*G + tid/SUB (this thread's first stage); the others follow at +WPS
-  uint32_t slot0 = (uint32_t)(tid / SUB) % (uint32_t)K, par0 = 0;
-  uint32_t base_slot = 0;
+  const uint32_t grp = (uint32_t)warp / WPSTG, wis = (uint32_t)warp % WPSTG;   // stage group, warp in stage
+  uint32_t slot = grp % (uint32_t)K, par = (grp / (uint32_t)K) & 1u;
 
   for (uint32_t it = 0; it < n_iter; ++it) {
-    // ---- load phase: EPT events per thread, stage -> registers ---------------------------------
-    uint32_t sig[EPT], phase[EPT], key[EPT];
-    long long start[EPT], end[EPT];
-    bool pending[EPT];
-    {
-      uint32_t sl = slot0, pr = par0;
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        const uint32_t s = it * G + (uint32_t)(e * WPS + tid / SUB);
-        const uint32_t idx = it * (EPT * NT) + (uint32_t)(e * NT + tid);
-        pending[e] = false; sig[e] = 0; phase[e] = 0; key[e] = KEY_NONE; start[e] = 0; end[e] = 0;
-        if (s < n_sub) {
-          mbar_wait(smem_u32(&H->bars[sl]), pr);
-          if (idx < n_ev) {
-            // lanes 0-3,8-11,.. read the first half first, the others the second: conflict-free LDS.128
-            const uint4* p = reinterpret_cast<const uint4*>(smem + stages + sl * (SUB * 32u)) + 2 * (tid % SUB);
-            const int h = (lane >> 2) & 1;
-            const uint4 a = p[h], b = p[h ^ 1];
-            const uint4 lo = h ? b : a, hi = h ? a : b;
-            sig[e] = lo.z; phase[e] = lo.w >> 16;
-            start[e] = (long long)(((unsigned long long)hi.y << 32) | hi.x);
-            end[e] = (long long)(((unsigned long long)hi.w << 32) | hi.z);
-            pending[e] = argus_event_key(D, lo.x, lo.y, lo.z, phase[e], start[e], end[e], key[e]);
-            n_invalid += pending[e] ? 0u : 1u;
-          }
-        }
-        sl += WPS; if (sl >= (uint32_t)K) { sl -= (uint32_t)K; pr ^= 1u; }
-      }
-      slot0 = sl; par0 = pr;     // EPT*WPS = G stages further
-    }
-    __syncthreads();   // every thread holds its events: the G stages can be refilled right away
-    if (tid == 0) {
-      uint32_t sl = base_slot;
-#pragma unroll 1
-      for (uint32_t g = 0; g < (uint32_t)G; ++g) {
-        const uint32_t sn = it * G + (uint32_t)K + g;
-        if (sn < n_sub) issue(sn, sl);
-        if (++sl == (uint32_t)K) sl = 0;
-      }
-    }
-    base_slot += G; if (base_slot >= (uint32_t)K) base_slot -= (uint32_t)K;
-
-    uint32_t ovf_mask = 0;
+    // ---- load: one event per lane, stage -> registers; release the stage at once --------------------
+    const uint32_t s = it * SPI + grp;
+    const uint32_t idx = it * NC + (uint32_t)tid;
+    const uint32_t my_pos = it * NC + (uint32_t)warp * 32u;     // first event of this warp's chunk
+    uint32_t sig = 0, phase = 0, key = KEY_NONE;
+    long long start = 0, end = 0;
+    bool pending = false;
+    // A warp beyond the requested rendezvous position joins it BEFORE taking its next chunk (also
+    // while it waits for data: a parked warp keeps its next stage unreleased, which may stall the
+    // in-order producer).  Warps before that position go on: their stages are always issued.
     for (;;) {
-      bool accept[EPT];
-      uint4 snap[EPT];
-      uint2 mmv[EPT];
-      // ---- table loads for all accepted events first (ILP), then the atomics ---------------------
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        accept[e] = pending[e] && key[e] == cur_key;
-        if (accept[e]) { snap[e] = *tb.slots(sig[e]); mmv[e] = *tb.mm(sig[e]); }
-      }
-      // ---- spans: warp-uniform fast path in registers, else per-phase ballot groups ---------------
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        const uint32_t ph0 = __shfl_sync(FULL, phase[e], 0);
-        if (__all_sync(FULL, accept[e] && phase[e] == ph0)) {
-          if (ws.phase != ph0) { ws.flush(lane); ws.phase = ph0; }
-          ws.mn = start[e] < ws.mn ? start[e] : ws.mn;
-          ws.mx = end[e] > ws.mx ? end[e] : ws.mx;
-          ws.n++;
-        } else {
-          uint32_t todo = __ballot_sync(FULL, accept[e]);
-          while (todo) {
-            const int leader = __ffs((int)todo) - 1;
-            const uint32_t ph = __shfl_sync(FULL, phase[e], leader);
-            const bool mine = accept[e] && phase[e] == ph;
-            const uint32_t grp = __ballot_sync(FULL, mine);
-            const long long a = warp_min_i64(mine ? start[e] : INT64_MAX);
-            const long long b = warp_max_i64(mine ? end[e] : INT64_MIN);
-            if (lane == leader) {
-              SpanAcc* sp = span_tab() + ph;
-              atomicMin(&sp->mn, a);
-              atomicMax(&sp->mx, b);
-              atomicAdd(&sp->n, (unsigned long long)__popc(grp));
-            }
-            todo &= ~grp;
-          }
-        }
-      }
-      // ---- cells ------------------------------------------------------------------------------------
-      uint32_t d32[EPT], old[EPT];
-      bool fits[EPT];
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        const unsigned long long d = (unsigned long long)(end[e] - start[e]);
-        d32[e] = (uint32_t)d;
-        fits[e] = accept[e] && (d >> 32) == 0ull;
-        if (fits[e]) {
-          const uint32_t tag = (31u - (uint32_t)__clz((int)(d32[e] | 1u))) + 1u;  // bucket + 1
-          fits[e] = slot_update(tb, sig[e], tag, snap[e]);
-        }
-        if (accept[e] && !fits[e]) { ovf_mask |= 1u << e; H->flags = 1u; }
-      }
-#pragma unroll
-      for (int e = 0; e < EPT; ++e)
-        if (fits[e]) old[e] = atomicAdd(tb.sum_lo(sig[e]), d32[e]);
-#pragma unroll
-      for (int e = 0; e < EPT; ++e)
-        if (fits[e]) {
-          if (~d32[e] > mmv[e].x) atomicMax(&tb.mm(sig[e])->x, ~d32[e]);
-          if (d32[e] > mmv[e].y) atomicMax(&tb.mm(sig[e])->y, d32[e]);
-        }
-      bool pend = false;
-#pragma unroll
-      for (int e = 0; e < EPT; ++e) {
-        if (fits[e] && old[e] + d32[e] < old[e]) atomicAdd(tb.sum_hi(sig[e]), 1u);
-        if (accept[e]) pending[e] = false;
-        pend |= pending[e];
-      }
-      const int any_pending = __syncthreads_or(pend ? 1 : 0);
-      if (H->flags) {  // uniform: written before the barrier
-        // rare: some event does not fit the compact cell -> make the record live, then L2 atomics
+      if (*reinterpret_cast<volatile uint32_t*>(&H->next_idx) < my_pos) {
         ws.flush(lane);
-        flush_table<NT>(gl, cur_key);
-#pragma unroll
-        for (int e = 0; e < EPT; ++e)
-          if (ovf_mask & (1u << e)) {
-            // the span part was already folded above; only the cell goes the global way
-            uint8_t* rec = records + (size_t)cur_key * D.rec_bytes;
-            const uint64_t d = (uint64_t)(end[e] - start[e]);
-            argus_cell* cl = reinterpret_cast<argus_cell*>(rec + D.cell_off) + sig[e];
-            atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
-            atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), (unsigned long long)d);
-            atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), (unsigned long long)d);
-            atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), (unsigned long long)d);
-            atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
+        const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
+        cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
+        continue;
+      }
+      if (s >= n_sub || mbar_try_wait(smem_u32(&H->full[slot]), par)) break;
+    }
+    if (s < n_sub) {
+      if (idx < n_ev) {
+        const uint4* p = reinterpret_cast<const uint4*>(smem + stages + slot * (SUBE * 32u)) + 2 * (wis * 32u + lane);
+#if ARGUS_SEG_SWIZZLED_LOAD
+        // lanes 0-3,8-11,.. read the first half first, the others the second: conflict-free LDS.128
+        const int h = (lane >> 2) & 1;
+        const uint4 a = p[h], b = p[h ^ 1];
+        const uint4 lo = h ? b : a, hi = h ? a : b;
+#else
+        const uint4 lo = p[0], hi = p[1];
+#endif
+        sig = lo.z; phase = lo.w >> 16;
+        start = (long long)(((unsigned long long)hi.y << 32) | hi.x);
+        end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
+        pending = argus_event_key(D, lo.x, lo.y, lo.z, phase, start, end, key);
+        n_invalid += pending ? 0u : 1u;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&H->empty[slot]));
+    }
+    slot += SPI; if (slot >= (uint32_t)K) { slot -= (uint32_t)K; par ^= 1u; }
+
+    for (;;) {
+      // ---- cells -----------------------------------------------------------------------------------
+      const bool accept = pending && key == cur_key;
+      bool ok = false;
+      if (accept) {
+        const unsigned long long d = (unsigned long long)(end - start);
+        const uint32_t d32 = (uint32_t)d;
+        bool fits = (d >> 32) == 0ull;
+        if (fits) {
+          const uint32_t tag = (31u - (uint32_t)__clz((int)(d32 | 1u))) + 1u;  // bucket + 1
+          const uint4 snap = *tb.slots(sig);
+          const uint2 mmv = *tb.mm(sig);
+          fits = slot_update(tb, sig, tag, snap);
+          if (fits) {
+            const uint32_t old = atomicAdd(tb.sum_lo(sig), d32);
+            if (~d32 > mmv.x) atomicMax(&tb.mm(sig)->x, ~d32);
+            if (d32 > mmv.y) atomicMax(&tb.mm(sig)->y, d32);
+            if (old + d32 < old) atomicAdd(tb.sum_hi(sig), 1u);
+            ok = true;
           }
-        ovf_mask = 0;
-        if (tid == 0) H->flags = 0u;
-        __syncthreads();
+        }
+        if (!fits && live) {
+          // the compact cell cannot take this event and the record is live: L2 atomics
+          argus_cell* cl = reinterpret_cast<argus_cell*>(records + (size_t)cur_key * D.rec_bytes + D.cell_off) + sig;
+          atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
+          atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), d);
+          atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), d);
+          atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), d);
+          atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
+          ok = true;
+        }
       }
-      if (!any_pending) break;
-      // ---- key switch: flush the finished record, adopt the key of the first pending event --------
-      if (cur_key != KEY_NONE) { ws.flush(lane); flush_table<NT>(gl, cur_key); }
-#pragma unroll
-      for (int e = EPT - 1; e >= 0; --e)
-        if (pending[e]) atomicMin(&H->next_idx, (uint32_t)(e * NT + tid));
-      __syncthreads();
-      {
-        const uint32_t pick = H->next_idx;
-#pragma unroll
-        for (int e = 0; e < EPT; ++e)
-          if ((uint32_t)(e * NT + tid) == pick) H->cur_key = key[e];
+      // ---- spans of the folded events: warp-uniform fast path in registers, else ballot groups ------
+      const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
+      if (__all_sync(FULL, ok && phase == ph0)) {
+        if (ws.phase != ph0) { ws.flush(lane); ws.phase = ph0; }
+        ws.mn = start < ws.mn ? start : ws.mn;
+        ws.mx = end > ws.mx ? end : ws.mx;
+        ws.n++;
+      } else {
+        uint32_t todo = __ballot_sync(FULL, ok);
+        while (todo) {
+          const int leader = __ffs((int)todo) - 1;
+          const uint32_t ph = __shfl_sync(FULL, phase, leader);
+          const bool mine = ok && phase == ph;
+          const uint32_t g2 = __ballot_sync(FULL, mine);
+          const long long a = warp_min_i64(mine ? start : INT64_MAX);
+          const long long b = warp_max_i64(mine ? end : INT64_MIN);
+          if (lane == leader) {
+            SpanAcc* sp = span_tab() + ph;
+            atomicMin(&sp->mn, a);
+            atomicMax(&sp->mx, b);
+            atomicAdd(&sp->n, (unsigned long long)__popc(g2));
+          }
+          todo &= ~g2;
+        }
       }
-      __syncthreads();
-      cur_key = H->cur_key;
-      if (tid == 0) H->next_idx = KEY_NONE;
-      // (next_idx is next read after at least one more barrier)
+      if (ok) pending = false;
+      if (!__any_sync(FULL, pending)) break;
+      ws.flush(lane);
+      const unsigned long long r = park<NC>(gl, pending, key, idx, cur_key, live);
+      cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
     }
   }
-  if (cur_key != KEY_NONE) { ws.flush(lane); flush_table<NT>(gl, cur_key); }
+  // ---- out of events: keep joining the rendezvous until every warp is done ---------------------------
+  ws.flush(lane);
+  if (lane == 0) atomicAdd(&H->n_finished, 1u);
+  for (;;) {
+    const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
+    if (r & PARK_DONE) break;
+    cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
+  }
 
   n_invalid = __reduce_add_sync(FULL, n_invalid);
   if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
-  if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // valid = seen - invalid (host)
+  if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
 }
 
-template <int NT, int EPT>
+template <int CW, int WPSTG>
 cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records,
                            cudaStream_t s) {
-  constexpr int G = EPT * NT / SUB;
+  constexpr int SPI = CW / WPSTG;
+  constexpr size_t STAGE_BYTES = (size_t)WPSTG * 32 * 32;
   const size_t fixed = stage_off(ctx->dims.S);
-  int K = (int)(((size_t)ctx->max_smem_optin - fixed) / ((size_t)SUB * 32));
+  int K = (int)(((size_t)ctx->max_smem_optin - fixed) / STAGE_BYTES);
   if (K > MAXK) K = MAXK;
-  if (K < G) return cudaErrorInvalidConfiguration;
-  const size_t smem_bytes = fixed + (size_t)K * SUB * 32;
-  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<NT, EPT>,
+  if (K < 2 * SPI + 1) return cudaErrorInvalidConfiguration;
+  const size_t smem_bytes = fixed + (size_t)K * STAGE_BYTES;
+  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
   if (e != cudaSuccess) return e;
   int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count;
   // a CTA's slot counters hold 26 bits between flushes: bound the span of one CTA
-  const uint64_t tile = (uint64_t)EPT * NT;
+  const uint64_t tile = (uint64_t)CW * 32;
   const uint64_t cap = (1ull << 26) - tile;
   uint64_t per_cta = (n + grid - 1) / grid;
   if (per_cta > cap) per_cta = cap;
   per_cta = (per_cta + tile - 1) / tile * tile;
   const uint64_t ctas = (n + per_cta - 1) / per_cta;
-  aggregate_seg_kernel<NT, EPT><<<(unsigned)ctas, NT, smem_bytes, s>>>(
+  aggregate_seg_kernel<CW, WPSTG><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
       ctx->d_counters, ctx->dims, K);
   return cudaGetLastError();
@@ -538,20 +580,20 @@ cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, vo
 }  // namespace
 
 bool argus_seg_supported(const argus_ctx* ctx) {
-  // the smallest variant consumes 4 stages (32 KB) per iteration
-  return (size_t)stage_off(ctx->dims.S) + (size_t)8 * SUB * 32 <= (size_t)ctx->max_smem_optin;
+  // default variant: 4 KB stages, 6 per iteration, at least 13 in the ring
+  return (size_t)stage_off(ctx->dims.S) + (size_t)13 * 4096 <= (size_t)ctx->max_smem_optin;
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
                                        void* d_records, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
   switch (ctx->tune_variant) {
-    case 1: return launch_variant<1024, 1>(ctx, ev, n, d_records, s);
-    case 2: return launch_variant<1024, 2>(ctx, ev, n, d_records, s);
-    case 3: return launch_variant<512, 2>(ctx, ev, n, d_records, s);
-    case 5: return launch_variant<256, 8>(ctx, ev, n, d_records, s);
-    case 6: return launch_variant<768, 2>(ctx, ev, n, d_records, s);
-    case 4:
-    default: return launch_variant<512, 4>(ctx, ev, n, d_records, s);
+    case 1: return launch_variant<16, 4>(ctx, ev, n, d_records, s);
+    case 2: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
+    case 3: return launch_variant<28, 4>(ctx, ev, n, d_records, s);
+    case 4: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
+    case 5: return launch_variant<30, 2>(ctx, ev, n, d_records, s);
+    case 6: return launch_variant<20, 4>(ctx, ev, n, d_records, s);
+    default: return launch_variant<24, 4>(ctx, ev, n, d_records, s);
   }
 }
