@@ -104,11 +104,11 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
   asm volatile(
       "{\n"
       ".reg .pred P1;\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2, %3;\n"
       "selp.u32 %0, 1, 0, P1;\n"
       "}"
       : "=r"(ok)
-      : "r"(bar), "r"(parity)
+      : "r"(bar), "r"(parity), "r"(2000u)   // suspend-time hint (ns): fewer wasted polls while waiting
       : "memory");
   return ok != 0u;
 }
@@ -143,7 +143,7 @@ struct WarpSpan {
   __device__ __forceinline__ void flush(int lane) {
     if (phase != KEY_NONE) {
       long long a = warp_min_i64(mn), b = warp_max_i64(mx);
-      uint32_t c = __reduce_add_sync(FULL, n);
+      const uint32_t c = n;              // warp-uniform
       if (lane == 0 && c) {
         SpanAcc* sp = span_tab() + phase;
         atomicMin(&sp->mn, a);
@@ -429,28 +429,28 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   uint32_t n_invalid = 0;
   const uint32_t grp = (uint32_t)warp / WPSTG, wis = (uint32_t)warp % WPSTG;   // stage group, warp in stage
   uint32_t slot = grp % (uint32_t)K, par = (grp / (uint32_t)K) & 1u;
+  uint32_t s = grp;                              // this warp's stage of the current iteration
+  uint32_t my_pos = (uint32_t)warp * 32u;        // first event of this warp's chunk
 
   for (uint32_t it = 0; it < n_iter; ++it) {
+    const uint32_t idx = my_pos + (uint32_t)lane;
     // ---- load: one event per lane, stage -> registers; release the stage at once --------------------
-    const uint32_t s = it * SPI + grp;
-    const uint32_t idx = it * NC + (uint32_t)tid;
-    const uint32_t my_pos = it * NC + (uint32_t)warp * 32u;     // first event of this warp's chunk
+    const bool have = s < n_sub;                 // this warp's stage exists (warp-uniform)
     uint32_t sig = 0, phase = 0, key = KEY_NONE;
     long long start = 0, end = 0;
     bool pending = false;
-    // A warp beyond the requested rendezvous position joins it BEFORE taking its next chunk (also
-    // while it waits for data: a parked warp keeps its next stage unreleased, which may stall the
-    // in-order producer).  Warps before that position go on: their stages are always issued.
-    for (;;) {
+    // While a warp waits for data it watches the rendezvous request: a warp beyond the requested
+    // position joins the rendezvous BEFORE taking its next chunk (a parked warp keeps its next
+    // stage unreleased, which may stall the in-order producer, so nobody may wait for data while
+    // others wait for him).  Warps before that position go on: their stages are always issued.
+    while (have && !mbar_try_wait(smem_u32(&H->full[slot]), par)) {
       if (*reinterpret_cast<volatile uint32_t*>(&H->next_idx) < my_pos) {
         ws.flush(lane);
         const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
         cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
-        continue;
       }
-      if (s >= n_sub || mbar_try_wait(smem_u32(&H->full[slot]), par)) break;
     }
-    if (s < n_sub) {
+    if (have) {
       if (idx < n_ev) {
         const uint4* p = reinterpret_cast<const uint4*>(smem + stages + slot * (SUBE * 32u)) + 2 * (wis * 32u + lane);
 #if ARGUS_SEG_SWIZZLED_LOAD
@@ -471,6 +471,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       if (lane == 0) mbar_arrive(smem_u32(&H->empty[slot]));
     }
     slot += SPI; if (slot >= (uint32_t)K) { slot -= (uint32_t)K; par ^= 1u; }
+    s += SPI; my_pos += NC;
 
     for (;;) {
       // ---- cells -----------------------------------------------------------------------------------
@@ -487,8 +488,10 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
           fits = slot_update(tb, sig, tag, snap);
           if (fits) {
             const uint32_t old = atomicAdd(tb.sum_lo(sig), d32);
-            if (~d32 > mmv.x) atomicMax(&tb.mm(sig)->x, ~d32);
-            if (d32 > mmv.y) atomicMax(&tb.mm(sig)->y, d32);
+            if ((~d32 > mmv.x) | (d32 > mmv.y)) {   // a new extreme: rare once a cell has a few events
+              atomicMax(&tb.mm(sig)->x, ~d32);
+              atomicMax(&tb.mm(sig)->y, d32);
+            }
             if (old + d32 < old) atomicAdd(tb.sum_hi(sig), 1u);
             ok = true;
           }
@@ -510,7 +513,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
         if (ws.phase != ph0) { ws.flush(lane); ws.phase = ph0; }
         ws.mn = start < ws.mn ? start : ws.mn;
         ws.mx = end > ws.mx ? end : ws.mx;
-        ws.n++;
+        ws.n += 32u;                       // warp-uniform count
       } else {
         uint32_t todo = __ballot_sync(FULL, ok);
         while (todo) {
@@ -580,20 +583,20 @@ cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, vo
 }  // namespace
 
 bool argus_seg_supported(const argus_ctx* ctx) {
-  // default variant: 4 KB stages, 6 per iteration, at least 13 in the ring
-  return (size_t)stage_off(ctx->dims.S) + (size_t)13 * 4096 <= (size_t)ctx->max_smem_optin;
+  // default variant: 6 KB stages, 5 per iteration, at least 11 in the ring
+  return (size_t)stage_off(ctx->dims.S) + (size_t)11 * 6144 <= (size_t)ctx->max_smem_optin;
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
                                        void* d_records, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
   switch (ctx->tune_variant) {
-    case 1: return launch_variant<16, 4>(ctx, ev, n, d_records, s);
-    case 2: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
-    case 3: return launch_variant<28, 4>(ctx, ev, n, d_records, s);
+    case 1: return launch_variant<30, 10>(ctx, ev, n, d_records, s);
+    case 2: return launch_variant<30, 15>(ctx, ev, n, d_records, s);
+    case 3: return launch_variant<28, 7>(ctx, ev, n, d_records, s);
     case 4: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
-    case 5: return launch_variant<30, 2>(ctx, ev, n, d_records, s);
-    case 6: return launch_variant<20, 4>(ctx, ev, n, d_records, s);
-    default: return launch_variant<24, 4>(ctx, ev, n, d_records, s);
+    case 5: return launch_variant<31, 31>(ctx, ev, n, d_records, s);
+    case 6: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
+    default: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
   }
 }
