@@ -41,7 +41,7 @@ def measured_peak_gbs():
 
 def profile_traffic_bytes(workload: str):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", f"r1_{workload}_dram.txt")
+    p = os.path.join(ROOT, "profiles", f"{workload}_seg_traffic.txt")
     try:
         with open(p) as f:
             for line in f:
