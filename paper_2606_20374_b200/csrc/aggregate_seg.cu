@@ -4,18 +4,22 @@
 // reductions where a block spans rank-step boundaries, and flush to global in one pass").
 //
 // One persistent CTA per SM walks a contiguous span of the event buffer.  Events arrive through a
-// ring of 8 KB stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx, L2
-// evict-first).  Each thread takes EPT events per iteration into registers; the stages are
-// refilled right after that load phase, so the whole ring is in flight while the CTA accumulates.
+// ring of shared-memory stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier
+// complete_tx, L2 evict-first) issued by a producer warp; each consumer lane takes one event per
+// iteration into registers and releases the stage at once.
 // The CTA keeps ONE (rank, step) table in shared memory at a time, 32 bytes per sig, laid out as
 // structure-of-arrays so that random sigs spread over all 32 banks:
-//   slots[S]  uint4: four tagged histogram slots {bucket+1 : 6 bits | count : 26 bits}; the word
-//                    a slot lives in is XOR-swizzled with sig bits 3-4
+//   slots[S]  uint4: four histogram counters, DIRECT-MAPPED by bucket & 3
 //   sum_lo[S], sum_hi[S] u32: the 64-bit sum with an explicit carry
-//   mm[S]     uint2: {~min, max} as u32
-// Only native 32-bit shared atomics are used (64-bit shared atomics are CAS loops on sm_100a).
-// An event the compact cell cannot take (duration >= 2^32 ns, or a fifth distinct bucket of one
-// sig) goes straight to the global record with L2 atomics.  When the (rank, step) key changes the
+//   mm[S]     u64 {~min : 32 | max : 32} (0 = empty cell)
+// Invariant of a compact cell: bucket(max) - bucket(min) <= 3, so the (at most four) occupied
+// buckets are consecutive and bucket & 3 names each of them uniquely — no tags, no lookup.  An
+// event inside [min, max] (the common case, checked with one 64-bit load) can never break the
+// invariant; an event that would extend the range goes through a 64-bit CAS that refuses the
+// extension when the invariant would break.  Only native 32-bit shared atomics are used on the
+// hot path (64-bit shared atomic adds are CAS loops on sm_100a).
+// An event the compact cell cannot take (duration >= 2^32 ns, or a range wider than four buckets)
+// goes straight to the global record with L2 atomics.  When the (rank, step) key changes the
 // table is flushed: the first CTA to reach a record claims it and writes the whole 160-byte cells
 // with coalesced 128-bit stores (no read-modify-write, no separate identity fill); any later
 // contribution to the same record merges with L2 reductions.  Correct for ANY event order; fast
@@ -161,56 +165,90 @@ struct Glob {             // global-memory side of the kernel
   argus_dims D;
 };
 
-// Histogram part of one event: bump the slot tagged bucket+1, claiming one if needed.
-// `s` is a (possibly stale) snapshot of the sig's four slot words.  Returns false if all four
-// slots hold other buckets.
-__device__ __forceinline__ bool slot_update(const Table& tb, uint32_t sig, uint32_t tag, const uint4& s) {
-  uint32_t* w = tb.slot_words(sig);
-  int p = -1;
-  if ((s.x & 63u) == tag) p = 0;
-  else if ((s.y & 63u) == tag) p = 1;
-  else if ((s.z & 63u) == tag) p = 2;
-  else if ((s.w & 63u) == tag) p = 3;
-  if (p >= 0) {
-    atomicAdd(w + p, 64u);
-    return true;
-  }
-  // claim (first events of a bucket in this rank-step).  Slots are claimed in a fixed per-sig
-  // order (logical j -> word j ^ swz) and never released before the flush, so a tag lives in at
-  // most one slot.  The swizzle spreads the first-claimed (hottest) slot over all banks.
-  const int swz = (int)((sig >> 3) & 3u);
-#pragma unroll 1
-  for (int j = 0; j < 4; ++j) {
-    uint32_t* q = w + (j ^ swz);
-    uint32_t v = *reinterpret_cast<volatile uint32_t*>(q);
-    if (v == 0u) {
-      v = atomicCAS(q, 0u, tag | 64u);
-      if (v == 0u) return true;
-    }
-    if ((v & 63u) == tag) { atomicAdd(q, 64u); return true; }
-  }
-  return false;
+// ---- shared-memory accessors on 32-bit shared-window addresses (no generic-address arithmetic) ----
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint2 lds64(uint32_t a) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void reds_add(uint32_t a, uint32_t v) {
+  asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t atoms_add(uint32_t a, uint32_t v) {
+  uint32_t o;
+  asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory");
+  return o;
+}
+__device__ __forceinline__ unsigned long long atoms_cas64(uint32_t a, unsigned long long cmp,
+                                                          unsigned long long val) {
+  unsigned long long o;
+  asm volatile("atom.shared.cas.b64 %0, [%1], %2, %3;" : "=l"(o) : "r"(a), "l"(cmp), "l"(val) : "memory");
+  return o;
+}
+__device__ __forceinline__ uint32_t bucket32(uint32_t d) {   // R4 for d < 2^32: floor(log2 d), 0 for d <= 1
+  return 31u - (uint32_t)__clz((int)(d | 1u));
 }
 
-// 16-byte chunk `part` (0..9) of the 160-byte argus_cell decoded from a compact cell.
+// Rare path of the compact cell: the event's duration d lies outside the cell's [min, max] (or the
+// cell is empty).  Extend the range with a 64-bit CAS unless that would spread the cell over more
+// than four consecutive buckets; returns false then (the event takes the global path instead).
+__device__ __noinline__ bool mm_extend(uint32_t a_mm, uint32_t d) {
+  const uint2 o2 = lds64(a_mm);
+  unsigned long long old = ((unsigned long long)o2.y << 32) | o2.x;
+  for (;;) {
+    const uint32_t nmin = (uint32_t)old, mx = (uint32_t)(old >> 32);
+    const uint32_t nn = nmin > ~d ? nmin : ~d, nx = mx > d ? mx : d;
+    if (bucket32(nx) - bucket32(~nn) > 3u) return false;
+    const unsigned long long nw = ((unsigned long long)nx << 32) | nn;
+    if (nw == old) return true;
+    const unsigned long long prev = atoms_cas64(a_mm, old, nw);
+    if (prev == old) return true;
+    old = prev;
+  }
+}
+
+// One event straight into the LIVE global record (the compact cell refused it).
+__device__ __noinline__ void global_cell_add(uint8_t* records, const argus_dims& D, uint32_t key,
+                                             uint32_t sig, unsigned long long d) {
+  argus_cell* cl = reinterpret_cast<argus_cell*>(records + (size_t)key * D.rec_bytes + D.cell_off) + sig;
+  atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
+  atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), d);
+  atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), d);
+  atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), d);
+  atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
+}
+
+// 16-byte chunk `part` (0..9) of the 160-byte argus_cell decoded from a compact cell:
+// s = the four direct-mapped counters, m = {~min, max} (0, 0 = empty).
 __device__ __forceinline__ uint4 cell_chunk(const uint4 s, uint32_t sum_lo, uint32_t sum_hi,
                                             const uint2 m, uint32_t part) {
-  const uint32_t c0 = s.x >> 6, c1 = s.y >> 6, c2 = s.z >> 6, c3 = s.w >> 6;
   if (part == 0u) {
-    unsigned long long cnt = (unsigned long long)c0 + c1 + c2 + c3;
+    const unsigned long long cnt = (unsigned long long)s.x + s.y + s.z + s.w;
     return make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), sum_lo, sum_hi);
   }
+  const bool empty = (m.x | m.y) == 0u;
   if (part == 1u) {
-    if ((c0 | c1 | c2 | c3) == 0u) return make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u);
+    if (empty) return make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u);
     return make_uint4(~m.x, 0u, m.y, 0u);
   }
-  const uint32_t b0 = 4u * (part - 2u) + 1u;  // tag of the chunk's first bucket
-  const uint32_t t0 = s.x & 63u, t1 = s.y & 63u, t2 = s.z & 63u, t3 = s.w & 63u;
+  if (empty) return make_uint4(0u, 0u, 0u, 0u);
+  const uint32_t bl = bucket32(~m.x), bh = bucket32(m.y);
+  const uint32_t b0 = 4u * (part - 2u);       // bucket b0 + j lives in counter j (b0 is a multiple of 4)
   uint4 v;
-  v.x = (t0 == b0 ? c0 : 0u) + (t1 == b0 ? c1 : 0u) + (t2 == b0 ? c2 : 0u) + (t3 == b0 ? c3 : 0u);
-  v.y = (t0 == b0 + 1 ? c0 : 0u) + (t1 == b0 + 1 ? c1 : 0u) + (t2 == b0 + 1 ? c2 : 0u) + (t3 == b0 + 1 ? c3 : 0u);
-  v.z = (t0 == b0 + 2 ? c0 : 0u) + (t1 == b0 + 2 ? c1 : 0u) + (t2 == b0 + 2 ? c2 : 0u) + (t3 == b0 + 2 ? c3 : 0u);
-  v.w = (t0 == b0 + 3 ? c0 : 0u) + (t1 == b0 + 3 ? c1 : 0u) + (t2 == b0 + 3 ? c2 : 0u) + (t3 == b0 + 3 ? c3 : 0u);
+  v.x = (b0 >= bl && b0 <= bh) ? s.x : 0u;
+  v.y = (b0 + 1u >= bl && b0 + 1u <= bh) ? s.y : 0u;
+  v.z = (b0 + 2u >= bl && b0 + 2u <= bh) ? s.z : 0u;
+  v.w = (b0 + 3u >= bl && b0 + 3u <= bh) ? s.w : 0u;
   return v;
 }
 
@@ -277,17 +315,17 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
     for (uint32_t sig = tid; sig < D.S; sig += NC) {
       const uint4 s = *tb.slots(sig);
       const uint2 m = *tb.mm(sig);
-      const uint32_t sl[4] = {s.x, s.y, s.z, s.w};
-      unsigned long long cnt = 0;
+      if ((m.x | m.y) != 0u) {
+        const uint32_t sl[4] = {s.x, s.y, s.z, s.w};
+        const uint32_t bl = bucket32(~m.x);
+        unsigned long long cnt = 0;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const uint32_t ck = sl[k] >> 6;
-        if (ck) {
-          atomicAdd(&cells[sig].hist[(sl[k] & 63u) - 1u], ck);
-          cnt += ck;
+        for (uint32_t k = 0; k < 4u; ++k) {
+          if (sl[k]) {
+            atomicAdd(&cells[sig].hist[bl + ((k - bl) & 3u)], sl[k]);   // the bucket >= bl with bucket & 3 == k
+            cnt += sl[k];
+          }
         }
-      }
-      if (cnt) {
         atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].count), cnt);
         atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].sum_ns),
                   ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig));
@@ -423,120 +461,135 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   }
 
   // ---- consumer warps -----------------------------------------------------------------------------
+  // All shared-memory traffic of the hot loop goes through 32-bit shared-window addresses.
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t a_slots = sbase + TAB_OFF, a_sumlo = a_slots + 16u * D.S, a_sumhi = a_slots + 20u * D.S,
+                 a_mm = a_slots + 24u * D.S;
+  const uint32_t a_ring = sbase + stages, ring_bytes = (uint32_t)K * (uint32_t)(SUBE * 32);
+  const uint32_t a_full = smem_u32(&H->full[0]), a_nextidx = smem_u32(&H->next_idx);
+  constexpr uint32_t EMPTY_OFF = MAXK * 8u;          // empty[k] sits MAXK*8 bytes after full[k]
   WarpSpan ws;
   ws.reset();
   uint32_t cur_key = KEY_NONE, live = 0u;
+  uint32_t cur_rank = 0u, cur_step = 0u, s_eff = 0u;   // s_eff = 0 while no key is current: nothing is accepted
   uint32_t n_invalid = 0;
   const uint32_t grp = (uint32_t)warp / WPSTG, wis = (uint32_t)warp % WPSTG;   // stage group, warp in stage
   uint32_t slot = grp % (uint32_t)K, par = (grp / (uint32_t)K) & 1u;
+  uint32_t a_ev = a_ring + slot * (uint32_t)(SUBE * 32) + wis * 1024u + (uint32_t)lane * 32u;
   uint32_t s = grp;                              // this warp's stage of the current iteration
   uint32_t my_pos = (uint32_t)warp * 32u;        // first event of this warp's chunk
+
+#define ARGUS_ADOPT(r)                                                              \
+  do {                                                                              \
+    cur_key = (uint32_t)(r); live = (uint32_t)((r) >> 32) & 1u;                     \
+    if (cur_key != KEY_NONE) {                                                      \
+      cur_rank = cur_key / D.T; cur_step = D.step_base + (cur_key - cur_rank * D.T); \
+      s_eff = D.S;                                                                  \
+    } else { s_eff = 0u; }                                                          \
+  } while (0)
 
   for (uint32_t it = 0; it < n_iter; ++it) {
     const uint32_t idx = my_pos + (uint32_t)lane;
     // ---- load: one event per lane, stage -> registers; release the stage at once --------------------
     const bool have = s < n_sub;                 // this warp's stage exists (warp-uniform)
-    uint32_t sig = 0, phase = 0, key = KEY_NONE;
-    long long start = 0, end = 0;
-    bool pending = false;
     // While a warp waits for data it watches the rendezvous request: a warp beyond the requested
     // position joins the rendezvous BEFORE taking its next chunk (a parked warp keeps its next
     // stage unreleased, which may stall the in-order producer, so nobody may wait for data while
     // others wait for him).  Warps before that position go on: their stages are always issued.
-    while (have && !mbar_try_wait(smem_u32(&H->full[slot]), par)) {
-      if (*reinterpret_cast<volatile uint32_t*>(&H->next_idx) < my_pos) {
+    const uint32_t a_bar = a_full + slot * 8u;
+    while (have && !mbar_try_wait(a_bar, par)) {
+      if (lds32(a_nextidx) < my_pos) {
         ws.flush(lane);
         const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
-        cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
+        ARGUS_ADOPT(r);
       }
     }
+    uint4 lo = make_uint4(0u, 0u, 0u, 0u), hi = make_uint4(0u, 0u, 0u, 0u);
+    const bool mine = have && idx < n_ev;
     if (have) {
-      if (idx < n_ev) {
-        const uint4* p = reinterpret_cast<const uint4*>(smem + stages + slot * (SUBE * 32u)) + 2 * (wis * 32u + lane);
-#if ARGUS_SEG_SWIZZLED_LOAD
-        // lanes 0-3,8-11,.. read the first half first, the others the second: conflict-free LDS.128
-        const int h = (lane >> 2) & 1;
-        const uint4 a = p[h], b = p[h ^ 1];
-        const uint4 lo = h ? b : a, hi = h ? a : b;
-#else
-        const uint4 lo = p[0], hi = p[1];
-#endif
-        sig = lo.z; phase = lo.w >> 16;
-        start = (long long)(((unsigned long long)hi.y << 32) | hi.x);
-        end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
-        pending = argus_event_key(D, lo.x, lo.y, lo.z, phase, start, end, key);
-        n_invalid += pending ? 0u : 1u;
-      }
+      lo = lds128(a_ev);
+      hi = lds128(a_ev + 16u);
       __syncwarp();
-      if (lane == 0) mbar_arrive(smem_u32(&H->empty[slot]));
+      if (lane == 0) mbar_arrive(a_bar + EMPTY_OFF);
     }
-    slot += SPI; if (slot >= (uint32_t)K) { slot -= (uint32_t)K; par ^= 1u; }
+    slot += SPI; a_ev += (uint32_t)(SPI * SUBE * 32);
+    if (slot >= (uint32_t)K) { slot -= (uint32_t)K; par ^= 1u; a_ev -= ring_bytes; }
     s += SPI; my_pos += NC;
+
+    // ---- decode.  Fast test first: the event belongs to the current key and fits a compact cell
+    // (same rank and step words as the current key, sig and phase in range, both timestamps
+    // non-negative, 0 <= end - start < 2^32).  Everything else is sorted out on the slow side.
+    const uint32_t sig = lo.z, phase = lo.w >> 16;
+    const long long start = (long long)(((unsigned long long)hi.y << 32) | hi.x);
+    const long long end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
+    const unsigned long long d = (unsigned long long)(end - start);
+    const uint32_t d32 = (uint32_t)d;
+    bool fast = mine & (lo.x == cur_rank) & (lo.y == cur_step) & (sig < s_eff) & (phase < D.P) &
+                ((int)(hi.y | hi.w) >= 0) & ((uint32_t)(d >> 32) == 0u);
+    bool pending = fast;
+    uint32_t key = cur_key;
+    if (!__all_sync(FULL, fast)) {
+      // full validity (R2, R3) of the lanes that failed the fast test
+      pending = mine && argus_event_key(D, lo.x, lo.y, sig, phase, start, end, key);
+      n_invalid += (mine && !pending) ? 1u : 0u;
+      fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
+    }
 
     for (;;) {
       // ---- cells -----------------------------------------------------------------------------------
-      const bool accept = pending && key == cur_key;
       bool ok = false;
-      if (accept) {
-        const unsigned long long d = (unsigned long long)(end - start);
-        const uint32_t d32 = (uint32_t)d;
-        bool fits = (d >> 32) == 0ull;
-        if (fits) {
-          const uint32_t tag = (31u - (uint32_t)__clz((int)(d32 | 1u))) + 1u;  // bucket + 1
-          const uint4 snap = *tb.slots(sig);
-          const uint2 mmv = *tb.mm(sig);
-          fits = slot_update(tb, sig, tag, snap);
-          if (fits) {
-            const uint32_t old = atomicAdd(tb.sum_lo(sig), d32);
-            if ((~d32 > mmv.x) | (d32 > mmv.y)) {   // a new extreme: rare once a cell has a few events
-              atomicMax(&tb.mm(sig)->x, ~d32);
-              atomicMax(&tb.mm(sig)->y, d32);
-            }
-            if (old + d32 < old) atomicAdd(tb.sum_hi(sig), 1u);
-            ok = true;
-          }
-        }
-        if (!fits && live) {
-          // the compact cell cannot take this event and the record is live: L2 atomics
-          argus_cell* cl = reinterpret_cast<argus_cell*>(records + (size_t)cur_key * D.rec_bytes + D.cell_off) + sig;
-          atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
-          atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), d);
-          atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), d);
-          atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), d);
-          atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
+      if (fast) {
+        const uint32_t a_m = a_mm + sig * 8u;
+        const uint2 m = lds64(a_m);
+        bool inside = (~d32 <= m.x) & (d32 <= m.y);      // min <= d <= max: the common case
+        if (!inside) inside = mm_extend(a_m, d32);
+        if (inside) {
+          reds_add(a_slots + sig * 16u + ((bucket32(d32) & 3u) << 2), 1u);
+          const uint32_t old = atoms_add(a_sumlo + sig * 4u, d32);
+          if (old + d32 < old) reds_add(a_sumhi + sig * 4u, 1u);
           ok = true;
         }
       }
+      if (!ok && pending && key == cur_key && live) {
+        // the compact cell cannot take this event and the record is live: L2 atomics
+        global_cell_add(records, D, cur_key, sig, d);
+        ok = true;
+      }
       // ---- spans of the folded events: warp-uniform fast path in registers, else ballot groups ------
-      const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
-      if (__all_sync(FULL, ok && phase == ph0)) {
-        if (ws.phase != ph0) { ws.flush(lane); ws.phase = ph0; }
+      if (__all_sync(FULL, ok && phase == ws.phase)) {
         ws.mn = start < ws.mn ? start : ws.mn;
         ws.mx = end > ws.mx ? end : ws.mx;
         ws.n += 32u;                       // warp-uniform count
       } else {
-        uint32_t todo = __ballot_sync(FULL, ok);
-        while (todo) {
-          const int leader = __ffs((int)todo) - 1;
-          const uint32_t ph = __shfl_sync(FULL, phase, leader);
-          const bool mine = ok && phase == ph;
-          const uint32_t g2 = __ballot_sync(FULL, mine);
-          const long long a = warp_min_i64(mine ? start : INT64_MAX);
-          const long long b = warp_max_i64(mine ? end : INT64_MIN);
-          if (lane == leader) {
-            SpanAcc* sp = span_tab() + ph;
-            atomicMin(&sp->mn, a);
-            atomicMax(&sp->mx, b);
-            atomicAdd(&sp->n, (unsigned long long)__popc(g2));
+        ws.flush(lane);
+        const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
+        if (__all_sync(FULL, ok && phase == ph0)) {
+          ws.phase = ph0; ws.mn = start; ws.mx = end; ws.n = 32u;
+        } else {
+          uint32_t todo = __ballot_sync(FULL, ok);
+          while (todo) {
+            const int leader = __ffs((int)todo) - 1;
+            const uint32_t ph = __shfl_sync(FULL, phase, leader);
+            const bool grp_mine = ok && phase == ph;
+            const uint32_t g2 = __ballot_sync(FULL, grp_mine);
+            const long long a = warp_min_i64(grp_mine ? start : INT64_MAX);
+            const long long b = warp_max_i64(grp_mine ? end : INT64_MIN);
+            if (lane == leader) {
+              SpanAcc* sp = span_tab() + ph;
+              atomicMin(&sp->mn, a);
+              atomicMax(&sp->mx, b);
+              atomicAdd(&sp->n, (unsigned long long)__popc(g2));
+            }
+            todo &= ~g2;
           }
-          todo &= ~g2;
         }
       }
-      if (ok) pending = false;
+      if (ok) { pending = false; fast = false; }
       if (!__any_sync(FULL, pending)) break;
       ws.flush(lane);
       const unsigned long long r = park<NC>(gl, pending, key, idx, cur_key, live);
-      cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
+      ARGUS_ADOPT(r);
+      fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
   }
   // ---- out of events: keep joining the rendezvous until every warp is done ---------------------------
@@ -547,6 +600,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     if (r & PARK_DONE) break;
     cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
   }
+#undef ARGUS_ADOPT
 
   n_invalid = __reduce_add_sync(FULL, n_invalid);
   if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
