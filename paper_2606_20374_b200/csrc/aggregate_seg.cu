@@ -24,9 +24,24 @@
 // with coalesced 128-bit stores (no read-modify-write, no separate identity fill); any later
 // contribution to the same record merges with L2 reductions.  Correct for ANY event order; fast
 // when events are grouped by (rank, step) (R18).
+#include <stdio.h>
+
 #include "argus_internal.cuh"
 
 namespace {
+
+// Optional cycle accounting (build with -DARGUS_SEG_PROF; prints from a few CTAs): where consumer
+// warp 0 spends its time — waiting for data, in rendezvous (park), of which flushing.
+#ifdef ARGUS_SEG_PROF
+#define PROF_DECL long long prof_wait = 0, prof_park = 0, prof_t0 = clock64()
+#define PROF_BEGIN(v) const long long v = clock64()
+#define PROF_END(acc, v) acc += clock64() - v
+__device__ long long g_prof_flush[148];
+#else
+#define PROF_DECL
+#define PROF_BEGIN(v)
+#define PROF_END(acc, v)
+#endif
 
 constexpr int MAXK = 48;             // ring stages (bounded by shared memory at launch)
 constexpr uint32_t KEY_NONE = 0xFFFFFFFFu;
@@ -184,6 +199,9 @@ __device__ __forceinline__ uint32_t lds32(uint32_t a) {
 __device__ __forceinline__ void reds_add(uint32_t a, uint32_t v) {
   asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
 }
+__device__ __forceinline__ void reds_max(uint32_t a, uint32_t v) {
+  asm volatile("red.shared.max.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
 __device__ __forceinline__ uint32_t atoms_add(uint32_t a, uint32_t v) {
   uint32_t o;
   asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory");
@@ -228,30 +246,6 @@ __device__ __noinline__ void global_cell_add(uint8_t* records, const argus_dims&
   atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
 }
 
-// 16-byte chunk `part` (0..9) of the 160-byte argus_cell decoded from a compact cell:
-// s = the four direct-mapped counters, m = {~min, max} (0, 0 = empty).
-__device__ __forceinline__ uint4 cell_chunk(const uint4 s, uint32_t sum_lo, uint32_t sum_hi,
-                                            const uint2 m, uint32_t part) {
-  if (part == 0u) {
-    const unsigned long long cnt = (unsigned long long)s.x + s.y + s.z + s.w;
-    return make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), sum_lo, sum_hi);
-  }
-  const bool empty = (m.x | m.y) == 0u;
-  if (part == 1u) {
-    if (empty) return make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u);
-    return make_uint4(~m.x, 0u, m.y, 0u);
-  }
-  if (empty) return make_uint4(0u, 0u, 0u, 0u);
-  const uint32_t bl = bucket32(~m.x), bh = bucket32(m.y);
-  const uint32_t b0 = 4u * (part - 2u);       // bucket b0 + j lives in counter j (b0 is a multiple of 4)
-  uint4 v;
-  v.x = (b0 >= bl && b0 <= bh) ? s.x : 0u;
-  v.y = (b0 + 1u >= bl && b0 + 1u <= bh) ? s.y : 0u;
-  v.z = (b0 + 2u >= bl && b0 + 2u <= bh) ? s.z : 0u;
-  v.w = (b0 + 3u >= bl && b0 + 3u <= bh) ? s.w : 0u;
-  return v;
-}
-
 __device__ __forceinline__ void bar_consumers(int n) {   // named barrier 1: consumer warps only
   asm volatile("bar.sync 1, %0;" ::"r"(n) : "memory");
 }
@@ -268,6 +262,9 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
   const Table tb{D.S};
   Hdr* H = hdr();
   SpanAcc* spans = span_tab();
+#ifdef ARGUS_SEG_PROF
+  const long long tf0 = clock64();
+#endif
   bar_consumers(NC);
   if (tid == 0) {
     uint32_t old = atomicCAS(&g.state[key], ARGUS_ST_LAZY, ARGUS_ST_BUSY);
@@ -283,28 +280,43 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
   const uint32_t mode = H->mode;
   uint8_t* rec = g.records + (size_t)key * D.rec_bytes;
   if (mode == ARGUS_ST_LAZY) {
-    // we own the record: write spans + cells once, coalesced 16-byte chunks
+    // we own the record: write spans + cells once with plain streaming stores
     uint4* dst = reinterpret_cast<uint4*>(rec + D.span_off);
     const uint32_t span_chunks = 2u * (D.P + 1u);
-    const uint32_t n_chunks = span_chunks + 10u * D.S;
-    for (uint32_t ch = tid; ch < n_chunks; ch += NC) {
+    for (uint32_t ch = tid; ch < span_chunks; ch += NC) {
       uint4 v;
-      if (ch < span_chunks) {
-        const uint32_t k = ch >> 1;
-        if (k < D.P && spans[k].n != 0ull) {
-          const SpanAcc a = spans[k];
-          v = (ch & 1u) ? make_uint4(0u, 0u, (uint32_t)a.n, (uint32_t)(a.n >> 32))
-                        : make_uint4((uint32_t)a.mn, (uint32_t)((unsigned long long)a.mn >> 32),
-                                     (uint32_t)a.mx, (uint32_t)((unsigned long long)a.mx >> 32));
-        } else {
-          v = argus_identity_chunk(D, ch);
-        }
+      const uint32_t k = ch >> 1;
+      if (k < D.P && spans[k].n != 0ull) {
+        const SpanAcc a = spans[k];
+        v = (ch & 1u) ? make_uint4(0u, 0u, (uint32_t)a.n, (uint32_t)(a.n >> 32))
+                      : make_uint4((uint32_t)a.mn, (uint32_t)((unsigned long long)a.mn >> 32),
+                                   (uint32_t)a.mx, (uint32_t)((unsigned long long)a.mx >> 32));
       } else {
-        const uint32_t cc = ch - span_chunks;
-        const uint32_t sig = cc / 10u, part = cc - sig * 10u;
-        v = cell_chunk(*tb.slots(sig), *tb.sum_lo(sig), *tb.sum_hi(sig), *tb.mm(sig), part);
+        v = argus_identity_chunk(D, ch);
       }
       __stcs(dst + ch, v);
+    }
+    // one thread per cell: decode the compact cell once, then ten 16-byte stores (the 160-byte
+    // cell is 32-byte aligned, so consecutive store pairs fill whole sectors in L2)
+    uint4* cdst = reinterpret_cast<uint4*>(rec + D.cell_off);
+    for (uint32_t sig = tid; sig < D.S; sig += NC) {
+      const uint4 c = *tb.slots(sig);
+      const uint2 m = *tb.mm(sig);
+      const uint32_t slo = *tb.sum_lo(sig), shi = *tb.sum_hi(sig);
+      uint4* o = cdst + 10u * sig;
+      const unsigned long long cnt = (unsigned long long)c.x + c.y + c.z + c.w;
+      const bool empty = (m.x | m.y) == 0u;
+      __stcs(o, make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), slo, shi));
+      __stcs(o + 1, empty ? make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u) : make_uint4(~m.x, 0u, m.y, 0u));
+      // counter j holds the bucket b in [bl, bh] with b & 3 == j; it belongs to hist chunk b >> 2
+      const uint32_t bl = bucket32(~m.x), bh = bucket32(m.y);
+      uint32_t kx = bl + ((0u - bl) & 3u), ky = bl + ((1u - bl) & 3u), kz = bl + ((2u - bl) & 3u),
+               kw = bl + ((3u - bl) & 3u);
+      kx = (empty || kx > bh) ? 0xFFu : kx >> 2; ky = (empty || ky > bh) ? 0xFFu : ky >> 2;
+      kz = (empty || kz > bh) ? 0xFFu : kz >> 2; kw = (empty || kw > bh) ? 0xFFu : kw >> 2;
+#pragma unroll
+      for (uint32_t k = 0; k < 8u; ++k)
+        __stcs(o + 2u + k, make_uint4(kx == k ? c.x : 0u, ky == k ? c.y : 0u, kz == k ? c.z : 0u, kw == k ? c.w : 0u));
     }
     __threadfence();
     bar_consumers(NC);
@@ -352,6 +364,9 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
   }
   bar_consumers(NC);
+#ifdef ARGUS_SEG_PROF
+  if (tid == 0) g_prof_flush[blockIdx.x] += clock64() - tf0;
+#endif
 }
 
 // Rendezvous of all consumer warps (the only CTA-wide synchronisation of the steady state, taken
@@ -470,6 +485,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   constexpr uint32_t EMPTY_OFF = MAXK * 8u;          // empty[k] sits MAXK*8 bytes after full[k]
   WarpSpan ws;
   ws.reset();
+  PROF_DECL;
   uint32_t cur_key = KEY_NONE, live = 0u;
   uint32_t cur_rank = 0u, cur_step = 0u, s_eff = 0u;   // s_eff = 0 while no key is current: nothing is accepted
   uint32_t n_invalid = 0;
@@ -488,29 +504,65 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     } else { s_eff = 0u; }                                                          \
   } while (0)
 
+  // The compact-cell update of one event (sig, d32 < 2^32): true if the cell took it.
+  //   inside [min, max]                      -> counters only (the common case)
+  //   inside the cell's current bucket range  -> one 32-bit max on ~min or max (cannot break the invariant)
+  //   else                                    -> mm_extend (64-bit CAS with the range check)
+#define ARGUS_COMPACT_ADD(took)                                                          \
+  do {                                                                                   \
+    const uint32_t a_m = a_mm + sig * 8u;                                                \
+    const uint2 m = lds64(a_m);                                                          \
+    const uint32_t nd = ~d32, b = bucket32(d32);                                         \
+    took = (nd <= m.x) & (d32 <= m.y);                                                   \
+    if (!took) {                                                                         \
+      if (b >= bucket32(~m.x) && b <= bucket32(m.y)) {                                   \
+        if (nd > m.x) reds_max(a_m, nd); else reds_max(a_m + 4u, d32);                   \
+        took = true;                                                                     \
+      } else {                                                                           \
+        took = mm_extend(a_m, d32);                                                      \
+      }                                                                                  \
+    }                                                                                    \
+    if (took) {                                                                          \
+      reds_add(a_slots + sig * 16u + ((b & 3u) << 2), 1u);                               \
+      const uint32_t old = atoms_add(a_sumlo + sig * 4u, d32);                           \
+      if (old > nd) reds_add(a_sumhi + sig * 4u, 1u);   /* old + d32 carried */          \
+    }                                                                                    \
+  } while (0)
+
+  const uint32_t n_full = n_ev / (uint32_t)NC;   // iterations in which every lane of every warp has an event
   for (uint32_t it = 0; it < n_iter; ++it) {
-    const uint32_t idx = my_pos + (uint32_t)lane;
     // ---- load: one event per lane, stage -> registers; release the stage at once --------------------
-    const bool have = s < n_sub;                 // this warp's stage exists (warp-uniform)
+    bool have = true, mine = true;
+    if (it >= n_full) {                          // the ragged last iteration
+      have = s < n_sub;                          // this warp's stage exists (warp-uniform)
+      mine = have && my_pos + (uint32_t)lane < n_ev;
+    }
     // While a warp waits for data it watches the rendezvous request: a warp beyond the requested
     // position joins the rendezvous BEFORE taking its next chunk (a parked warp keeps its next
     // stage unreleased, which may stall the in-order producer, so nobody may wait for data while
     // others wait for him).  Warps before that position go on: their stages are always issued.
     const uint32_t a_bar = a_full + slot * 8u;
-    while (have && !mbar_try_wait(a_bar, par)) {
-      if (lds32(a_nextidx) < my_pos) {
-        ws.flush(lane);
-        const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
-        ARGUS_ADOPT(r);
-      }
+    if (have && !mbar_try_wait(a_bar, par)) {
+      PROF_BEGIN(tw);
+      do {
+        if (lds32(a_nextidx) < my_pos) {
+          ws.flush(lane);
+          PROF_BEGIN(tp);
+          const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
+          PROF_END(prof_park, tp);
+          ARGUS_ADOPT(r);
+        }
+      } while (!mbar_try_wait(a_bar, par));
+      PROF_END(prof_wait, tw);
     }
-    uint4 lo = make_uint4(0u, 0u, 0u, 0u), hi = make_uint4(0u, 0u, 0u, 0u);
-    const bool mine = have && idx < n_ev;
+    uint4 lo, hi;
     if (have) {
       lo = lds128(a_ev);
       hi = lds128(a_ev + 16u);
       __syncwarp();
       if (lane == 0) mbar_arrive(a_bar + EMPTY_OFF);
+    } else {
+      lo = make_uint4(0u, 0u, 0u, 0u); hi = lo;
     }
     slot += SPI; a_ev += (uint32_t)(SPI * SUBE * 32);
     if (slot >= (uint32_t)K) { slot -= (uint32_t)K; par ^= 1u; a_ev -= ring_bytes; }
@@ -526,30 +578,33 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     const uint32_t d32 = (uint32_t)d;
     bool fast = mine & (lo.x == cur_rank) & (lo.y == cur_step) & (sig < s_eff) & (phase < D.P) &
                 ((int)(hi.y | hi.w) >= 0) & ((uint32_t)(d >> 32) == 0u);
-    bool pending = fast;
+    bool pending, ok = false, tried = false;
     uint32_t key = cur_key;
-    if (!__all_sync(FULL, fast)) {
+    if (__all_sync(FULL, fast)) {
+      // ---- hot path: the whole warp folds into the current table -------------------------------------
+      ARGUS_COMPACT_ADD(ok);
+      if (__all_sync(FULL, ok && phase == ws.phase)) {
+        ws.mn = start < ws.mn ? start : ws.mn;
+        ws.mx = end > ws.mx ? end : ws.mx;
+        ws.n += 32u;                       // warp-uniform count
+        continue;
+      }
+      pending = true; tried = true;        // a refused event or a phase change: general handling below
+    } else {
       // full validity (R2, R3) of the lanes that failed the fast test
       pending = mine && argus_event_key(D, lo.x, lo.y, sig, phase, start, end, key);
       n_invalid += (mine && !pending) ? 1u : 0u;
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
 
+    const uint32_t idx = my_pos - (uint32_t)NC + (uint32_t)lane;   // position of this lane's event
     for (;;) {
       // ---- cells -----------------------------------------------------------------------------------
-      bool ok = false;
-      if (fast) {
-        const uint32_t a_m = a_mm + sig * 8u;
-        const uint2 m = lds64(a_m);
-        bool inside = (~d32 <= m.x) & (d32 <= m.y);      // min <= d <= max: the common case
-        if (!inside) inside = mm_extend(a_m, d32);
-        if (inside) {
-          reds_add(a_slots + sig * 16u + ((bucket32(d32) & 3u) << 2), 1u);
-          const uint32_t old = atoms_add(a_sumlo + sig * 4u, d32);
-          if (old + d32 < old) reds_add(a_sumhi + sig * 4u, 1u);
-          ok = true;
-        }
+      if (!tried) {
+        ok = false;
+        if (fast) ARGUS_COMPACT_ADD(ok);
       }
+      tried = false;
       if (!ok && pending && key == cur_key && live) {
         // the compact cell cannot take this event and the record is live: L2 atomics
         global_cell_add(records, D, cur_key, sig, d);
@@ -559,7 +614,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       if (__all_sync(FULL, ok && phase == ws.phase)) {
         ws.mn = start < ws.mn ? start : ws.mn;
         ws.mx = end > ws.mx ? end : ws.mx;
-        ws.n += 32u;                       // warp-uniform count
+        ws.n += 32u;
       } else {
         ws.flush(lane);
         const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
@@ -587,11 +642,14 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       if (ok) { pending = false; fast = false; }
       if (!__any_sync(FULL, pending)) break;
       ws.flush(lane);
+      PROF_BEGIN(tp2);
       const unsigned long long r = park<NC>(gl, pending, key, idx, cur_key, live);
+      PROF_END(prof_park, tp2);
       ARGUS_ADOPT(r);
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
   }
+#undef ARGUS_COMPACT_ADD
   // ---- out of events: keep joining the rendezvous until every warp is done ---------------------------
   ws.flush(lane);
   if (lane == 0) atomicAdd(&H->n_finished, 1u);
@@ -601,6 +659,11 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
   }
 #undef ARGUS_ADOPT
+#ifdef ARGUS_SEG_PROF
+  if ((warp == 0 || warp == CW - 1) && lane == 0 && (blockIdx.x % 37) == 0)
+    printf("cta %3d warp %2d: total %lld  wait-data %lld  park %lld (flush %lld)  iters %u\n", blockIdx.x, warp,
+           clock64() - prof_t0, prof_wait, prof_park, g_prof_flush[blockIdx.x], n_iter);
+#endif
 
   n_invalid = __reduce_add_sync(FULL, n_invalid);
   if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
