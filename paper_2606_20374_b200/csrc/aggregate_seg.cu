@@ -24,7 +24,10 @@
 // with coalesced 128-bit stores (no read-modify-write, no separate identity fill); any later
 // contribution to the same record merges with L2 reductions.  Correct for ANY event order; fast
 // when events are grouped by (rank, step) (R18).
+#include <stddef.h>
 #include <stdio.h>
+
+#include <type_traits>
 
 #include "argus_internal.cuh"
 
@@ -477,11 +480,13 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
 
   // ---- consumer warps -----------------------------------------------------------------------------
   // All shared-memory traffic of the hot loop goes through 32-bit shared-window addresses.
-  const uint32_t sbase = smem_u32(smem);
+  uint32_t sbase = smem_u32(smem);
+  asm volatile("mov.u32 %0, %0;" : "+r"(sbase));   // opaque: keep it in a register, do not rematerialise
   const uint32_t a_slots = sbase + TAB_OFF, a_sumlo = a_slots + 16u * D.S, a_sumhi = a_slots + 20u * D.S,
                  a_mm = a_slots + 24u * D.S;
   const uint32_t a_ring = sbase + stages, ring_bytes = (uint32_t)K * (uint32_t)(SUBE * 32);
-  const uint32_t a_full = smem_u32(&H->full[0]), a_nextidx = smem_u32(&H->next_idx);
+  const uint32_t a_nextidx = sbase + (uint32_t)offsetof(Hdr, next_idx);
+  const uint32_t bar_ring = (uint32_t)K * 8u;     // bytes of full[0..K)
   constexpr uint32_t EMPTY_OFF = MAXK * 8u;          // empty[k] sits MAXK*8 bytes after full[k]
   WarpSpan ws;
   ws.reset();
@@ -490,9 +495,12 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   uint32_t cur_rank = 0u, cur_step = 0u, s_eff = 0u;   // s_eff = 0 while no key is current: nothing is accepted
   uint32_t n_invalid = 0;
   const uint32_t grp = (uint32_t)warp / WPSTG, wis = (uint32_t)warp % WPSTG;   // stage group, warp in stage
-  uint32_t slot = grp % (uint32_t)K, par = (grp / (uint32_t)K) & 1u;
-  uint32_t a_ev = a_ring + slot * (uint32_t)(SUBE * 32) + wis * 1024u + (uint32_t)lane * 32u;
-  uint32_t s = grp;                              // this warp's stage of the current iteration
+  const uint32_t slot0 = grp % (uint32_t)K;
+  uint32_t par = (grp / (uint32_t)K) & 1u;
+  uint32_t a_bar = sbase + (uint32_t)offsetof(Hdr, full) + slot0 * 8u;      // full[slot] of this iteration
+  const uint32_t a_bar_end = sbase + (uint32_t)offsetof(Hdr, full) + bar_ring;
+  uint32_t a_ev = a_ring + slot0 * (uint32_t)(SUBE * 32) + wis * 1024u + (uint32_t)lane * 32u;
+  uint32_t s = grp;                              // this warp's stage (tail iteration only)
   uint32_t my_pos = (uint32_t)warp * 32u;        // first event of this warp's chunk
 
 #define ARGUS_ADOPT(r)                                                              \
@@ -530,10 +538,12 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   } while (0)
 
   const uint32_t n_full = n_ev / (uint32_t)NC;   // iterations in which every lane of every warp has an event
-  for (uint32_t it = 0; it < n_iter; ++it) {
+  // One iteration of a consumer warp.  TAIL = the ragged last iteration (stage or lanes may be missing).
+  auto body = [&](auto tail_c) {
+    constexpr bool TAIL = decltype(tail_c)::value;
     // ---- load: one event per lane, stage -> registers; release the stage at once --------------------
     bool have = true, mine = true;
-    if (it >= n_full) {                          // the ragged last iteration
+    if (TAIL) {
       have = s < n_sub;                          // this warp's stage exists (warp-uniform)
       mine = have && my_pos + (uint32_t)lane < n_ev;
     }
@@ -541,7 +551,6 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     // position joins the rendezvous BEFORE taking its next chunk (a parked warp keeps its next
     // stage unreleased, which may stall the in-order producer, so nobody may wait for data while
     // others wait for him).  Warps before that position go on: their stages are always issued.
-    const uint32_t a_bar = a_full + slot * 8u;
     if (have && !mbar_try_wait(a_bar, par)) {
       PROF_BEGIN(tw);
       do {
@@ -564,9 +573,14 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     } else {
       lo = make_uint4(0u, 0u, 0u, 0u); hi = lo;
     }
-    slot += SPI; a_ev += (uint32_t)(SPI * SUBE * 32);
-    if (slot >= (uint32_t)K) { slot -= (uint32_t)K; par ^= 1u; a_ev -= ring_bytes; }
-    s += SPI; my_pos += NC;
+    a_bar += (uint32_t)(SPI * 8); a_ev += (uint32_t)(SPI * SUBE * 32);
+    if (a_bar >= a_bar_end) { a_bar -= bar_ring; par ^= 1u; a_ev -= ring_bytes; }
+    if (TAIL) s += SPI;
+    my_pos += NC;
+#ifdef ARGUS_SEG_NOCOMPUTE
+    n_invalid += (lo.x ^ hi.x) == 0x12345u;     // experiment: stream only (results are wrong)
+    return;
+#endif
 
     // ---- decode.  Fast test first: the event belongs to the current key and fits a compact cell
     // (same rank and step words as the current key, sig and phase in range, both timestamps
@@ -587,7 +601,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
         ws.mn = start < ws.mn ? start : ws.mn;
         ws.mx = end > ws.mx ? end : ws.mx;
         ws.n += 32u;                       // warp-uniform count
-        continue;
+        return;
       }
       pending = true; tried = true;        // a refused event or a phase change: general handling below
     } else {
@@ -648,7 +662,10 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       ARGUS_ADOPT(r);
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
-  }
+  };
+#pragma unroll 1
+  for (uint32_t it = 0; it < n_full; ++it) body(std::false_type{});
+  if (n_iter > n_full) { s = grp + n_full * (uint32_t)SPI; body(std::true_type{}); }
 #undef ARGUS_COMPACT_ADD
   // ---- out of events: keep joining the rendezvous until every warp is done ---------------------------
   ws.flush(lane);
@@ -678,7 +695,11 @@ cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, vo
   const size_t fixed = stage_off(ctx->dims.S);
   int K = (int)(((size_t)ctx->max_smem_optin - fixed) / STAGE_BYTES);
   if (K > MAXK) K = MAXK;
-  if (K < 2 * SPI + 1) return cudaErrorInvalidConfiguration;
+  // K must be a multiple of the stages taken per iteration: a warp group then always returns to
+  // the slots it released itself, so the parity it waits for can never alias a fill that is two
+  // rounds behind (bulk copies of different stages may complete out of order)
+  K -= K % SPI;
+  if (K < 2 * SPI) return cudaErrorInvalidConfiguration;
   const size_t smem_bytes = fixed + (size_t)K * STAGE_BYTES;
   cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
@@ -700,8 +721,8 @@ cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, vo
 }  // namespace
 
 bool argus_seg_supported(const argus_ctx* ctx) {
-  // default variant: 6 KB stages, 5 per iteration, at least 11 in the ring
-  return (size_t)stage_off(ctx->dims.S) + (size_t)11 * 6144 <= (size_t)ctx->max_smem_optin;
+  // default variant: 10 KB stages, 3 per iteration, at least 6 in the ring
+  return (size_t)stage_off(ctx->dims.S) + (size_t)6 * 10240 <= (size_t)ctx->max_smem_optin;
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
@@ -714,6 +735,6 @@ cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, ui
     case 4: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
     case 5: return launch_variant<31, 31>(ctx, ev, n, d_records, s);
     case 6: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
-    default: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
+    default: return launch_variant<30, 10>(ctx, ev, n, d_records, s);
   }
 }
