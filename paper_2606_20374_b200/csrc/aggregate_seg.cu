@@ -299,27 +299,36 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
       }
       __stcs(dst + ch, v);
     }
-    // one thread per cell: decode the compact cell once, then ten 16-byte stores (the 160-byte
-    // cell is 32-byte aligned, so consecutive store pairs fill whole sectors in L2)
+    // cells, as two coalesced streams of 16-byte chunks (the compact cell is re-read from shared
+    // memory by every lane that needs it; lanes of one cell read the same words: broadcast).
+    // (1) histogram chunks: 8 lanes per cell, a warp store covers 4 cells x 128 contiguous bytes.
+    //     Counter j of a cell holds the bucket b >= bl with b & 3 == j, bl = bucket(min): bucket
+    //     4k + j is live iff (4k + j - bl) mod 2^32 < 4 (counters beyond bucket(max) are 0 anyway).
     uint4* cdst = reinterpret_cast<uint4*>(rec + D.cell_off);
-    for (uint32_t sig = tid; sig < D.S; sig += NC) {
+    for (uint32_t i = tid; i < 8u * D.S; i += NC) {
+      const uint32_t sig = i >> 3, k4 = (i & 7u) << 2;
+      const uint4 c = *tb.slots(sig);
+      const uint32_t bl = bucket32(~tb.mm(sig)->x);
+      uint4 v;
+      v.x = (k4 - bl) < 4u ? c.x : 0u;
+      v.y = (k4 + 1u - bl) < 4u ? c.y : 0u;
+      v.z = (k4 + 2u - bl) < 4u ? c.z : 0u;
+      v.w = (k4 + 3u - bl) < 4u ? c.w : 0u;
+      __stcs(cdst + 10u * sig + 2u + (i & 7u), v);
+    }
+    // (2) head chunks {count, sum} {min, max}: 2 lanes per cell
+    for (uint32_t i = tid; i < 2u * D.S; i += NC) {
+      const uint32_t sig = i >> 1;
       const uint4 c = *tb.slots(sig);
       const uint2 m = *tb.mm(sig);
-      const uint32_t slo = *tb.sum_lo(sig), shi = *tb.sum_hi(sig);
-      uint4* o = cdst + 10u * sig;
-      const unsigned long long cnt = (unsigned long long)c.x + c.y + c.z + c.w;
-      const bool empty = (m.x | m.y) == 0u;
-      __stcs(o, make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), slo, shi));
-      __stcs(o + 1, empty ? make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u) : make_uint4(~m.x, 0u, m.y, 0u));
-      // counter j holds the bucket b in [bl, bh] with b & 3 == j; it belongs to hist chunk b >> 2
-      const uint32_t bl = bucket32(~m.x), bh = bucket32(m.y);
-      uint32_t kx = bl + ((0u - bl) & 3u), ky = bl + ((1u - bl) & 3u), kz = bl + ((2u - bl) & 3u),
-               kw = bl + ((3u - bl) & 3u);
-      kx = (empty || kx > bh) ? 0xFFu : kx >> 2; ky = (empty || ky > bh) ? 0xFFu : ky >> 2;
-      kz = (empty || kz > bh) ? 0xFFu : kz >> 2; kw = (empty || kw > bh) ? 0xFFu : kw >> 2;
-#pragma unroll
-      for (uint32_t k = 0; k < 8u; ++k)
-        __stcs(o + 2u + k, make_uint4(kx == k ? c.x : 0u, ky == k ? c.y : 0u, kz == k ? c.z : 0u, kw == k ? c.w : 0u));
+      uint4 v;
+      if ((i & 1u) == 0u) {
+        const unsigned long long cnt = (unsigned long long)c.x + c.y + c.z + c.w;
+        v = make_uint4((uint32_t)cnt, (uint32_t)(cnt >> 32), *tb.sum_lo(sig), *tb.sum_hi(sig));
+      } else {
+        v = (m.x | m.y) == 0u ? make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u) : make_uint4(~m.x, 0u, m.y, 0u);
+      }
+      __stcs(cdst + 10u * sig + (i & 1u), v);
     }
     __threadfence();
     bar_consumers(NC);
