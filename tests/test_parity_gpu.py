@@ -122,6 +122,30 @@ def test_hot_single_sig_carry():
     assert_parity(ev, 1, 1, 1, 1, 0, path=PATH_SEG)
 
 
+def test_bucket_window_invariant_cells():
+    # the compact cell holds at most four CONSECUTIVE buckets: sweep one sig over
+    # every bucket upward, downward and bimodally (b and b+4 collide in the direct-mapped counters),
+    # concurrently from all lanes, over several rank-steps; the refused events take the global path
+    n_sig, R, T = 6, 3, 2
+    rows = []
+    t0 = 0
+    for r in range(R):
+        for t in range(T):
+            for i in range(4000):
+                k = i % 64
+                up = (1 << (k % 33)) + (i % 3)                 # sig 0: all buckets upward (incl. >= 2^32)
+                down = (1 << (32 - k % 33)) - (i % 2)          # sig 1: all buckets downward
+                bi = (1 << 10) + i % 7 if i % 2 else (1 << 14) + i % 5   # sig 2: buckets 10 and 14
+                tri = [3, 40, 700, 9000, 100000][i % 5]        # sig 3: five spread buckets
+                edge = [(1 << 12) - 1, 1 << 12, (1 << 16) - 1, 1 << 16][i % 4]  # sig 4: window edges 11,12,15,16
+                for s_, d in ((0, up), (1, down), (2, bi), (3, tri), (4, edge), (5, 1000 + i % 50)):
+                    rows.append((r, t, s_, 0, i % 2, t0, t0 + d))
+                    t0 += 7
+    ev = make_events(rows)
+    for grid in (None, 5):
+        assert_parity(ev, R, T, n_sig, 2, 0, path=PATH_SEG, grid=grid)
+
+
 @pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
 def test_mid_scaled(path):
     wl = build_workload(scaled("mid", n_ranks=48, n_steps=3))
