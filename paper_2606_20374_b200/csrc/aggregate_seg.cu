@@ -217,7 +217,9 @@ __device__ __forceinline__ unsigned long long atoms_cas64(uint32_t a, unsigned l
   return o;
 }
 __device__ __forceinline__ uint32_t bucket32(uint32_t d) {   // R4 for d < 2^32: floor(log2 d), 0 for d <= 1
-  return 31u - (uint32_t)__clz((int)(d | 1u));
+  uint32_t b;
+  asm("bfind.u32 %0, %1;" : "=r"(b) : "r"(d | 1u));     // bit position of the leading one (FLO)
+  return b;
 }
 
 // Rare path of the compact cell: the event's duration d lies outside the cell's [min, max] (or the
@@ -575,8 +577,18 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     }
     uint4 lo, hi;
     if (have) {
+#ifdef ARGUS_SEG_SWZ
+      // lanes 4-7, 12-15, ... read their second half first: every quarter-warp then covers all
+      // eight 16-byte bank groups (conflict-free LDS.128) at the price of eight selects
+      const bool hsw = (lane & 4) != 0;
+      const uint4 A = lds128(a_ev + (hsw ? 16u : 0u));
+      const uint4 B = lds128(a_ev + (hsw ? 0u : 16u));
+      lo.x = hsw ? B.x : A.x; lo.y = hsw ? B.y : A.y; lo.z = hsw ? B.z : A.z; lo.w = hsw ? B.w : A.w;
+      hi.x = hsw ? A.x : B.x; hi.y = hsw ? A.y : B.y; hi.z = hsw ? A.z : B.z; hi.w = hsw ? A.w : B.w;
+#else
       lo = lds128(a_ev);
       hi = lds128(a_ev + 16u);
+#endif
       __syncwarp();
       if (lane == 0) mbar_arrive(a_bar + EMPTY_OFF);
     } else {
