@@ -82,6 +82,17 @@ struct Table {
   __device__ __forceinline__ uint32_t* sum_lo(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF + 16u * S) + sig; }
   __device__ __forceinline__ uint32_t* sum_hi(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF + 20u * S) + sig; }
   __device__ __forceinline__ uint2* mm(uint32_t sig) const { return reinterpret_cast<uint2*>(smem + TAB_OFF + 24u * S) + sig; }
+  // zero the cells of sigs [0, n): four arrays (S here is the compiled capacity, n <= S the live sigs)
+  __device__ __forceinline__ void clear(uint32_t n, uint32_t t, uint32_t nt) const {
+    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+    uint4* a = slots(0);
+    for (uint32_t i = t; i < n; i += nt) a[i] = z;
+    uint4* b = reinterpret_cast<uint4*>(sum_lo(0));
+    uint4* c = reinterpret_cast<uint4*>(sum_hi(0));
+    for (uint32_t i = t; i < (n + 3u) / 4u; i += nt) { b[i] = z; c[i] = z; }
+    uint4* d = reinterpret_cast<uint4*>(mm(0));
+    for (uint32_t i = t; i < (n + 1u) / 2u; i += nt) d[i] = z;
+  }
 };
 __device__ __forceinline__ Hdr* hdr() { return reinterpret_cast<Hdr*>(smem); }
 __device__ __forceinline__ SpanAcc* span_tab() { return reinterpret_cast<SpanAcc*>(smem + HDR_BYTES); }
@@ -260,11 +271,11 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 
 // Flush the shared table of record `key` to global memory and clear it.  All NC consumer threads
 // call (tid < NC); each warp has flushed its WarpSpan first.  Ends with a consumer barrier.
-template <int NC>
+template <int NC, uint32_t SCAP>
 __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
   const int tid = threadIdx.x;
   const argus_dims& D = g.D;
-  const Table tb{D.S};
+  const Table tb{SCAP};
   Hdr* H = hdr();
   SpanAcc* spans = span_tab();
 #ifdef ARGUS_SEG_PROF
@@ -372,8 +383,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
     }
   }
   bar_consumers(NC);
-  uint4* all = tb.slots(0);           // slots, sum_lo, sum_hi, mm are contiguous: 2*S uint4
-  for (uint32_t i = tid; i < 2u * D.S; i += NC) all[i] = make_uint4(0u, 0u, 0u, 0u);
+  tb.clear(D.S, (uint32_t)tid, (uint32_t)NC);
   for (uint32_t k = tid; k < D.P; k += NC) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
   }
@@ -392,7 +402,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
 // Result packed as {cur_key : 32 | live : 1 | all_done : 1} (by value: keeps the caller's state in registers).
 constexpr unsigned long long PARK_LIVE = 1ull << 32, PARK_DONE = 1ull << 33;
 constexpr uint32_t DEC_SWITCH = 0u, DEC_SPURIOUS = 1u, DEC_DONE = 2u;
-template <int NC>
+template <int NC, uint32_t SCAP>
 __device__ __noinline__ unsigned long long park(const Glob& gl, bool pending, uint32_t key,
                                                 uint32_t my_idx, uint32_t cur_key, uint32_t live) {
   Hdr* H = hdr();
@@ -415,10 +425,10 @@ __device__ __noinline__ unsigned long long park(const Glob& gl, bool pending, ui
     return (unsigned long long)cur_key | (live ? PARK_LIVE : 0ull);
   }
   if (dec == DEC_DONE) {
-    if (cur_key != KEY_NONE) flush_table<NC>(gl, cur_key);
+    if (cur_key != KEY_NONE) flush_table<NC, SCAP>(gl, cur_key);
     return PARK_DONE | cur_key;
   }
-  if (cur_key != KEY_NONE) flush_table<NC>(gl, cur_key);   // begins and ends with a consumer barrier
+  if (cur_key != KEY_NONE) flush_table<NC, SCAP>(gl, cur_key);   // begins and ends with a consumer barrier
   else bar_consumers(NC);
   if (tid == 0) H->next_idx = KEY_NONE;
   bar_consumers(NC);
@@ -428,19 +438,35 @@ __device__ __noinline__ unsigned long long park(const Glob& gl, bool pending, ui
 }
 
 // CW consumer warps + 1 producer warp.  Stage = WPSTG warps' worth of events (WPSTG KB).
-template <int CW, int WPSTG>
+// Ring depth for a table capacity SCAP and a stage of stage_bytes: everything left of the 227 KB a CTA
+// may use, capped at MAXK, rounded down to a multiple of the stages taken per iteration (a warp
+// group then always returns to the slots it released itself, so the parity it waits for can never
+// alias a fill two rounds behind: bulk copies of different stages may complete out of order).
+constexpr uint32_t SMEM_MAX = 232448;          // 227 KB: the opt-in limit of one CTA on sm_100
+constexpr uint32_t ARGUS_SEG_MAX_SIGS = 5120;   // largest table capacity that still leaves a 6-stage ring
+__host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes, int spi) {
+  int k = (int)((SMEM_MAX - ((TAB_OFF + 32u * scap + 127u) & ~127u)) / stage_bytes);
+  if (k > MAXK) k = MAXK;
+  return k - k % spi;
+}
+
+// CW consumer warps + 1 producer warp; a stage = WPSTG warps' worth of events (WPSTG KB); the table
+// layout is compiled for SCAP sigs (S <= SCAP), so every table address is base + sig * c + constant.
+template <int CW, int WPSTG, uint32_t SCAP>
 __global__ void __launch_bounds__((CW + 1) * 32, 1)
 aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta, uint8_t* records,
-                     uint32_t* state, unsigned long long* counters, argus_dims D, int K) {
+                     uint32_t* state, unsigned long long* counters, argus_dims D) {
+  constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG);
+  static_assert(K >= 2 * (CW / WPSTG), "ring too shallow for this geometry");
   constexpr int NC = CW * 32;            // consumer threads
   constexpr int SUBE = WPSTG * 32;       // events per stage
   constexpr int SPI = CW / WPSTG;        // stages per iteration
   static_assert(CW % WPSTG == 0, "geometry");
   Glob gl;
   gl.records = records; gl.state = state; gl.D = D;
-  const Table tb{D.S};
+  const Table tb{SCAP};
   Hdr* H = hdr();
-  const uint32_t stages = stage_off(D.S);     // byte offset of the stage ring in smem
+  constexpr uint32_t stages = (TAB_OFF + 32u * SCAP + 127u) & ~127u;   // byte offset of the stage ring in smem
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint64_t e0 = (uint64_t)blockIdx.x * per_cta;
@@ -461,8 +487,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   {
-    uint4* all = tb.slots(0);
-    for (uint32_t i = tid; i < 2u * D.S; i += (CW + 1) * 32) all[i] = make_uint4(0u, 0u, 0u, 0u);
+    tb.clear(D.S, (uint32_t)tid, (uint32_t)(CW + 1) * 32u);
     SpanAcc* spans = span_tab();
     for (uint32_t k = tid; k < ARGUS_MAX_PHASES; k += (CW + 1) * 32) {
       spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
@@ -493,8 +518,8 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   // All shared-memory traffic of the hot loop goes through 32-bit shared-window addresses.
   uint32_t sbase = smem_u32(smem);
   asm volatile("mov.u32 %0, %0;" : "+r"(sbase));   // opaque: keep it in a register, do not rematerialise
-  const uint32_t a_slots = sbase + TAB_OFF, a_sumlo = a_slots + 16u * D.S, a_sumhi = a_slots + 20u * D.S,
-                 a_mm = a_slots + 24u * D.S;
+  const uint32_t a_slots = sbase + TAB_OFF, a_sumlo = a_slots + 16u * SCAP, a_sumhi = a_slots + 20u * SCAP,
+                 a_mm = a_slots + 24u * SCAP;
   const uint32_t a_ring = sbase + stages, ring_bytes = (uint32_t)K * (uint32_t)(SUBE * 32);
   const uint32_t a_nextidx = sbase + (uint32_t)offsetof(Hdr, next_idx);
   const uint32_t bar_ring = (uint32_t)K * 8u;     // bytes of full[0..K)
@@ -568,7 +593,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
         if (lds32(a_nextidx) < my_pos) {
           ws.flush(lane);
           PROF_BEGIN(tp);
-          const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
+          const unsigned long long r = park<NC, SCAP>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
           PROF_END(prof_park, tp);
           ARGUS_ADOPT(r);
         }
@@ -678,7 +703,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       if (!__any_sync(FULL, pending)) break;
       ws.flush(lane);
       PROF_BEGIN(tp2);
-      const unsigned long long r = park<NC>(gl, pending, key, idx, cur_key, live);
+      const unsigned long long r = park<NC, SCAP>(gl, pending, key, idx, cur_key, live);
       PROF_END(prof_park, tp2);
       ARGUS_ADOPT(r);
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
@@ -692,7 +717,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   ws.flush(lane);
   if (lane == 0) atomicAdd(&H->n_finished, 1u);
   for (;;) {
-    const unsigned long long r = park<NC>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
+    const unsigned long long r = park<NC, SCAP>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
     if (r & PARK_DONE) break;
     cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
   }
@@ -708,54 +733,54 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
 }
 
-template <int CW, int WPSTG>
-cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records,
-                           cudaStream_t s) {
-  constexpr int SPI = CW / WPSTG;
+template <int CW, int WPSTG, uint32_t SCAP>
+cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records, cudaStream_t s) {
   constexpr size_t STAGE_BYTES = (size_t)WPSTG * 32 * 32;
-  const size_t fixed = stage_off(ctx->dims.S);
-  int K = (int)(((size_t)ctx->max_smem_optin - fixed) / STAGE_BYTES);
-  if (K > MAXK) K = MAXK;
-  // K must be a multiple of the stages taken per iteration: a warp group then always returns to
-  // the slots it released itself, so the parity it waits for can never alias a fill that is two
-  // rounds behind (bulk copies of different stages may complete out of order)
-  K -= K % SPI;
-  if (K < 2 * SPI) return cudaErrorInvalidConfiguration;
-  const size_t smem_bytes = fixed + (size_t)K * STAGE_BYTES;
-  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG>,
+  constexpr int K = ring_depth(SCAP, (uint32_t)STAGE_BYTES, CW / WPSTG);
+  constexpr size_t smem_bytes = ((TAB_OFF + 32u * SCAP + 127u) & ~127u) + (size_t)K * STAGE_BYTES;
+  static_assert(smem_bytes <= SMEM_MAX, "shared memory");
+  if ((size_t)ctx->max_smem_optin < smem_bytes) return cudaErrorInvalidConfiguration;
+  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
   if (e != cudaSuccess) return e;
   int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count;
-  // a CTA's slot counters hold 26 bits between flushes: bound the span of one CTA
+  // the u32 histogram counters of a CTA must not wrap between flushes: bound the span of one CTA
   const uint64_t tile = (uint64_t)CW * 32;
   const uint64_t cap = (1ull << 26) - tile;
   uint64_t per_cta = (n + grid - 1) / grid;
   if (per_cta > cap) per_cta = cap;
   per_cta = (per_cta + tile - 1) / tile * tile;
   const uint64_t ctas = (n + per_cta - 1) / per_cta;
-  aggregate_seg_kernel<CW, WPSTG><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
+  aggregate_seg_kernel<CW, WPSTG, SCAP><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
-      ctx->d_counters, ctx->dims, K);
+      ctx->d_counters, ctx->dims);
   return cudaGetLastError();
+}
+
+// The table layout is compiled for a few capacities; S picks the smallest that holds it.
+template <int CW, int WPSTG>
+cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records,
+                           cudaStream_t s) {
+  const uint32_t S = ctx->dims.S;
+  if (S <= 1024u) return launch_cap<CW, WPSTG, 1024u>(ctx, ev, n, d_records, s);
+  if (S <= 2048u) return launch_cap<CW, WPSTG, 2048u>(ctx, ev, n, d_records, s);
+  if (S <= 4096u) return launch_cap<CW, WPSTG, 4096u>(ctx, ev, n, d_records, s);
+  if (S <= ARGUS_SEG_MAX_SIGS) return launch_cap<CW, WPSTG, ARGUS_SEG_MAX_SIGS>(ctx, ev, n, d_records, s);
+  return cudaErrorInvalidConfiguration;
 }
 
 }  // namespace
 
 bool argus_seg_supported(const argus_ctx* ctx) {
-  // default variant: 10 KB stages, 3 per iteration, at least 6 in the ring
-  return (size_t)stage_off(ctx->dims.S) + (size_t)6 * 10240 <= (size_t)ctx->max_smem_optin;
+  return ctx->dims.S <= ARGUS_SEG_MAX_SIGS && (size_t)ctx->max_smem_optin >= SMEM_MAX;
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
                                        void* d_records, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
   switch (ctx->tune_variant) {
-    case 1: return launch_variant<30, 10>(ctx, ev, n, d_records, s);
-    case 2: return launch_variant<30, 15>(ctx, ev, n, d_records, s);
-    case 3: return launch_variant<28, 7>(ctx, ev, n, d_records, s);
-    case 4: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
-    case 5: return launch_variant<31, 31>(ctx, ev, n, d_records, s);
-    case 6: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
+    case 1: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
+    case 2: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
     default: return launch_variant<30, 10>(ctx, ev, n, d_records, s);
   }
 }
