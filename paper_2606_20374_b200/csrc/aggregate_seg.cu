@@ -62,13 +62,11 @@ struct SpanAcc {                      // shared-memory span accumulator of one p
 struct Hdr {
   unsigned long long full[MAXK];      // mbarriers: stage filled by TMA (tx bytes)
   unsigned long long empty[MAXK];     // mbarriers: stage read by all its consumer warps
-  uint32_t cur_key;                   // key adopted at the rendezvous
-  uint32_t pad0;
-  uint32_t next_idx;                  // lowest pending event index
-  uint32_t mode;                      // state word seen by the flush claim
+  unsigned long long next;            // rendezvous request {lowest pending event index : 32 | its key : 32}
+  uint32_t mode;                      // claim on the current key's record: LAZY = ours to write, LIVE, BUSY = another CTA's
   uint32_t n_finished;                // consumer warps that ran out of events
-  uint32_t decision;                  // outcome of the current rendezvous
 };
+constexpr unsigned long long NEXT_NONE = ~0ull;
 static_assert(sizeof(Hdr) <= HDR_BYTES, "header");
 
 extern __shared__ __align__(128) uint8_t smem[];
@@ -78,7 +76,6 @@ extern __shared__ __align__(128) uint8_t smem[];
 struct Table {
   uint32_t S;
   __device__ __forceinline__ uint4* slots(uint32_t sig) const { return reinterpret_cast<uint4*>(smem + TAB_OFF) + sig; }
-  __device__ __forceinline__ uint32_t* slot_words(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF) + 4u * sig; }
   __device__ __forceinline__ uint32_t* sum_lo(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF + 16u * S) + sig; }
   __device__ __forceinline__ uint32_t* sum_hi(uint32_t sig) const { return reinterpret_cast<uint32_t*>(smem + TAB_OFF + 20u * S) + sig; }
   __device__ __forceinline__ uint2* mm(uint32_t sig) const { return reinterpret_cast<uint2*>(smem + TAB_OFF + 24u * S) + sig; }
@@ -96,9 +93,6 @@ struct Table {
 };
 __device__ __forceinline__ Hdr* hdr() { return reinterpret_cast<Hdr*>(smem); }
 __device__ __forceinline__ SpanAcc* span_tab() { return reinterpret_cast<SpanAcc*>(smem + HDR_BYTES); }
-__host__ __device__ __forceinline__ uint32_t stage_off(uint32_t S) {
-  return (TAB_OFF + 32u * ((S + 3u) & ~3u) + 127u) & ~127u;
-}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
@@ -270,9 +264,13 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 }
 
 // Flush the shared table of record `key` to global memory and clear it.  All NC consumer threads
-// call (tid < NC); each warp has flushed its WarpSpan first.  Ends with a consumer barrier.
+// call between the rendezvous barrier (the table is final: every warp has flushed its WarpSpan)
+// and the closing barrier of park().  The claim on the record was taken when the key was adopted
+// (H->mode), so no global round trip sits on this path; the publication of a record we wrote
+// (fence + state LIVE) is left to thread 0 alone, after the barrier that orders everybody's stores
+// before it (fence cumulativity), while the others already clear the table.
 template <int NC, uint32_t SCAP>
-__device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
+__device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence_all) {
   const int tid = threadIdx.x;
   const argus_dims& D = g.D;
   const Table tb{SCAP};
@@ -281,19 +279,16 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
 #ifdef ARGUS_SEG_PROF
   const long long tf0 = clock64();
 #endif
-  bar_consumers(NC);
-  if (tid == 0) {
-    uint32_t old = atomicCAS(&g.state[key], ARGUS_ST_LAZY, ARGUS_ST_BUSY);
-    if (old == ARGUS_ST_BUSY) {
-      // another (resident, running) CTA is writing this record: wait for it, then merge
+  uint32_t mode = *reinterpret_cast<volatile uint32_t*>(&H->mode);
+  if (mode == ARGUS_ST_BUSY) {
+    // another (resident, running) CTA owns this record and is writing it: wait for it, then merge
+    if (tid == 0) {
       while (atomicAdd(&g.state[key], 0u) != ARGUS_ST_LIVE) __nanosleep(128);
       __threadfence();
-      old = ARGUS_ST_LIVE;
     }
-    H->mode = old;
+    bar_consumers(NC);
+    mode = ARGUS_ST_LIVE;
   }
-  bar_consumers(NC);
-  const uint32_t mode = H->mode;
   uint8_t* rec = g.records + (size_t)key * D.rec_bytes;
   if (mode == ARGUS_ST_LAZY) {
     // we own the record: write spans + cells once with plain streaming stores
@@ -343,9 +338,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
       }
       __stcs(cdst + 10u * sig + (i & 1u), v);
     }
-    __threadfence();
-    bar_consumers(NC);
-    if (tid == 0) atomicExch(&g.state[key], ARGUS_ST_LIVE);
+    if (fence_all) __threadfence();   // the callers go on with L2 atomics on this record at once
   } else {
     // merge into a live record with L2 reductions (non-empty fields only)
     argus_cell* cells = reinterpret_cast<argus_cell*>(rec + D.cell_off);
@@ -383,56 +376,54 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key) {
     }
   }
   bar_consumers(NC);
+  if (tid == 0 && mode == ARGUS_ST_LAZY) {
+    __threadfence();
+    atomicExch(&g.state[key], ARGUS_ST_LIVE);
+  }
   tb.clear(D.S, (uint32_t)tid, (uint32_t)NC);
   for (uint32_t k = tid; k < D.P; k += NC) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
   }
-  bar_consumers(NC);
 #ifdef ARGUS_SEG_PROF
   if (tid == 0) g_prof_flush[blockIdx.x] += clock64() - tf0;
 #endif
 }
 
 // Rendezvous of all consumer warps (the only CTA-wide synchronisation of the steady state, taken
-// once per (rank, step) boundary on grouped input).  A warp comes here when it holds an event it
-// cannot fold: another key than the table's, or an event that needs the global path while the
-// record is not live yet.  Warps that see H->park_flag, or have run out of events, join.  Then the
-// table is flushed and the key of the lowest pending event becomes current.  Returns true when no
-// warp has anything left (the last table has been flushed).
+// once per (rank, step) boundary on grouped input): three barriers.  A warp comes here when it
+// holds an event it cannot fold: another key than the table's, or an event that needs the global
+// path while the record is not live yet; it posts {event index, key} with a 64-bit min.  Warps
+// that see a request below their position, or have run out of events, join.  Then the table is
+// flushed and the key of the lowest pending event becomes current; thread 0 claims its record
+// (state LAZY -> BUSY) after the closing barrier, so the claim's round trip is off everybody's path.
 // Result packed as {cur_key : 32 | live : 1 | all_done : 1} (by value: keeps the caller's state in registers).
 constexpr unsigned long long PARK_LIVE = 1ull << 32, PARK_DONE = 1ull << 33;
-constexpr uint32_t DEC_SWITCH = 0u, DEC_SPURIOUS = 1u, DEC_DONE = 2u;
 template <int NC, uint32_t SCAP>
 __device__ __noinline__ unsigned long long park(const Glob& gl, bool pending, uint32_t key,
                                                 uint32_t my_idx, uint32_t cur_key, uint32_t live) {
   Hdr* H = hdr();
   const int tid = threadIdx.x;
-  // a pending event's index is the rendezvous request: every warp whose position in the stream is
-  // beyond H->next_idx comes here instead of going on (finished warps just wait here)
-  if (pending) atomicMin(&H->next_idx, my_idx);
+  if (pending) atomicMin(&H->next, ((unsigned long long)my_idx << 32) | key);
   bar_consumers(NC);
-  const uint32_t pick = *reinterpret_cast<volatile uint32_t*>(&H->next_idx);
-  if (tid == 0) {
-    const uint32_t fin = *reinterpret_cast<volatile uint32_t*>(&H->n_finished);
-    H->decision = pick != KEY_NONE ? DEC_SWITCH : (fin == (uint32_t)(NC / 32) ? DEC_DONE : DEC_SPURIOUS);
-  }
-  if (pending && my_idx == pick) H->cur_key = key;
-  bar_consumers(NC);
-  const uint32_t dec = *reinterpret_cast<volatile uint32_t*>(&H->decision);
-  const uint32_t nk = *reinterpret_cast<volatile uint32_t*>(&H->cur_key);
-  if (dec == DEC_SPURIOUS) {            // nobody holds a pending event, but not every warp is done
+  const unsigned long long nx = *reinterpret_cast<volatile unsigned long long*>(&H->next);
+  const uint32_t fin = *reinterpret_cast<volatile uint32_t*>(&H->n_finished);
+  const uint32_t nk = (uint32_t)nx;
+  const bool none = nx == NEXT_NONE;
+  if (none && fin != (uint32_t)(NC / 32)) {   // nobody holds a pending event, but not every warp is done
     bar_consumers(NC);
     return (unsigned long long)cur_key | (live ? PARK_LIVE : 0ull);
   }
-  if (dec == DEC_DONE) {
-    if (cur_key != KEY_NONE) flush_table<NC, SCAP>(gl, cur_key);
-    return PARK_DONE | cur_key;
-  }
-  if (cur_key != KEY_NONE) flush_table<NC, SCAP>(gl, cur_key);   // begins and ends with a consumer barrier
-  else bar_consumers(NC);
-  if (tid == 0) H->next_idx = KEY_NONE;
+  const bool same = !none && nk == cur_key;   // an overflow event asked for a live record
+  if (cur_key != KEY_NONE) flush_table<NC, SCAP>(gl, cur_key, same);
+  else bar_consumers(NC);                      // everybody has read H->next
+  if (none) return PARK_DONE | cur_key;
+  if (tid == 0) H->next = NEXT_NONE;
   bar_consumers(NC);
-  if (nk == cur_key) live = 1u;          // an overflow event asked for a live record
+  if (tid == 0) {
+    // the claim on the (new) current record, consumed by the next flush (after its rendezvous barrier)
+    H->mode = same ? ARGUS_ST_LIVE : atomicCAS(&gl.state[nk], ARGUS_ST_LAZY, ARGUS_ST_BUSY);
+  }
+  if (same) live = 1u;
   else { cur_key = nk; live = 0u; }
   return (unsigned long long)cur_key | (live ? PARK_LIVE : 0ull);
 }
@@ -482,8 +473,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       mbar_init(smem_u32(&H->full[k]), 1u);
       mbar_init(smem_u32(&H->empty[k]), (uint32_t)WPSTG);
     }
-    H->cur_key = KEY_NONE; H->pad0 = 0u; H->next_idx = KEY_NONE; H->mode = 0u;
-    H->n_finished = 0u; H->decision = 0u;
+    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   {
@@ -521,7 +511,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   const uint32_t a_slots = sbase + TAB_OFF, a_sumlo = a_slots + 16u * SCAP, a_sumhi = a_slots + 20u * SCAP,
                  a_mm = a_slots + 24u * SCAP;
   const uint32_t a_ring = sbase + stages, ring_bytes = (uint32_t)K * (uint32_t)(SUBE * 32);
-  const uint32_t a_nextidx = sbase + (uint32_t)offsetof(Hdr, next_idx);
+  const uint32_t a_nextidx = sbase + (uint32_t)offsetof(Hdr, next) + 4u;   // high word: the requested index
   const uint32_t bar_ring = (uint32_t)K * 8u;     // bytes of full[0..K)
   constexpr uint32_t EMPTY_OFF = MAXK * 8u;          // empty[k] sits MAXK*8 bytes after full[k]
   WarpSpan ws;
