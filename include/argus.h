@@ -32,7 +32,10 @@ extern "C" {
 #define ARGUS_ENOMEM  -5  /* host or device allocation of ctx workspace failed                  */
 
 /* ---- config flags ------------------------------------------------------------------------- */
-/* Performance hint (R18): records arrive grouped by (rank, step) — the segmented kernel is used.
+/* Performance hint (R18): records arrive grouped by (rank, step) — the segmented kernel reads them
+ * in place.  Without the hint argus_aggregate first groups the n events of the call by (rank, step)
+ * into a ctx-owned device workspace of n*32 bytes (allocated on first use, grown on demand; if it
+ * cannot be allocated the slower global-table kernel is used instead).
  * Results never depend on the hint; a violated hint only costs time. */
 #define ARGUS_FLAG_SORTED 0x1u
 
@@ -142,8 +145,8 @@ typedef struct argus_diag_out {
 
 typedef struct argus_ctx argus_ctx;  /* opaque */
 
-/* Create a context for one table geometry.  Allocates only small device workspace (per-record
- * state words, counters).  [host] cfg, [host] out. */
+/* Create a context for one table geometry.  Allocates only small device workspace (two u32 per
+ * record slot, counters); see ARGUS_FLAG_SORTED for the grouping workspace.  [host] cfg, [host] out. */
 int argus_create(const argus_config* cfg, argus_ctx** out);
 int argus_destroy(argus_ctx* ctx);
 
@@ -197,7 +200,7 @@ int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid);
 
 /* Tuning knobs for measurement (not needed for correctness): which = ARGUS_TUNE_*.  */
 #define ARGUS_TUNE_GRID_CTAS   1  /* persistent CTAs of the segmented kernel (0 = #SMs)  */
-#define ARGUS_TUNE_FORCE_PATH  2  /* 0 = by flags, 1 = segmented, 2 = global-table        */
+#define ARGUS_TUNE_FORCE_PATH  2  /* 0 = by flags, 1 = segmented, 2 = global-table, 3 = group then segmented */
 #define ARGUS_TUNE_SEG_VARIANT 3  /* thread/unroll geometry of the segmented kernel (0 = default) */
 int argus_tune(argus_ctx* ctx, int which, int64_t value);
 

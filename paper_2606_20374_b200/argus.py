@@ -15,7 +15,7 @@ from ._build import build_argus
 OK, EINVAL, ECUDA, ESIZE, ESTATE, ENOMEM = 0, -1, -2, -3, -4, -5
 FLAG_SORTED = 0x1
 TUNE_GRID_CTAS, TUNE_FORCE_PATH, TUNE_SEG_VARIANT = 1, 2, 3
-PATH_AUTO, PATH_SEGMENTED, PATH_GLOBAL = 0, 1, 2
+PATH_AUTO, PATH_SEGMENTED, PATH_GLOBAL, PATH_GROUPED = 0, 1, 2, 3
 
 EVENT_DTYPE = np.dtype(
     [("rank", "<u4"), ("step", "<u4"), ("sig", "<u4"), ("stream", "<u2"), ("phase", "<u2"),

@@ -65,7 +65,9 @@ struct Hdr {
   unsigned long long next;            // rendezvous request {lowest pending event index : 32 | its key : 32}
   uint32_t mode;                      // claim on the current key's record: LAZY = ours to write, LIVE, BUSY = another CTA's
   uint32_t n_finished;                // consumer warps that ran out of events
+  uint32_t ovf_n;                     // events parked in this CTA's overflow list since the last flush
 };
+constexpr uint32_t OVF_CAP = 4096;    // entries of a CTA's overflow list (16 bytes each, global memory)
 constexpr unsigned long long NEXT_NONE = ~0ull;
 static_assert(sizeof(Hdr) <= HDR_BYTES, "header");
 
@@ -185,6 +187,7 @@ struct WarpSpan {
 struct Glob {             // global-memory side of the kernel
   uint8_t* records;
   uint32_t* state;
+  uint4* ovf;             // this CTA's overflow list: {sig, 0, duration lo, duration hi} of events the compact cell refused
   argus_dims D;
 };
 
@@ -280,6 +283,8 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
   const long long tf0 = clock64();
 #endif
   uint32_t mode = *reinterpret_cast<volatile uint32_t*>(&H->mode);
+  uint32_t n_ovf = *reinterpret_cast<volatile uint32_t*>(&H->ovf_n);
+  n_ovf = n_ovf < OVF_CAP ? n_ovf : OVF_CAP;
   if (mode == ARGUS_ST_BUSY) {
     // another (resident, running) CTA owns this record and is writing it: wait for it, then merge
     if (tid == 0) {
@@ -338,7 +343,7 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
       }
       __stcs(cdst + 10u * sig + (i & 1u), v);
     }
-    if (fence_all) __threadfence();   // the callers go on with L2 atomics on this record at once
+    if (fence_all || n_ovf) __threadfence();   // L2 atomics on this record follow at once
   } else {
     // merge into a live record with L2 reductions (non-empty fields only)
     argus_cell* cells = reinterpret_cast<argus_cell*>(rec + D.cell_off);
@@ -380,6 +385,13 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
     __threadfence();
     atomicExch(&g.state[key], ARGUS_ST_LIVE);
   }
+  // the events the compact cells refused since the last flush: straight into the record (written or
+  // merged above) with L2 reductions; they commute with everybody else's, so publication need not wait
+  for (uint32_t i = tid; i < n_ovf; i += NC) {
+    const uint4 e = __ldcg(g.ovf + i);
+    global_cell_add(g.records, D, key, e.x, ((unsigned long long)e.w << 32) | e.z);
+  }
+  if (tid == 0) H->ovf_n = 0u;
   tb.clear(D.S, (uint32_t)tid, (uint32_t)NC);
   for (uint32_t k = tid; k < D.P; k += NC) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
@@ -446,7 +458,7 @@ __host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes
 template <int CW, int WPSTG, uint32_t SCAP>
 __global__ void __launch_bounds__((CW + 1) * 32, 1)
 aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta, uint8_t* records,
-                     uint32_t* state, unsigned long long* counters, argus_dims D) {
+                     uint32_t* state, unsigned long long* counters, uint4* ovf, argus_dims D) {
   constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG);
   static_assert(K >= 2 * (CW / WPSTG), "ring too shallow for this geometry");
   constexpr int NC = CW * 32;            // consumer threads
@@ -455,6 +467,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   static_assert(CW % WPSTG == 0, "geometry");
   Glob gl;
   gl.records = records; gl.state = state; gl.D = D;
+  gl.ovf = ovf + (size_t)blockIdx.x * OVF_CAP;
   const Table tb{SCAP};
   Hdr* H = hdr();
   constexpr uint32_t stages = (TAB_OFF + 32u * SCAP + 127u) & ~127u;   // byte offset of the stage ring in smem
@@ -473,7 +486,7 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       mbar_init(smem_u32(&H->full[k]), 1u);
       mbar_init(smem_u32(&H->empty[k]), (uint32_t)WPSTG);
     }
-    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u;
+    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u; H->ovf_n = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   {
@@ -655,38 +668,36 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
         if (fast) ARGUS_COMPACT_ADD(ok);
       }
       tried = false;
-      if (!ok && pending && key == cur_key && live) {
-        // the compact cell cannot take this event and the record is live: L2 atomics
-        global_cell_add(records, D, cur_key, sig, d);
-        ok = true;
+      if (!ok && pending && key == cur_key) {
+        // the compact cell cannot take this event: L2 atomics if the record is live, else the CTA's
+        // overflow list (applied at the flush); a full list asks for a live record at the rendezvous
+        if (live) {
+          global_cell_add(records, D, cur_key, sig, d);
+          ok = true;
+        } else {
+          const uint32_t oi = atomicAdd(&H->ovf_n, 1u);
+          if (oi < OVF_CAP) {
+            gl.ovf[oi] = make_uint4(sig, 0u, d32, (uint32_t)(d >> 32));
+            ok = true;
+          }
+        }
       }
-      // ---- spans of the folded events: warp-uniform fast path in registers, else ballot groups ------
-      if (__all_sync(FULL, ok && phase == ws.phase)) {
-        ws.mn = start < ws.mn ? start : ws.mn;
-        ws.mx = end > ws.mx ? end : ws.mx;
-        ws.n += 32u;
-      } else {
-        ws.flush(lane);
+      // ---- spans of the folded events.  A warp whose 32 events share one phase keeps the span in
+      // registers; a warp with mixed phases (ungrouped or boundary input) updates the shared
+      // accumulators lane by lane: test min/max with a plain load first (they rarely improve after
+      // the first few events), count with a 32-bit add (a CTA's span holds < 2^26 events: no carry).
+      {
         const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
         if (__all_sync(FULL, ok && phase == ph0)) {
-          ws.phase = ph0; ws.mn = start; ws.mx = end; ws.n = 32u;
-        } else {
-          uint32_t todo = __ballot_sync(FULL, ok);
-          while (todo) {
-            const int leader = __ffs((int)todo) - 1;
-            const uint32_t ph = __shfl_sync(FULL, phase, leader);
-            const bool grp_mine = ok && phase == ph;
-            const uint32_t g2 = __ballot_sync(FULL, grp_mine);
-            const long long a = warp_min_i64(grp_mine ? start : INT64_MAX);
-            const long long b = warp_max_i64(grp_mine ? end : INT64_MIN);
-            if (lane == leader) {
-              SpanAcc* sp = span_tab() + ph;
-              atomicMin(&sp->mn, a);
-              atomicMax(&sp->mx, b);
-              atomicAdd(&sp->n, (unsigned long long)__popc(g2));
-            }
-            todo &= ~g2;
-          }
+          if (ph0 != ws.phase) { ws.flush(lane); ws.phase = ph0; }
+          ws.mn = start < ws.mn ? start : ws.mn;
+          ws.mx = end > ws.mx ? end : ws.mx;
+          ws.n += 32u;
+        } else if (ok) {
+          SpanAcc* sp = span_tab() + phase;
+          if (start < *reinterpret_cast<volatile long long*>(&sp->mn)) atomicMin(&sp->mn, start);
+          if (end > *reinterpret_cast<volatile long long*>(&sp->mx)) atomicMax(&sp->mx, end);
+          atomicAdd(reinterpret_cast<uint32_t*>(&sp->n), 1u);
         }
       }
       if (ok) { pending = false; fast = false; }
@@ -741,9 +752,18 @@ cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* 
   if (per_cta > cap) per_cta = cap;
   per_cta = (per_cta + tile - 1) / tile * tile;
   const uint64_t ctas = (n + per_cta - 1) / per_cta;
+  if (ctx->ovf_ctas < ctas) {          // overflow lists, one per CTA (grow-only; 64 KB each)
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return e;
+    if (ctx->d_ovf) cudaFree(ctx->d_ovf);
+    ctx->d_ovf = nullptr; ctx->ovf_ctas = 0;
+    e = cudaMalloc(&ctx->d_ovf, ctas * OVF_CAP * sizeof(uint4));
+    if (e != cudaSuccess) return e;
+    ctx->ovf_ctas = ctas;
+  }
   aggregate_seg_kernel<CW, WPSTG, SCAP><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
-      ctx->d_counters, ctx->dims);
+      ctx->d_counters, static_cast<uint4*>(ctx->d_ovf), ctx->dims);
   return cudaGetLastError();
 }
 

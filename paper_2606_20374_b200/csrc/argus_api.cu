@@ -56,6 +56,7 @@ extern "C" int argus_create(const argus_config* cfg, argus_ctx** out) {
     e = cudaMalloc(&ctx->d_state, sizeof(uint32_t) * (size_t)D.R * D.T);
   }
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_hist, sizeof(uint32_t) * ((size_t)D.R * D.T + 1u));
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ingest_event, cudaEventDisableTiming);
   if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
   if (e != cudaSuccess) {
@@ -72,6 +73,9 @@ extern "C" int argus_destroy(argus_ctx* ctx) {
   cudaSetDevice(ctx->cfg.device);
   if (ctx->d_state) cudaFree(ctx->d_state);
   if (ctx->d_counters) cudaFree(ctx->d_counters);
+  if (ctx->d_hist) cudaFree(ctx->d_hist);
+  if (ctx->d_group) cudaFree(ctx->d_group);
+  if (ctx->d_ovf) cudaFree(ctx->d_ovf);
   if (ctx->ingest_event) cudaEventDestroy(ctx->ingest_event);
   for (uint32_t i = 0; i < ctx->n_slot_events; ++i) {
     cudaEventDestroy(ctx->slot_free[i]);
@@ -110,11 +114,23 @@ extern "C" int argus_ingest(argus_ctx* ctx, const argus_event* h_src, uint64_t n
   return ARGUS_OK;
 }
 
+// Path choice: grouped input (ARGUS_FLAG_SORTED) -> segmented kernel; ungrouped input -> group the
+// events by (rank, step) first, then the segmented kernel; the global-table kernel is what is left
+// when the table does not fit the segmented kernel or the grouping workspace cannot be allocated.
 static int aggregate_impl(argus_ctx* ctx, const argus_event* d_events, uint64_t n, void* d_records,
                           cudaStream_t s) {
   int path = ctx->tune_path;
-  if (path == 0) path = (ctx->cfg.flags & ARGUS_FLAG_SORTED) ? 1 : 2;
-  if (path == 1 && !argus_seg_supported(ctx)) path = 2;
+  if (path == 0) path = (ctx->cfg.flags & ARGUS_FLAG_SORTED) ? 1 : 3;
+  if ((path == 1 || path == 3) && !argus_seg_supported(ctx)) path = 2;
+  if (path == 3) {
+    cudaError_t e = argus_launch_partition(ctx, d_events, n, s);
+    if (e == cudaErrorMemoryAllocation) path = 2;
+    else {
+      CU(ctx, e);
+      d_events = ctx->d_group;
+      path = 1;
+    }
+  }
   if (path == 1) CU(ctx, argus_launch_aggregate_seg(ctx, d_events, n, d_records, s));
   else CU(ctx, argus_launch_aggregate_global(ctx, d_events, n, d_records, s));
   return ARGUS_OK;
@@ -234,7 +250,7 @@ extern "C" int argus_tune(argus_ctx* ctx, int which, int64_t value) {
       ctx->tune_variant = (int)value;
       return ARGUS_OK;
     case ARGUS_TUNE_FORCE_PATH:
-      if (value < 0 || value > 2) return ARGUS_EINVAL;
+      if (value < 0 || value > 3) return ARGUS_EINVAL;
       ctx->tune_path = (int)value;
       return ARGUS_OK;
     default:

@@ -27,6 +27,11 @@ struct argus_ctx {
   int max_smem_optin;
   uint32_t* d_state;          // [R*T]
   unsigned long long* d_counters;  // [2] n_valid, n_invalid
+  uint32_t* d_hist;           // [R*T + 1] group sizes / cursors of the partition pass
+  argus_event* d_group;       // grouping workspace of the partition pass (grown on demand)
+  uint64_t group_capacity;    // events d_group can hold
+  void* d_ovf;                // per-CTA overflow lists of the segmented kernel (grown on demand)
+  uint64_t ovf_ctas;          // CTAs d_ovf can serve
   void* d_records;            // table given to the last argus_reset
   cudaEvent_t ingest_event;   // recorded after every argus_ingest copy
   bool ingest_pending;
@@ -46,6 +51,7 @@ cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, ui
                                        void* d_records, cudaStream_t s);
 cudaError_t argus_launch_aggregate_global(argus_ctx* ctx, const argus_event* ev, uint64_t n,
                                           void* d_records, cudaStream_t s);
+cudaError_t argus_launch_partition(argus_ctx* ctx, const argus_event* ev, uint64_t n, cudaStream_t s);
 cudaError_t argus_launch_materialise_all(argus_ctx* ctx, void* d_records, cudaStream_t s);
 cudaError_t argus_launch_finalize(argus_ctx* ctx, void* d_records, argus_span* d_spans_out,
                                   cudaStream_t s);

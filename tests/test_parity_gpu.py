@@ -13,7 +13,7 @@ from paper_2606_20374_b200.workload import EVENT_DTYPE, build_workload, scaled
 
 pytestmark = pytest.mark.gpu
 
-PATH_SEG, PATH_GLOBAL = 1, 2
+PATH_SEG, PATH_GLOBAL, PATH_GROUPED = 1, 2, 3
 
 
 def _dims(spec):
@@ -34,7 +34,7 @@ def test_handworked_golden_gpu():
         ctx.close()
 
 
-@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL, PATH_GROUPED])
 def test_tiny_parity(path):
     wl = build_workload("tiny")
     ev = wl.expand_host()
@@ -42,7 +42,7 @@ def test_tiny_parity(path):
     assert (diag["sig_flags"][:, 17, 5] == 1).all() and diag["span_flags"][2, 1, 3] == 1
 
 
-@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL, PATH_GROUPED])
 def test_tiny_chunked_mid_rank_step(path):
     wl = build_workload("tiny")
     ev = wl.expand_host()
@@ -92,7 +92,7 @@ def _random_events(rnd, n, R, T, S, P, base, big):
 @pytest.mark.parametrize("seed,dims,big", [(1, (3, 2, 5, 2, 0), False), (2, (8, 3, 16, 4, 10), True),
                                            (3, (1, 1, 1, 1, 0), True), (4, (5, 1, 7, 3, 1000), True),
                                            (5, (2, 2, 3, 64, 5), True)])
-@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL, PATH_GROUPED])
 def test_random_with_invalid_and_overflow(seed, dims, big, path):
     R, T, S, P, base = dims
     ev = _random_events(random.Random(seed), 6000, R, T, S, P, base, big)
@@ -100,7 +100,7 @@ def test_random_with_invalid_and_overflow(seed, dims, big, path):
     assert o.n_invalid > 0
 
 
-@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
+@pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL, PATH_GROUPED])
 def test_empty_input(path):
     ev = np.zeros(0, dtype=EVENT_DTYPE)
     assert_parity(ev, 4, 2, 9, 3, 0, path=path)
@@ -161,9 +161,13 @@ def test_production_scaled_large_S():
 
 
 def test_unsorted_scaled():
+    # shuffled input: without the hint the events are grouped first (path 3), then the segmented kernel
     wl = build_workload(scaled("unsorted", n_ranks=64, n_events=20000))
     ev = wl.expand_host()
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False)
+    assert_parity(ev, *_dims(wl.spec), sorted_hint=False, path=PATH_GLOBAL)
+    # the shuffled events in uneven chunks: every call groups its own chunk
+    assert_parity(ev, *_dims(wl.spec), sorted_hint=False, cuts=[0, 7, 100_000, 100_001, 900_000, ev.size])
 
 
 def test_odd_rank_counts_select():
