@@ -263,11 +263,12 @@ def run_ours(args, world):
         "raw_event_gbs": 32 * value / 1e9,
         "hbm_frac_step": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
         "hbm_frac_step_vs_8tbs": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0,
-        "roofline": {"bound": "hbm", "kernel": "aggregate_seg_kernel" if not s.shuffle else "aggregate_global_kernel",
+        "roofline": {"bound": "hbm", "kernel": "aggregate_seg_kernel" if not s.shuffle else
+                     "argus_aggregate = partition_count/offsets/scan/scatter + aggregate_seg_kernel",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "kernel_ms": agg_ms,
                      "algorithmic_bytes": alg_bytes, "share_of_step": agg_ms / ms_step},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": 3 * args.steps,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": (7 if s.shuffle else 3) * args.steps,
         "counters": {"n_valid": n_valid, "n_invalid": n_invalid},
     }
     if world.size == 1 and not args.no_cpu_baseline:

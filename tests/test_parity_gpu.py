@@ -201,3 +201,13 @@ def test_device_expander_matches_host():
         h = wl.expand_host().view(np.uint8).reshape(-1)
         d = wl.expand_device().cpu().numpy()
         assert (h == d).all(), name
+
+
+def test_grouping_with_many_groups():
+    # R*T + 1 = 65,537 group counters do not fit shared memory: the grouping pass falls back to one
+    # global counter array (L2 atomics); R*T = 3,000 uses the per-CTA shared-memory histograms
+    rnd = random.Random(5)
+    for R, T in ((8192, 8), (1000, 3)):
+        rows = [(rnd.randrange(R + 1), 3 + rnd.randrange(T + 1), rnd.randrange(4), 0, rnd.randrange(2),
+                 rnd.randrange(10**6), 10**6 + rnd.randrange(10**5)) for _ in range(30000)]
+        assert_parity(make_events(rows), R, T, 4, 2, 3, sorted_hint=False)
