@@ -24,6 +24,7 @@
 // with coalesced 128-bit stores (no read-modify-write, no separate identity fill); any later
 // contribution to the same record merges with L2 reductions.  Correct for ANY event order; fast
 // when events are grouped by (rank, step) (R18).
+#include <cuda.h>
 #include <stddef.h>
 #include <stdio.h>
 
@@ -71,7 +72,7 @@ constexpr uint32_t OVF_CAP = 4096;    // entries of a CTA's overflow list (16 by
 constexpr unsigned long long NEXT_NONE = ~0ull;
 static_assert(sizeof(Hdr) <= HDR_BYTES, "header");
 
-extern __shared__ __align__(128) uint8_t smem[];
+extern __shared__ __align__(1024) uint8_t smem[];   // 1024: the 128-byte swizzle atom of the TMA stages
 
 // The compact table of one (rank, step), addressed by 32-bit offsets from the dynamic shared
 // window: slots[S] uint4 | sum_lo[S] u32 | sum_hi[S] u32 | mm[S] uint2 {~min, max}.
@@ -112,6 +113,18 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint3
       "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
       "[%0], [%1], %2, [%3], %4;" ::"r"(dst),
       "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+      : "memory");
+}
+// 2-D tiled TMA load of one stage: rows of 128 bytes (4 events) starting at row `row`, written to
+// shared memory with the 128-byte swizzle (16-byte chunk index XOR row & 7), which makes the
+// consumers' per-lane LDS.128 of 32-byte records bank-conflict free.  Rows beyond the tensor are
+// zero-filled and still count towards the transaction bytes.
+__device__ __forceinline__ void tma_load_rows(uint32_t dst, const CUtensorMap* tmap, uint32_t row,
+                                              uint32_t bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+      "[%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst),
+      "l"(tmap), "r"(0), "r"(row), "r"(bar), "l"(policy)
       : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
@@ -457,8 +470,9 @@ __host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes
 // layout is compiled for SCAP sigs (S <= SCAP), so every table address is base + sig * c + constant.
 template <int CW, int WPSTG, uint32_t SCAP>
 __global__ void __launch_bounds__((CW + 1) * 32, 1)
-aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta, uint8_t* records,
-                     uint32_t* state, unsigned long long* counters, uint4* ovf, argus_dims D) {
+aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __restrict__ ev, uint64_t n,
+                     uint64_t per_cta, uint8_t* records, uint32_t* state, unsigned long long* counters,
+                     uint4* ovf, argus_dims D) {
   constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG);
   static_assert(K >= 2 * (CW / WPSTG), "ring too shallow for this geometry");
   constexpr int NC = CW * 32;            // consumer threads
@@ -504,13 +518,18 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
       uint64_t policy;
       asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(policy));
       uint32_t slot = 0, round = 0;
+      const uint64_t rows_total = n >> 2;                 // whole 128-byte rows of the buffer: the tensor
+      const uint64_t row_cta = e0 >> 2;                   // e0 is a multiple of the tile, hence of 4
       for (uint32_t s = 0; s < n_sub; ++s) {
         if (round) mbar_wait(smem_u32(&H->empty[slot]), (round - 1u) & 1u);
-        const uint32_t cnt = (n_ev - s * SUBE < (uint32_t)SUBE) ? n_ev - s * SUBE : (uint32_t)SUBE;
         const uint32_t bar = smem_u32(&H->full[slot]);
-        mbar_expect_tx(bar, cnt * 32u);
-        tma_load_1d(smem_u32(smem + stages + slot * (SUBE * 32u)), src + 2 * (size_t)s * SUBE,
-                    cnt * 32u, bar, policy);
+        const uint64_t row = row_cta + (uint64_t)s * (SUBE / 4);
+        if (row < rows_total) {
+          mbar_expect_tx(bar, (uint32_t)SUBE * 32u);
+          tma_load_rows(smem_u32(smem + stages + slot * (SUBE * 32u)), &tmap, (uint32_t)row, bar, policy);
+        } else {
+          mbar_arrive(bar);      // only the last < 4 events live here: the consumers load them directly
+        }
         if (++slot == (uint32_t)K) { slot = 0; ++round; }
       }
     }
@@ -538,7 +557,10 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
   uint32_t par = (grp / (uint32_t)K) & 1u;
   uint32_t a_bar = sbase + (uint32_t)offsetof(Hdr, full) + slot0 * 8u;      // full[slot] of this iteration
   const uint32_t a_bar_end = sbase + (uint32_t)offsetof(Hdr, full) + bar_ring;
-  uint32_t a_ev = a_ring + slot0 * (uint32_t)(SUBE * 32) + wis * 1024u + (uint32_t)lane * 32u;
+  // this lane's record in a stage: row (lane >> 2) of the warp's 8 rows, 16-byte chunks 2q and 2q + 1
+  // (q = lane & 3), each XOR-swizzled with the row number: lo at a_ev, hi at a_ev ^ 16
+  uint32_t a_ev = a_ring + slot0 * (uint32_t)(SUBE * 32) + wis * 1024u + ((uint32_t)lane >> 2) * 128u +
+                  ((((uint32_t)lane & 3u) * 2u) ^ ((uint32_t)lane >> 2)) * 16u;
   uint32_t s = grp;                              // this warp's stage (tail iteration only)
   uint32_t my_pos = (uint32_t)warp * 32u;        // first event of this warp's chunk
 
@@ -605,18 +627,13 @@ aggregate_seg_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t per_cta,
     }
     uint4 lo, hi;
     if (have) {
-#ifdef ARGUS_SEG_SWZ
-      // lanes 4-7, 12-15, ... read their second half first: every quarter-warp then covers all
-      // eight 16-byte bank groups (conflict-free LDS.128) at the price of eight selects
-      const bool hsw = (lane & 4) != 0;
-      const uint4 A = lds128(a_ev + (hsw ? 16u : 0u));
-      const uint4 B = lds128(a_ev + (hsw ? 0u : 16u));
-      lo.x = hsw ? B.x : A.x; lo.y = hsw ? B.y : A.y; lo.z = hsw ? B.z : A.z; lo.w = hsw ? B.w : A.w;
-      hi.x = hsw ? A.x : B.x; hi.y = hsw ? A.y : B.y; hi.z = hsw ? A.z : B.z; hi.w = hsw ? A.w : B.w;
-#else
       lo = lds128(a_ev);
-      hi = lds128(a_ev + 16u);
-#endif
+      hi = lds128(a_ev ^ 16u);
+      if (TAIL) {
+        // the last n % 4 events of the buffer are not part of the tensor (whole 128-byte rows only)
+        const uint64_t g = e0 + my_pos + (uint32_t)lane;
+        if (g >= (n & ~3ull) && g < n) { lo = __ldg(ev + 2 * g); hi = __ldg(ev + 2 * g + 1); }
+      }
       __syncwarp();
       if (lane == 0) mbar_arrive(a_bar + EMPTY_OFF);
     } else {
@@ -761,8 +778,30 @@ cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* 
     if (e != cudaSuccess) return e;
     ctx->ovf_ctas = ctas;
   }
+  // the events as a 2-D tensor of whole 128-byte rows (4 events), loaded a stage (WPSTG * 8 rows) at a
+  // time with the 128-byte shared-memory swizzle; the last n % 4 events are read by the consumers
+  CUtensorMap tmap;
+  {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+    const encode_fn encode = reinterpret_cast<encode_fn>(ctx->fn_tmap_encode);
+    if (!encode) return cudaErrorNotSupported;
+    const uint64_t rows = n >> 2;
+    const cuuint64_t dims[2] = {32u, rows ? rows : 1u};          // u32 elements per row, rows
+    const cuuint64_t strides[1] = {128u};                        // bytes between rows
+    const cuuint32_t box[2] = {32u, (cuuint32_t)(WPSTG * 8)};
+    const cuuint32_t estr[2] = {1u, 1u};
+    // rows == 0: the map is never used (the producer only arrives), but it must still encode; point
+    // it at the buffer with a single row that is never fetched
+    const CUresult r = encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2u, const_cast<argus_event*>(ev), dims,
+                              strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
+  }
   aggregate_seg_kernel<CW, WPSTG, SCAP><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
-      reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
+      tmap, reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
       ctx->d_counters, static_cast<uint4*>(ctx->d_ovf), ctx->dims);
   return cudaGetLastError();
 }
@@ -782,7 +821,7 @@ cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, vo
 }  // namespace
 
 bool argus_seg_supported(const argus_ctx* ctx) {
-  return ctx->dims.S <= ARGUS_SEG_MAX_SIGS && (size_t)ctx->max_smem_optin >= SMEM_MAX;
+  return ctx->dims.S <= ARGUS_SEG_MAX_SIGS && (size_t)ctx->max_smem_optin >= SMEM_MAX && ctx->fn_tmap_encode != nullptr;
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,

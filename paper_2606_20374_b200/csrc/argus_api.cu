@@ -55,6 +55,14 @@ extern "C" int argus_create(const argus_config* cfg, argus_ctx** out) {
     ctx->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
     e = cudaMalloc(&ctx->d_state, sizeof(uint32_t) * (size_t)D.R * D.T);
   }
+  if (e == cudaSuccess) {
+    cudaDriverEntryPointQueryResult q;
+    void* fn = nullptr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      ctx->fn_tmap_encode = fn;
+    (void)cudaGetLastError();
+  }
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 2 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_hist, sizeof(uint32_t) * ((size_t)D.R * D.T + 1u));
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ingest_event, cudaEventDisableTiming);

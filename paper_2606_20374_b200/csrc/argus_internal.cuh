@@ -30,6 +30,7 @@ struct argus_ctx {
   uint32_t* d_hist;           // [R*T + 1] group sizes / cursors of the partition pass
   argus_event* d_group;       // grouping workspace of the partition pass (grown on demand)
   uint64_t group_capacity;    // events d_group can hold
+  void* fn_tmap_encode;       // cuTensorMapEncodeTiled, resolved through the runtime (no libcuda link)
   void* d_part;               // per-CTA key histograms of the partition pass [n_cta][R*T + 1]
   uint64_t part_rows;         // u32 entries d_part holds
   void* d_ovf;                // per-CTA overflow lists of the segmented kernel (grown on demand)
