@@ -17,6 +17,7 @@ __global__ void materialise_kernel(uint8_t* records, uint32_t* state, argus_dims
     if (state[rec] != ARGUS_ST_LAZY) continue;   // uniform per CTA; nobody else runs on this stream
     uint4* dst = reinterpret_cast<uint4*>(records + (size_t)rec * D.rec_bytes + D.span_off);
     for (uint32_t ch = threadIdx.x; ch < n_chunks; ch += blockDim.x) dst[ch] = argus_identity_chunk(D, ch);
+    argus_zero_sums_row(D, rec, threadIdx.x, blockDim.x);
     __syncthreads();
     if (threadIdx.x == 0) state[rec] = ARGUS_ST_LIVE;
   }
@@ -55,7 +56,7 @@ aggregate_global_kernel(const uint4* __restrict__ ev, uint64_t n, uint8_t* recor
       const long long end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
       uint32_t key;
       if (argus_event_key(D, lo.x, lo.y, lo.z, phase, start, end, key)) {
-        argus_global_accumulate(records + (size_t)key * D.rec_bytes, D, lo.z, phase, start, end);
+        argus_global_accumulate(records + (size_t)key * D.rec_bytes, key, D, lo.z, phase, start, end);
       } else {
         ++n_invalid;
       }

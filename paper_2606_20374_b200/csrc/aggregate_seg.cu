@@ -267,6 +267,7 @@ __device__ __noinline__ void global_cell_add(uint8_t* records, const argus_dims&
   argus_cell* cl = reinterpret_cast<argus_cell*>(records + (size_t)key * D.rec_bytes + D.cell_off) + sig;
   atomicAdd(reinterpret_cast<unsigned long long*>(&cl->count), 1ull);
   atomicAdd(reinterpret_cast<unsigned long long*>(&cl->sum_ns), d);
+  if (D.sums) atomicAdd(&D.sums[(size_t)key * D.S + sig], d);
   atomicMin(reinterpret_cast<unsigned long long*>(&cl->min_ns), d);
   atomicMax(reinterpret_cast<unsigned long long*>(&cl->max_ns), d);
   atomicAdd(&cl->hist[argus_bucket64(d)], 1u);
@@ -356,6 +357,11 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
       }
       __stcs(cdst + 10u * sig + (i & 1u), v);
     }
+    if (D.sums) {      // the record's row of the sum plane, sig-contiguous
+      unsigned long long* row = D.sums + (size_t)key * D.S;
+      for (uint32_t sig = tid; sig < D.S; sig += NC)
+        row[sig] = ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig);
+    }
     if (fence_all || n_ovf) __threadfence();   // L2 atomics on this record follow at once
   } else {
     // merge into a live record with L2 reductions (non-empty fields only)
@@ -375,8 +381,9 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
           }
         }
         atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].count), cnt);
-        atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].sum_ns),
-                  ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig));
+        const unsigned long long sm = ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig);
+        atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].sum_ns), sm);
+        if (D.sums) atomicAdd(&D.sums[(size_t)key * D.S + sig], sm);
         atomicMin(reinterpret_cast<unsigned long long*>(&cells[sig].min_ns),
                   (unsigned long long)(~m.x));
         atomicMax(reinterpret_cast<unsigned long long*>(&cells[sig].max_ns),

@@ -63,6 +63,14 @@ extern "C" int argus_create(const argus_config* cfg, argus_ctx** out) {
       ctx->fn_tmap_encode = fn;
     (void)cudaGetLastError();
   }
+  if (e == cudaSuccess) {
+    // the sum plane (8 bytes per cell, 5 % of the table) is an accelerator of argus_diagnose only:
+    // without it the gather falls back to the records
+    if (cudaMalloc(&D.sums, sizeof(unsigned long long) * (size_t)D.R * D.T * D.S) != cudaSuccess) {
+      D.sums = nullptr;
+      (void)cudaGetLastError();
+    }
+  }
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 2 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_hist, sizeof(uint32_t) * ((size_t)D.R * D.T + 1u));
   if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ingest_event, cudaEventDisableTiming);
@@ -81,6 +89,7 @@ extern "C" int argus_destroy(argus_ctx* ctx) {
   cudaSetDevice(ctx->cfg.device);
   if (ctx->d_state) cudaFree(ctx->d_state);
   if (ctx->d_counters) cudaFree(ctx->d_counters);
+  if (ctx->dims.sums) cudaFree(ctx->dims.sums);
   if (ctx->d_hist) cudaFree(ctx->d_hist);
   if (ctx->d_group) cudaFree(ctx->d_group);
   if (ctx->d_ovf) cudaFree(ctx->d_ovf);
@@ -106,6 +115,7 @@ extern "C" int argus_reset(argus_ctx* ctx, void* d_records, void* stream) {
   CU(ctx, cudaMemsetAsync(ctx->d_state, 0, sizeof(uint32_t) * (size_t)ctx->dims.R * ctx->dims.T, s));
   CU(ctx, cudaMemsetAsync(ctx->d_counters, 0, 2 * sizeof(unsigned long long), s));
   ctx->d_records = d_records;
+  ctx->finalized = false;
   ctx->last_stream = s;
   return ARGUS_OK;
 }
@@ -221,6 +231,7 @@ extern "C" int argus_phase_times(argus_ctx* ctx, void* d_records, argus_span* d_
   CU(ctx, cudaSetDevice(ctx->cfg.device));
   ctx->last_stream = s;
   CU(ctx, argus_launch_finalize(ctx, d_records, d_spans_out, s));
+  ctx->finalized = true;
   return ARGUS_OK;
 }
 
@@ -231,7 +242,9 @@ extern "C" int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus
   cudaStream_t s = (cudaStream_t)stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
   ctx->last_stream = s;
-  CU(ctx, argus_launch_diagnose(ctx, d_records, outs, s));
+  // the sum plane mirrors the table given to argus_reset, finalised by argus_phase_times
+  const bool use_sums = ctx->dims.sums != nullptr && d_records == ctx->d_records && ctx->finalized;
+  CU(ctx, argus_launch_diagnose(ctx, d_records, outs, use_sums, s));
   return ARGUS_OK;
 }
 

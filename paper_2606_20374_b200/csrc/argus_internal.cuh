@@ -18,6 +18,11 @@ struct argus_dims {
   uint32_t rec_bytes;   // 64 + 32*(P+1) + 160*S
   uint32_t span_off;    // 64
   uint32_t cell_off;    // 64 + 32*(P+1)
+  // Sum plane (ctx workspace, may be null): sums[(rank*T + t)*S + sig] mirrors cell.sum_ns of the table
+  // given to argus_reset, sig-contiguous, so that the cross-rank gather of argus_diagnose reads whole
+  // sectors of neighbouring sigs instead of one 32-byte sector per 160-byte cell.  Every kernel that
+  // writes a cell's sum (flush, merge, global path, identity fill) keeps it in step.
+  unsigned long long* sums;
 };
 
 struct argus_ctx {
@@ -38,6 +43,7 @@ struct argus_ctx {
   void* d_records;            // table given to the last argus_reset
   cudaEvent_t ingest_event;   // recorded after every argus_ingest copy
   bool ingest_pending;
+  bool finalized;             // argus_phase_times ran since the last argus_reset / argus_aggregate
   cudaStream_t copy_stream;   // internal, for argus_aggregate_host
   cudaEvent_t* slot_free;     // ring-slot reuse events (argus_aggregate_host)
   cudaEvent_t* slot_full;
@@ -59,7 +65,7 @@ cudaError_t argus_launch_materialise_all(argus_ctx* ctx, void* d_records, cudaSt
 cudaError_t argus_launch_finalize(argus_ctx* ctx, void* d_records, argus_span* d_spans_out,
                                   cudaStream_t s);
 cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
-                                  cudaStream_t s);
+                                  bool use_sums, cudaStream_t s);
 bool argus_seg_supported(const argus_ctx* ctx);
 
 // ---- device helpers shared by the kernels ------------------------------------------------------
@@ -84,13 +90,14 @@ __device__ __forceinline__ bool argus_event_key(const argus_dims& D, uint32_t ra
 // One event straight into a LIVE record with L2 atomics (global-table path, and the overflow path
 // of the segmented kernel).  min/max and span bounds are tested first: after the first few events
 // of a cell they rarely improve, so most events cost 3 reductions (count, sum, hist) + 1 (span n).
-__device__ __forceinline__ void argus_global_accumulate(uint8_t* rec, const argus_dims& D,
+__device__ __forceinline__ void argus_global_accumulate(uint8_t* rec, uint32_t key, const argus_dims& D,
                                                         uint32_t sig, uint32_t phase, int64_t start,
                                                         int64_t end) {
   uint64_t d = (uint64_t)(end - start);
   argus_cell* c = reinterpret_cast<argus_cell*>(rec + D.cell_off) + sig;
   atomicAdd(reinterpret_cast<unsigned long long*>(&c->count), 1ull);
   atomicAdd(reinterpret_cast<unsigned long long*>(&c->sum_ns), (unsigned long long)d);
+  if (D.sums) atomicAdd(&D.sums[(size_t)key * D.S + sig], (unsigned long long)d);
   if (d < *reinterpret_cast<volatile uint64_t*>(&c->min_ns))
     atomicMin(reinterpret_cast<unsigned long long*>(&c->min_ns), (unsigned long long)d);
   if (d > *reinterpret_cast<volatile uint64_t*>(&c->max_ns))
@@ -116,6 +123,13 @@ __device__ __forceinline__ uint4 argus_identity_chunk(const argus_dims& D, uint3
   uint32_t part = (chunk - span_chunks) % 10u;
   if (part == 1u) return make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0u, 0u);
   return make_uint4(0u, 0u, 0u, 0u);
+}
+
+// The sum-plane row of a record whose cells were just set to their identities.
+__device__ __forceinline__ void argus_zero_sums_row(const argus_dims& D, uint32_t key, uint32_t t, uint32_t nt) {
+  if (!D.sums) return;
+  unsigned long long* row = D.sums + (size_t)key * D.S;
+  for (uint32_t i = t; i < D.S; i += nt) row[i] = 0ull;
 }
 
 #endif  // __CUDACC__

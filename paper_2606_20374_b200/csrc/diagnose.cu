@@ -154,7 +154,7 @@ __device__ unsigned long long block_median(const unsigned long long (&v)[EPT], u
 
 template <int NT>
 __global__ void __launch_bounds__(NT)
-diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_out out) {
+diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_out out, bool use_sums) {
   __shared__ SelSmem sm;
   const int tid = threadIdx.x;
   const uint32_t F = D.S + D.P + 1u;
@@ -174,10 +174,15 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
     const uint32_t r = (uint32_t)(j * NT + tid);
     x[j] = 0ull;
     if (r < R) {
-      const ulonglong2 q = __ldg(reinterpret_cast<const ulonglong2*>(
-          records + ((size_t)r * D.T + t) * D.rec_bytes + off));
-      // cell: {count, sum} -> sum if count (R11: empty = 0);  span: {span_ns, n_events} -> span_ns
-      x[j] = is_sig ? (q.x ? q.y : 0ull) : q.x;
+      if (is_sig && use_sums) {
+        // the sum plane: 8 bytes per rank, neighbouring sigs (other CTAs) share the sector
+        x[j] = __ldg(D.sums + ((size_t)r * D.T + t) * D.S + f);
+      } else {
+        const ulonglong2 q = __ldg(reinterpret_cast<const ulonglong2*>(
+            records + ((size_t)r * D.T + t) * D.rec_bytes + off));
+        // cell: {count, sum} -> sum if count (R11: empty = 0);  span: {span_ns, n_events} -> span_ns
+        x[j] = is_sig ? (q.x ? q.y : 0ull) : q.x;
+      }
     }
   }
   // ---- a7 median, a8 MAD ----------------------------------------------------------------------
@@ -219,7 +224,7 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
 }  // namespace
 
 cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
-                                  cudaStream_t s) {
+                                  bool use_sums, cudaStream_t s) {
   const argus_dims& D = ctx->dims;
   if (o->rank_score) {
     cudaError_t e = cudaMemsetAsync(o->rank_score, 0, (size_t)D.T * D.R * sizeof(uint32_t), s);
@@ -228,8 +233,8 @@ cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const a
   const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);
   if (blocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
   const uint8_t* rec = static_cast<const uint8_t*>(d_records);
-  if (D.R <= 64u * EPT) diagnose_kernel<64><<<(unsigned)blocks, 64, 0, s>>>(rec, D, *o);
-  else if (D.R <= 256u * EPT) diagnose_kernel<256><<<(unsigned)blocks, 256, 0, s>>>(rec, D, *o);
-  else diagnose_kernel<1024><<<(unsigned)blocks, 1024, 0, s>>>(rec, D, *o);
+  if (D.R <= 64u * EPT) diagnose_kernel<64><<<(unsigned)blocks, 64, 0, s>>>(rec, D, *o, use_sums);
+  else if (D.R <= 256u * EPT) diagnose_kernel<256><<<(unsigned)blocks, 256, 0, s>>>(rec, D, *o, use_sums);
+  else diagnose_kernel<1024><<<(unsigned)blocks, 1024, 0, s>>>(rec, D, *o, use_sums);
   return cudaGetLastError();
 }

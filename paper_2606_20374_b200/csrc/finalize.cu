@@ -17,6 +17,7 @@ finalize_kernel(uint8_t* records, uint32_t* state, argus_span* spans_out, argus_
     if (state[rec] == ARGUS_ST_LAZY) {
       uint4* dst = reinterpret_cast<uint4*>(base + D.span_off);
       for (uint32_t ch = threadIdx.x; ch < n_chunks; ch += blockDim.x) dst[ch] = argus_identity_chunk(D, ch);
+      argus_zero_sums_row(D, rec, threadIdx.x, blockDim.x);
       __syncthreads();
       if (threadIdx.x == 0) state[rec] = ARGUS_ST_LIVE;
     }
