@@ -594,6 +594,9 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       if (b >= bucket32(~m.x) && b <= bucket32(m.y)) {                                   \
         if (nd > m.x) reds_max(a_m, nd); else reds_max(a_m + 4u, d32);                   \
         took = true;                                                                     \
+      } else if ((m.x | m.y) == 0u &&                                                    \
+                 atoms_cas64(a_m, 0ull, ((unsigned long long)d32 << 32) | nd) == 0ull) { \
+        took = true;                     /* first event of an empty cell */              \
       } else {                                                                           \
         took = mm_extend(a_m, d32);                                                      \
       }                                                                                  \
