@@ -467,20 +467,23 @@ __device__ __noinline__ unsigned long long park(const Glob& gl, bool pending, ui
 // alias a fill two rounds behind: bulk copies of different stages may complete out of order).
 constexpr uint32_t SMEM_MAX = 232448;          // 227 KB: the opt-in limit of one CTA on sm_100
 constexpr uint32_t ARGUS_SEG_MAX_SIGS = 5120;   // largest table capacity that still leaves a 6-stage ring
-__host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes, int spi) {
-  int k = (int)((SMEM_MAX - ((TAB_OFF + 32u * scap + 127u) & ~127u)) / stage_bytes);
+// MINB CTAs share an SM (228 KB, 1 KB of it reserved per CTA): small tables leave room for several
+// smaller CTAs, whose rendezvous and flushes then overlap with the streaming of their neighbours.
+__host__ __device__ constexpr uint32_t smem_budget(int minb) { return 233472u / (uint32_t)minb - 1024u; }
+__host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes, int spi, int minb) {
+  int k = (int)((smem_budget(minb) - ((TAB_OFF + 32u * scap + 127u) & ~127u)) / stage_bytes);
   if (k > MAXK) k = MAXK;
   return k - k % spi;
 }
 
 // CW consumer warps + 1 producer warp; a stage = WPSTG warps' worth of events (WPSTG KB); the table
 // layout is compiled for SCAP sigs (S <= SCAP), so every table address is base + sig * c + constant.
-template <int CW, int WPSTG, uint32_t SCAP>
-__global__ void __launch_bounds__((CW + 1) * 32, 1)
+template <int CW, int WPSTG, uint32_t SCAP, int MINB>
+__global__ void __launch_bounds__((CW + 1) * 32, MINB)
 aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __restrict__ ev, uint64_t n,
                      uint64_t per_cta, uint8_t* records, uint32_t* state, unsigned long long* counters,
                      uint4* ovf, argus_dims D) {
-  constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG);
+  constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG, MINB);
   static_assert(K >= 2 * (CW / WPSTG), "ring too shallow for this geometry");
   constexpr int NC = CW * 32;            // consumer threads
   constexpr int SUBE = WPSTG * 32;       // events per stage
@@ -639,22 +642,38 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     if (have) {
       lo = lds128(a_ev);
       hi = lds128(a_ev ^ 16u);
+#ifdef ARGUS_SEG_CHECK
+      {   // debug: the staged record must equal the record in global memory
+        const uint64_t gc = e0 + my_pos + (uint32_t)lane;
+        if (gc < (n & ~3ull) && gc < e1) {
+          const uint4 gl0 = ev[2 * gc], gl1 = ev[2 * gc + 1];
+          const bool bad_lo = gl0.x != lo.x || gl0.y != lo.y || gl0.z != lo.z || gl0.w != lo.w;
+          const bool bad_hi = gl1.x != hi.x || gl1.y != hi.y || gl1.z != hi.z || gl1.w != hi.w;
+          if (bad_lo || bad_hi)
+            printf("stage mismatch cta %d warp %d lane %d ev %llu lo %d hi %d (smem %08x %08x | glob %08x %08x)\n",
+                   blockIdx.x, warp, lane, (unsigned long long)gc, (int)bad_lo, (int)bad_hi, hi.x, hi.z, gl1.x, gl1.z);
+        }
+      }
+#endif
       if (TAIL) {
         // the last n % 4 events of the buffer are not part of the tensor (whole 128-byte rows only)
         const uint64_t g = e0 + my_pos + (uint32_t)lane;
         if (g >= (n & ~3ull) && g < n) { lo = __ldg(ev + 2 * g); hi = __ldg(ev + 2 * g + 1); }
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(a_bar + EMPTY_OFF);
     } else {
       lo = make_uint4(0u, 0u, 0u, 0u); hi = lo;
     }
+    const uint32_t a_rel = a_bar + EMPTY_OFF;     // released below, once every lane's loads have landed
     a_bar += (uint32_t)(SPI * 8); a_ev += (uint32_t)(SPI * SUBE * 32);
     if (a_bar >= a_bar_end) { a_bar -= bar_ring; par ^= 1u; a_ev -= ring_bytes; }
     if (TAIL) s += SPI;
     my_pos += NC;
 #ifdef ARGUS_SEG_NOCOMPUTE
-    n_invalid += (lo.x ^ hi.x) == 0x12345u;     // experiment: stream only (results are wrong)
+    {
+      const bool odd = ((lo.x ^ hi.x) == 0x12345u);   // experiment: stream only (results are wrong)
+      n_invalid += __all_sync(FULL, odd) ? 1u : 0u;
+      if (have && lane == 0) mbar_arrive(a_rel);
+    }
     return;
 #endif
 
@@ -670,7 +689,13 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
                 ((int)(hi.y | hi.w) >= 0) & ((uint32_t)(d >> 32) == 0u);
     bool pending, ok = false, tried = false;
     uint32_t key = cur_key;
-    if (__all_sync(FULL, fast)) {
+    const bool all_fast = __all_sync(FULL, fast);
+    // Release the stage only now: the vote above consumed both halves of every lane's record, so
+    // all 32 lanes' LDS have returned.  (An arrive issued right behind the loads can overtake
+    // them in a congested shared-memory pipe; with a short ring the refill then lands under a
+    // pending load — seen as records whose second half belonged to another event.)
+    if (have && lane == 0) mbar_arrive(a_rel);
+    if (all_fast) {
       // ---- hot path: the whole warp folds into the current table -------------------------------------
       ARGUS_COMPACT_ADD(ok);
       if (__all_sync(FULL, ok && phase == ws.phase)) {
@@ -761,17 +786,17 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
 }
 
-template <int CW, int WPSTG, uint32_t SCAP>
+template <int CW, int WPSTG, uint32_t SCAP, int MINB>
 cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records, cudaStream_t s) {
   constexpr size_t STAGE_BYTES = (size_t)WPSTG * 32 * 32;
-  constexpr int K = ring_depth(SCAP, (uint32_t)STAGE_BYTES, CW / WPSTG);
+  constexpr int K = ring_depth(SCAP, (uint32_t)STAGE_BYTES, CW / WPSTG, MINB);
   constexpr size_t smem_bytes = ((TAB_OFF + 32u * SCAP + 127u) & ~127u) + (size_t)K * STAGE_BYTES;
-  static_assert(smem_bytes <= SMEM_MAX, "shared memory");
+  static_assert(smem_bytes <= smem_budget(MINB), "shared memory");
   if ((size_t)ctx->max_smem_optin < smem_bytes) return cudaErrorInvalidConfiguration;
-  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP>,
+  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
   if (e != cudaSuccess) return e;
-  int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count;
+  int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count * MINB;
   // the u32 histogram counters of a CTA must not wrap between flushes: bound the span of one CTA
   const uint64_t tile = (uint64_t)CW * 32;
   const uint64_t cap = (1ull << 26) - tile;
@@ -810,7 +835,7 @@ cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* 
                               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
   }
-  aggregate_seg_kernel<CW, WPSTG, SCAP><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
+  aggregate_seg_kernel<CW, WPSTG, SCAP, MINB><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       tmap, reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
       ctx->d_counters, static_cast<uint4*>(ctx->d_ovf), ctx->dims);
   return cudaGetLastError();
@@ -821,11 +846,19 @@ template <int CW, int WPSTG>
 cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records,
                            cudaStream_t s) {
   const uint32_t S = ctx->dims.S;
-  if (S <= 1024u) return launch_cap<CW, WPSTG, 1024u>(ctx, ev, n, d_records, s);
-  if (S <= 2048u) return launch_cap<CW, WPSTG, 2048u>(ctx, ev, n, d_records, s);
-  if (S <= 4096u) return launch_cap<CW, WPSTG, 4096u>(ctx, ev, n, d_records, s);
-  if (S <= ARGUS_SEG_MAX_SIGS) return launch_cap<CW, WPSTG, ARGUS_SEG_MAX_SIGS>(ctx, ev, n, d_records, s);
+  if (S <= 1024u) return launch_cap<CW, WPSTG, 1024u, 1>(ctx, ev, n, d_records, s);
+  if (S <= 2048u) return launch_cap<CW, WPSTG, 2048u, 1>(ctx, ev, n, d_records, s);
+  if (S <= 4096u) return launch_cap<CW, WPSTG, 4096u, 1>(ctx, ev, n, d_records, s);
+  if (S <= ARGUS_SEG_MAX_SIGS) return launch_cap<CW, WPSTG, ARGUS_SEG_MAX_SIGS, 1>(ctx, ev, n, d_records, s);
   return cudaErrorInvalidConfiguration;
+}
+
+// Default geometry: as many CTAs per SM as the table leaves room for.
+cudaError_t launch_default(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records, cudaStream_t s) {
+  const uint32_t S = ctx->dims.S;
+  if (S <= 1024u) return launch_cap<9, 3, 1024u, 3>(ctx, ev, n, d_records, s);
+  if (S <= 2048u) return launch_cap<15, 5, 2048u, 2>(ctx, ev, n, d_records, s);
+  return launch_variant<30, 10>(ctx, ev, n, d_records, s);
 }
 
 }  // namespace
@@ -838,8 +871,8 @@ cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, ui
                                        void* d_records, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
   switch (ctx->tune_variant) {
-    case 1: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
-    case 2: return launch_variant<24, 8>(ctx, ev, n, d_records, s);
-    default: return launch_variant<30, 10>(ctx, ev, n, d_records, s);
+    case 1: return launch_variant<30, 10>(ctx, ev, n, d_records, s);   // one CTA per SM whatever S
+    case 2: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
+    default: return launch_default(ctx, ev, n, d_records, s);
   }
 }
