@@ -166,6 +166,12 @@ def test_unsorted_scaled():
     ev = wl.expand_host()
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False)
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False, path=PATH_GLOBAL)
+    # S <= 1024 runs three 9-warp CTAs per SM with a short stage ring (the geometry that once exposed a
+    # stage released before its loads had landed): repeat, the race was timing dependent
+    wl2 = build_workload(scaled("unsorted", n_ranks=64, n_events=20000, n_sigs=1000))
+    ev2 = wl2.expand_host()
+    for _ in range(3):
+        assert_parity(ev2, *_dims(wl2.spec), sorted_hint=False)
     # the shuffled events in uneven chunks: every call groups its own chunk
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False, cuts=[0, 7, 100_000, 100_001, 900_000, ev.size])
 
