@@ -268,7 +268,7 @@ def run_ours(args, world):
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "kernel_ms": agg_ms,
                      "algorithmic_bytes": alg_bytes, "share_of_step": agg_ms / ms_step},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": (7 if s.shuffle else 3) * args.steps,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": (8 if s.shuffle else 4) * args.steps,
         "counters": {"n_valid": n_valid, "n_invalid": n_invalid},
     }
     if world.size == 1 and not args.no_cpu_baseline:

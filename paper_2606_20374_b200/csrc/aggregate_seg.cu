@@ -873,6 +873,11 @@ cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, ui
   switch (ctx->tune_variant) {
     case 1: return launch_variant<30, 10>(ctx, ev, n, d_records, s);   // one CTA per SM whatever S
     case 2: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
+    case 3: return launch_cap<30, 5, 4096u, 1>(ctx, ev, n, d_records, s);
+    case 4: return launch_cap<30, 3, 4096u, 1>(ctx, ev, n, d_records, s);
+    case 5: return launch_cap<30, 15, 4096u, 1>(ctx, ev, n, d_records, s);
+    case 6: return launch_cap<30, 2, 4096u, 1>(ctx, ev, n, d_records, s);
+    case 7: return launch_cap<28, 7, 4096u, 1>(ctx, ev, n, d_records, s);
     default: return launch_default(ctx, ev, n, d_records, s);
   }
 }

@@ -93,6 +93,7 @@ extern "C" int argus_destroy(argus_ctx* ctx) {
   if (ctx->d_hist) cudaFree(ctx->d_hist);
   if (ctx->d_group) cudaFree(ctx->d_group);
   if (ctx->d_ovf) cudaFree(ctx->d_ovf);
+  if (ctx->d_diag_todo) cudaFree(ctx->d_diag_todo);
   if (ctx->d_part) cudaFree(ctx->d_part);
   if (ctx->ingest_event) cudaEventDestroy(ctx->ingest_event);
   for (uint32_t i = 0; i < ctx->n_slot_events; ++i) {

@@ -38,6 +38,8 @@ struct argus_ctx {
   void* fn_tmap_encode;       // cuTensorMapEncodeTiled, resolved through the runtime (no libcuda link)
   void* d_part;               // per-CTA key histograms of the partition pass [n_cta][R*T + 1]
   uint64_t part_rows;         // u32 entries d_part holds
+  void* d_diag_todo;          // argus_diagnose: one byte per series, set by the 32-bit pass for the 64-bit pass
+  uint64_t diag_todo_len;
   void* d_ovf;                // per-CTA overflow lists of the segmented kernel (grown on demand)
   uint64_t ovf_ctas;          // CTAs d_ovf can serve
   void* d_records;            // table given to the last argus_reset

@@ -23,12 +23,15 @@ struct SelSmem {
   uint32_t pick_digit, pick_before, pick_count;
 };
 
-template <int NT>
-__device__ __forceinline__ void block_minmax(unsigned long long mn, unsigned long long mx, SelSmem& sm,
-                                             unsigned long long& omn, unsigned long long& omx) {
+template <typename K> __device__ __forceinline__ int top_bit(K v);     // index of the leading one (v != 0)
+template <> __device__ __forceinline__ int top_bit<unsigned long long>(unsigned long long v) { return 63 - __clzll((long long)v); }
+template <> __device__ __forceinline__ int top_bit<uint32_t>(uint32_t v) { return 31 - __clz((int)v); }
+
+template <int NT, typename K>
+__device__ __forceinline__ void block_minmax(K mn, K mx, SelSmem& sm, K& omn, K& omx) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
-    unsigned long long a = __shfl_xor_sync(FULL, mn, o), b = __shfl_xor_sync(FULL, mx, o);
+    K a = __shfl_xor_sync(FULL, mn, o), b = __shfl_xor_sync(FULL, mx, o);
     mn = a < mn ? a : mn;
     mx = b > mx ? b : mx;
   }
@@ -36,11 +39,11 @@ __device__ __forceinline__ void block_minmax(unsigned long long mn, unsigned lon
   __syncthreads();
   if (lane == 0) { sm.red_a[w] = mn; sm.red_b[w] = mx; }
   __syncthreads();
-  mn = lane < NT / 32 ? sm.red_a[lane] : ~0ull;
-  mx = lane < NT / 32 ? sm.red_b[lane] : 0ull;
+  mn = lane < NT / 32 ? (K)sm.red_a[lane] : (K)~(K)0;
+  mx = lane < NT / 32 ? (K)sm.red_b[lane] : (K)0;
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) {
-    unsigned long long a = __shfl_xor_sync(FULL, mn, o), b = __shfl_xor_sync(FULL, mx, o);
+    K a = __shfl_xor_sync(FULL, mn, o), b = __shfl_xor_sync(FULL, mx, o);
     mn = a < mn ? a : mn;
     mx = b > mx ? b : mx;
   }
@@ -62,23 +65,23 @@ __device__ __forceinline__ void block_sum2(uint32_t a, uint32_t b, SelSmem& sm, 
 }
 
 // k-th smallest (0-based) of the block's values v[j] (element index j*NT + tid < R).  Exact.
-template <int NT>
-__device__ unsigned long long block_select(const unsigned long long (&v)[EPT], uint32_t R, uint32_t k,
-                                           SelSmem& sm) {
+template <int NT, typename K>
+__device__ K block_select(const K (&v)[EPT], uint32_t R, uint32_t k, SelSmem& sm) {
   const int tid = threadIdx.x;
-  unsigned long long mn = ~0ull, mx = 0ull;
+  constexpr int TOP = (int)sizeof(K) * 8 - 1;
+  K mn = (K)~(K)0, mx = (K)0;
 #pragma unroll
   for (int j = 0; j < EPT; ++j)
     if ((uint32_t)(j * NT + tid) < R) { mn = v[j] < mn ? v[j] : mn; mx = v[j] > mx ? v[j] : mx; }
-  block_minmax<NT>(mn, mx, sm, mn, mx);
+  block_minmax<NT, K>(mn, mx, sm, mn, mx);
   if (mn == mx) return mn;
-  int top = 63 - __clzll((long long)(mn ^ mx));          // highest bit where candidates differ
-  unsigned long long prefix = (top == 63) ? 0ull : (mn >> (top + 1)) << (top + 1);
-  unsigned long long pmask = (top == 63) ? 0ull : (~0ull << (top + 1));  // bits already fixed
+  int top = top_bit<K>(mn ^ mx);                         // highest bit where candidates differ
+  K prefix = (top == TOP) ? (K)0 : (K)((mn >> (top + 1)) << (top + 1));
+  K pmask = (top == TOP) ? (K)0 : (K)(~(K)0 << (top + 1));   // bits already fixed
   int hi_bit = top;
   for (;;) {
     const int shift = hi_bit >= 7 ? hi_bit - 7 : 0;
-    const uint32_t dmask = (uint32_t)((1ull << (hi_bit - shift + 1)) - 1ull);
+    const uint32_t dmask = (1u << (hi_bit - shift + 1)) - 1u;
     __syncthreads();
     sm.hist[tid & 255] = 0u;
     if (NT < 256) for (int i = tid; i < 256; i += NT) sm.hist[i] = 0u;
@@ -113,8 +116,8 @@ __device__ unsigned long long block_select(const unsigned long long (&v)[EPT], u
     __syncthreads();
     const uint32_t digit = sm.pick_digit, cnt = sm.pick_count;
     k -= sm.pick_before;
-    prefix |= (unsigned long long)digit << shift;
-    pmask |= (unsigned long long)dmask << shift;
+    prefix |= (K)digit << shift;
+    pmask |= (K)dmask << shift;
     if (shift == 0) return prefix;
     if (cnt == 1u) {
       // a single candidate is left: whoever holds it publishes it
@@ -122,22 +125,22 @@ __device__ unsigned long long block_select(const unsigned long long (&v)[EPT], u
       for (int j = 0; j < EPT; ++j)
         if ((uint32_t)(j * NT + tid) < R && (v[j] & pmask) == prefix) sm.bcast[0] = v[j];
       __syncthreads();
-      return sm.bcast[0];
+      return (K)sm.bcast[0];
     }
     hi_bit = shift - 1;
   }
 }
 
 // median (R10) of the block's values: lo = v_(k), hi = v_(k+1 if R even), med = lo + (hi-lo)/2
-template <int NT>
-__device__ unsigned long long block_median(const unsigned long long (&v)[EPT], uint32_t R, SelSmem& sm) {
+template <int NT, typename K>
+__device__ K block_median(const K (&v)[EPT], uint32_t R, SelSmem& sm) {
   const int tid = threadIdx.x;
   const uint32_t k = (R - 1) / 2;
-  const unsigned long long lo = block_select<NT>(v, R, k, sm);
+  const K lo = block_select<NT, K>(v, R, k, sm);
   if ((R & 1u) != 0u) return lo;
   // hi = v[R/2] = v[k+1]: equals lo when at least k+2 values are <= lo, else the smallest value > lo
   uint32_t le = 0;
-  unsigned long long gt_min = ~0ull;
+  K gt_min = (K)~(K)0;
 #pragma unroll
   for (int j = 0; j < EPT; ++j)
     if ((uint32_t)(j * NT + tid) < R) {
@@ -146,16 +149,22 @@ __device__ unsigned long long block_median(const unsigned long long (&v)[EPT], u
     }
   uint32_t le_all, dummy;
   block_sum2<NT>(le, 0u, sm, le_all, dummy);
-  unsigned long long mn, mx;
-  block_minmax<NT>(gt_min, 0ull, sm, mn, mx);
-  const unsigned long long hi = (le_all >= k + 2u) ? lo : mn;
-  return lo + (hi - lo) / 2ull;
+  K mn, mx;
+  block_minmax<NT, K>(gt_min, (K)0, sm, mn, mx);
+  const K hi = (le_all >= k + 2u) ? lo : mn;
+  return lo + (hi - lo) / (K)2;
 }
 
-template <int NT>
-__global__ void __launch_bounds__(NT)
-diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_out out, bool use_sums) {
+// K = uint32_t: the fast pass.  A series whose values span less than 2^32 (the usual case: per-rank
+// sums of one kernel differ by far less than 4.29 s) is selected on exact 32-bit offsets from its
+// minimum — half the registers, twice the resident CTAs; |x - med| fits 32 bits too.  A wider series is
+// only marked in todo[].  K = unsigned long long: the second pass, which does the marked series.
+template <int NT, typename K>
+__global__ void __launch_bounds__(NT, (sizeof(K) == 4 && NT <= 256) ? 1024 / NT : 1)
+diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_out out, bool use_sums,
+                uint8_t* __restrict__ todo) {
   __shared__ SelSmem sm;
+  if (sizeof(K) == 8 && !todo[blockIdx.x]) return;
   const int tid = threadIdx.x;
   const uint32_t F = D.S + D.P + 1u;
   const uint32_t t = blockIdx.x / F, f = blockIdx.x % F;
@@ -186,11 +195,27 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
     }
   }
   // ---- a7 median, a8 MAD ----------------------------------------------------------------------
-  const unsigned long long med = block_median<NT>(x, R, sm);
-  unsigned long long dev[EPT];
+  K v[EPT];
+  unsigned long long base = 0ull;
+  if (sizeof(K) == 4) {
+    unsigned long long xmn = ~0ull, xmx = 0ull;
 #pragma unroll
-  for (int j = 0; j < EPT; ++j) dev[j] = x[j] >= med ? x[j] - med : med - x[j];
-  const unsigned long long mad = block_median<NT>(dev, R, sm);
+    for (int j = 0; j < EPT; ++j)
+      if ((uint32_t)(j * NT + tid) < R) { xmn = x[j] < xmn ? x[j] : xmn; xmx = x[j] > xmx ? x[j] : xmx; }
+    block_minmax<NT, unsigned long long>(xmn, xmx, sm, xmn, xmx);
+    const bool wide = xmx - xmn > 0xFFFFFFFFull;
+    if (tid == 0) todo[blockIdx.x] = wide ? 1 : 0;
+    if (wide) return;
+    base = xmn;
+  }
+#pragma unroll
+  for (int j = 0; j < EPT; ++j) v[j] = (uint32_t)(j * NT + tid) < R ? (K)(x[j] - base) : (K)0;
+  const K med_k = block_median<NT, K>(v, R, sm);
+  K dev[EPT];
+#pragma unroll
+  for (int j = 0; j < EPT; ++j) dev[j] = v[j] >= med_k ? v[j] - med_k : med_k - v[j];
+  const K mad_k = block_median<NT, K>(dev, R, sm);
+  const unsigned long long med = base + med_k, mad = mad_k;
   const unsigned long long thr = mad > 0xFFFFFFFFFFFFFFFFull / 3ull ? 0xFFFFFFFFFFFFFFFFull : 3ull * mad;  // R12
   // ---- flags + roll-ups -------------------------------------------------------------------------
   uint8_t* fl = is_sig ? out.sig_flags : out.span_flags;
@@ -201,7 +226,7 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
     const uint32_t r = (uint32_t)(j * NT + tid);
     if (r < R) {
       uint8_t g = ARGUS_FLAG_NONE;
-      if (dev[j] > thr) g = x[j] > med ? ARGUS_FLAG_HIGH : ARGUS_FLAG_LOW;   // R13, R14
+      if ((unsigned long long)dev[j] > thr) g = v[j] > med_k ? ARGUS_FLAG_HIGH : ARGUS_FLAG_LOW;   // R13, R14
       nh += g == ARGUS_FLAG_HIGH;
       nl += g == ARGUS_FLAG_LOW;
       if (fl) fl[series * R + r] = g;
@@ -233,8 +258,26 @@ cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const a
   const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);
   if (blocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
   const uint8_t* rec = static_cast<const uint8_t*>(d_records);
-  if (D.R <= 64u * EPT) diagnose_kernel<64><<<(unsigned)blocks, 64, 0, s>>>(rec, D, *o, use_sums);
-  else if (D.R <= 256u * EPT) diagnose_kernel<256><<<(unsigned)blocks, 256, 0, s>>>(rec, D, *o, use_sums);
-  else diagnose_kernel<1024><<<(unsigned)blocks, 1024, 0, s>>>(rec, D, *o, use_sums);
+  if (ctx->diag_todo_len < blocks) {       // one byte per series (grow-only)
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return e;
+    if (ctx->d_diag_todo) cudaFree(ctx->d_diag_todo);
+    ctx->d_diag_todo = nullptr; ctx->diag_todo_len = 0;
+    e = cudaMalloc(&ctx->d_diag_todo, blocks);
+    if (e != cudaSuccess) return e;
+    ctx->diag_todo_len = blocks;
+  }
+  uint8_t* todo = static_cast<uint8_t*>(ctx->d_diag_todo);
+  const unsigned nb = (unsigned)blocks;
+  if (D.R <= 64u * EPT) {
+    diagnose_kernel<64, uint32_t><<<nb, 64, 0, s>>>(rec, D, *o, use_sums, todo);
+    diagnose_kernel<64, unsigned long long><<<nb, 64, 0, s>>>(rec, D, *o, use_sums, todo);
+  } else if (D.R <= 256u * EPT) {
+    diagnose_kernel<256, uint32_t><<<nb, 256, 0, s>>>(rec, D, *o, use_sums, todo);
+    diagnose_kernel<256, unsigned long long><<<nb, 256, 0, s>>>(rec, D, *o, use_sums, todo);
+  } else {
+    diagnose_kernel<1024, uint32_t><<<nb, 1024, 0, s>>>(rec, D, *o, use_sums, todo);
+    diagnose_kernel<1024, unsigned long long><<<nb, 1024, 0, s>>>(rec, D, *o, use_sums, todo);
+  }
   return cudaGetLastError();
 }
