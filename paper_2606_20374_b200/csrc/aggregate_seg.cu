@@ -107,14 +107,6 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
                : "memory");
 }
-__device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint32_t bytes,
-                                            uint32_t bar, uint64_t policy) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
-      "[%0], [%1], %2, [%3], %4;" ::"r"(dst),
-      "l"(src), "r"(bytes), "r"(bar), "l"(policy)
-      : "memory");
-}
 // 2-D tiled TMA load of one stage: rows of 128 bytes (4 events) starting at row `row`, written to
 // shared memory with the 128-byte swizzle (16-byte chunk index XOR row & 7), which makes the
 // consumers' per-lane LDS.128 of 32-byte records bank-conflict free.  Rows beyond the tensor are
@@ -503,7 +495,6 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   const uint32_t n_ev = (uint32_t)(e1 - e0);
   const uint32_t n_sub = (n_ev + SUBE - 1) / SUBE;
   const uint32_t n_iter = (n_ev + NC - 1) / NC;
-  const uint4* src = ev + 2 * e0;
 
   if (tid == 0) {
     for (int k = 0; k < K; ++k) {
@@ -873,11 +864,6 @@ cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, ui
   switch (ctx->tune_variant) {
     case 1: return launch_variant<30, 10>(ctx, ev, n, d_records, s);   // one CTA per SM whatever S
     case 2: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
-    case 3: return launch_cap<30, 5, 4096u, 1>(ctx, ev, n, d_records, s);
-    case 4: return launch_cap<30, 3, 4096u, 1>(ctx, ev, n, d_records, s);
-    case 5: return launch_cap<30, 15, 4096u, 1>(ctx, ev, n, d_records, s);
-    case 6: return launch_cap<30, 2, 4096u, 1>(ctx, ev, n, d_records, s);
-    case 7: return launch_cap<28, 7, 4096u, 1>(ctx, ev, n, d_records, s);
     default: return launch_default(ctx, ev, n, d_records, s);
   }
 }
