@@ -3,18 +3,23 @@
 spans -> cross-rank median/MAD diagnosis (BASELINE.json `metric`), on seeded synthetic events.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload production] [--impl ours|reference]
+                  [--scaling weak|strong]
 
 One step = one pass of the whole path over the workload: argus_reset + argus_aggregate +
 argus_phase_times + argus_diagnose.  `value` is timed with CUDA events with the events resident in
 HBM; `e2e` is the same step through argus_aggregate_host with HOST (pinned) buffers: the 256 MiB
-chunked host->device copies and the device->host read of the diagnosis are inside the timed region.
-Prints ONE JSON line on rank 0.  `--impl reference` times the CPU oracle (oracle/) instead.
+chunked host->device copies and the device->host read of the diagnosis are inside the timed region,
+and its outputs are compared with the resident leg's.  Prints ONE JSON line on rank 0.
+`--impl reference` times the CPU oracle (oracle/) instead.  `--gpus N` (N > 1) outside torchrun
+re-launches itself under torch.distributed.run with N ranks, or fails if the box has fewer GPUs.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
+import subprocess
 import sys
 import threading
 import time
@@ -94,23 +99,34 @@ class ClockSampler(threading.Thread):
 
 # ---------------------------------------------------------------------------------------------
 def oracle_sample(wl, n_ranks_sample: int, threads: int):
-    """Time the oracle, as it stands, on the first `n_ranks_sample` ranks of the workload."""
+    """Time the oracle, as it stands (one thread), on the first `n_ranks_sample` ranks of the
+    workload; the events are expanded on the host in blocks of ranks (untimed) so that a whole config
+    fits host memory.  Returns (events, oracle seconds, oracle object)."""
     from oracle import Oracle
     s = wl.spec
+    dt, n_ev = 0.0, 0
     if s.shuffle:
         ev = wl.expand_host(0, s.n_ranks, threads=threads)
         ev = ev[: n_ranks_sample * s.n_steps * s.n_events]
-        R = s.n_ranks
+        o = Oracle(s.n_ranks, s.n_steps, s.n_sigs, s.n_phases, s.step_base)
+        t0 = time.perf_counter()
+        o.aggregate(ev)
+        dt += time.perf_counter() - t0
+        n_ev = ev.size
     else:
-        ev = wl.expand_host(0, n_ranks_sample, threads=threads)
-        R = n_ranks_sample
-    o = Oracle(R, s.n_steps, s.n_sigs, s.n_phases, s.step_base)
+        o = Oracle(n_ranks_sample, s.n_steps, s.n_sigs, s.n_phases, s.step_base)
+        block = max(1, 40_000_000 // (s.n_steps * s.n_events))       # ~1.3 GB of events per block
+        for lo in range(0, n_ranks_sample, block):
+            ev = wl.expand_host(lo, min(n_ranks_sample, lo + block), threads=threads)
+            t0 = time.perf_counter()
+            o.aggregate(ev)
+            dt += time.perf_counter() - t0
+            n_ev += ev.size
     t0 = time.perf_counter()
-    o.aggregate(ev)
     o.phase_times()
     o.diagnose()
-    dt = time.perf_counter() - t0
-    return ev.size, dt
+    dt += time.perf_counter() - t0
+    return n_ev, dt, o
 
 
 def run_reference(args, world):
@@ -124,7 +140,7 @@ def run_reference(args, world):
     threads = os.cpu_count() or 1
     times, n_ev = [], 0
     for i in range(args.warmup + args.steps):
-        n_ev, dt = oracle_sample(wl, sample_ranks, threads)
+        n_ev, dt, _ = oracle_sample(wl, sample_ranks, threads)
         if i >= args.warmup:
             times.append(dt)
     t = float(np.mean(times))
@@ -143,6 +159,10 @@ def run_reference(args, world):
 
 
 # ---------------------------------------------------------------------------------------------
+def _ms(pairs):
+    return [a.elapsed_time(b) for a, b in pairs]
+
+
 def run_ours(args, world):
     import torch
     from paper_2606_20374_b200 import argus as A
@@ -152,6 +172,9 @@ def run_ours(args, world):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    if args.scaling == "strong" and world.size > 1:
+        from paper_2606_20374_b200 import sharded
+        return sharded.bench_strong(args, world, METRIC, measured_peak_gbs, ClockSampler)
     torch.cuda.set_device(world.local_rank)
     dev = world.local_rank
     wl0 = build_workload(args.workload)
@@ -161,9 +184,8 @@ def run_ours(args, world):
     n = s.total_events
 
     d_ev = wl.expand_device(device=f"cuda:{dev}")
-    ctx = A.Argus(s.n_ranks, s.n_steps, s.n_sigs, s.n_phases, s.step_base, sorted_hint=not s.shuffle, device=dev)
-    if args.variant:
-        ctx.tune(A.TUNE_SEG_VARIANT, args.variant)
+    ctx = A.Argus(s.n_ranks, s.n_steps, s.n_sigs, s.n_phases, s.step_base, sorted_hint=not s.shuffle,
+                  device=dev, max_ungrouped_events=n if s.shuffle else 0)
     rec = ctx.alloc_records()
     outs = ctx.alloc_diag()
     torch.cuda.synchronize()
@@ -177,6 +199,8 @@ def run_ours(args, world):
             ev_pairs[1].record()
         ctx.phase_times(rec)
         ctx.diagnose(rec, outs)
+        if ev_pairs is not None:
+            ev_pairs[2].record()
 
     for _ in range(args.warmup):
         step()
@@ -185,22 +209,29 @@ def run_ours(args, world):
 
     sampler = ClockSampler(dev)
     sampler.start()
-    t_beg, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    pairs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    mk = lambda: torch.cuda.Event(enable_timing=True)
+    t_beg, t_end = mk(), mk()
+    marks = [(mk(), mk(), mk()) for _ in range(args.steps)]
+    k0, m0 = ctx.launch_count()
     torch.cuda.synchronize()
     t_beg.record()
     for i in range(args.steps):
-        step(pairs[i])
+        step(marks[i])
     t_end.record()
     torch.cuda.synchronize()
     clocks = sampler.stop()
+    k1, m1 = ctx.launch_count()
     D.barrier(world)
     ms_total = D.max_over_ranks(world, t_beg.elapsed_time(t_end))
     ms_step = ms_total / args.steps
-    agg_ms = float(np.mean([a.elapsed_time(b) for a, b in pairs]))
+    agg_list = _ms([(a, b) for a, b, _ in marks])
+    agg_ms = float(np.mean(agg_list))
+    # per-step durations (reset of step i+1 is two tiny memsets: attributed to the step they precede)
+    step_list = [marks[i][0].elapsed_time(marks[i][2]) for i in range(args.steps)]
     n_valid, n_invalid = ctx.stats()
     total_events = D.sum_over_ranks(world, float(n))
     value = total_events / (ms_step * 1e-3)
+    resident = {k: v.clone() for k, v in outs.items()}
 
     # ---- e2e: HOST buffers through argus_aggregate_host, copies inside the timed region ----------
     e2e = None
@@ -214,6 +245,9 @@ def run_ours(args, world):
             d_ring = torch.empty(RING_SLOTS * chunk * 32, dtype=torch.uint8, device=f"cuda:{dev}")
             h_out = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True) for k, v in outs.items()}
             d2h = sum(v.numel() * v.element_size() for v in outs.values())
+            rec_keep = rec.clone()
+            for v in outs.values():
+                v.zero_()
 
             def e2e_step():
                 ctx.reset(rec)
@@ -227,17 +261,47 @@ def run_ours(args, world):
             e2e_step()
             torch.cuda.synchronize()
             D.barrier(world)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a, b = mk(), mk()
             a.record()
             for _ in range(e2e_steps):
                 e2e_step()
             b.record()
             torch.cuda.synchronize()
             e_ms = D.max_over_ranks(world, a.elapsed_time(b)) / e2e_steps
+            # the e2e leg checks itself: same table bytes, same six outputs (device and host copies),
+            # same counters as the resident leg
+            nv2, ni2 = ctx.stats()
+            verified = bool(torch.equal(rec, rec_keep)) and (nv2, ni2) == (n_valid, n_invalid)
+            for k in outs:
+                verified = verified and bool(torch.equal(outs[k], resident[k])) and \
+                    bool(torch.equal(h_out[k], resident[k].cpu()))
+            del rec_keep
+            # overlap efficiency max(t_copy, t_agg) / t_total: the copies alone through
+            # the same ring on the copy stream (argus_ingest), the aggregation alone from the resident
+            # leg, and the overlapped host-streamed aggregation
+            cs = torch.cuda.Stream()
+            with torch.cuda.stream(cs):
+                c0, c1 = mk(), mk()
+                c0.record()
+                for c, lo in enumerate(range(0, n, chunk)):
+                    cnt = min(chunk, n - lo)
+                    ctx.ingest(h_ev.data_ptr() + lo * 32, cnt, d_ring.data_ptr() + (c % RING_SLOTS) * chunk * 32, cs)
+                c1.record()
+            torch.cuda.synchronize()
+            t_copy = c0.elapsed_time(c1)
+            g0, g1 = mk(), mk()
+            ctx.reset(rec)
+            g0.record()
+            ctx.aggregate_host(h_ev, n, chunk, d_ring, RING_SLOTS, rec)
+            g1.record()
+            torch.cuda.synchronize()
+            t_total = g0.elapsed_time(g1)
             e2e = {"value": total_events / (e_ms * 1e-3), "unit": "events/s", "ms_per_step": e_ms,
                    "steps": e2e_steps, "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": d2h,
                    "h2d_gbs": 32 * n / (e_ms * 1e-3) / 1e9, "chunk_bytes": chunk * 32,
-                   "ring_slots": RING_SLOTS}
+                   "ring_slots": RING_SLOTS, "verified": verified,
+                   "overlap": {"t_copy_ms": t_copy, "t_agg_ms": agg_ms, "t_total_ms": t_total,
+                               "efficiency": max(t_copy, agg_ms) / t_total}}
         except Exception as e:  # e.g. the box cannot pin the whole buffer
             e2e = {"value": None, "unit": "events/s", "error": repr(e)[:200],
                    "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": None}
@@ -253,33 +317,65 @@ def run_ours(args, world):
     step_bytes = alg_bytes + diag_bytes
     out = {
         "metric": METRIC, "value": value, "unit": "events/s", "n_gpus": world.size, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "warmup": args.warmup, "ms_per_step": ms_step, "ms_per_step_median": float(np.median(step_list)),
+        "ms_per_step_best": float(np.min(step_list)), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int64", "data": "synthetic",
         "config": {"workload": s.name, "n_ranks": s.n_ranks, "n_steps": s.n_steps,
                    "events_per_rank_step": s.n_events, "n_sigs": s.n_sigs, "n_phases": s.n_phases,
                    "events": n, "raw_bytes": 32 * n, "table_bytes": ctx.table_bytes,
+                   "workspace_bytes": ctx.workspace_bytes,
                    "l2": "inputs (raw events) are larger than L2; no flush needed",
                    "jobs": "one independent job of this size per GPU"},
         "raw_event_gbs": 32 * value / 1e9,
         "hbm_frac_step": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
         "hbm_frac_step_vs_8tbs": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0,
         "roofline": {"bound": "hbm", "kernel": "aggregate_seg_kernel" if not s.shuffle else
-                     "argus_aggregate = partition_count/offsets/scan/scatter + aggregate_seg_kernel",
+                     "argus_aggregate = grouping pass + aggregate_seg_kernel",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "peak_source": peak_src, "kernel_ms": agg_ms,
+                     "kernel_ms_median": float(np.median(agg_list)), "kernel_ms_best": float(np.min(agg_list)),
                      "algorithmic_bytes": alg_bytes, "share_of_step": agg_ms / ms_step},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": (8 if s.shuffle else 4) * args.steps,
+        "clocks": clocks, "e2e": e2e,
+        "gpu_launches": k1 - k0, "gpu_memsets": m1 - m0,     # counted by the library (argus_launch_count)
         "counters": {"n_valid": n_valid, "n_invalid": n_invalid},
     }
     if world.size == 1 and not args.no_cpu_baseline:
-        sample_ranks = max(1, min(s.n_ranks, (160_000_000 // (s.n_steps * s.n_events)) or 1))
-        n_ev, dt = oracle_sample(wl, sample_ranks, os.cpu_count() or 1)
+        k = args.cpu_baseline_ranks if args.cpu_baseline_ranks > 0 else s.n_ranks
+        if args.cpu_baseline_ranks < 0:      # default: a bounded sample, about 15 s of oracle time
+            k = max(1, min(s.n_ranks, (670_000_000 // (s.n_steps * s.n_events)) or 1))
+        if s.shuffle:
+            k = s.n_ranks
+        n_ev, dt, o = oracle_sample(wl, k, os.cpu_count() or 1)
         out["cpu_baseline"] = {"value": n_ev / dt, "unit": "events/s", "cores": 1, "kind": "oracle",
-                               "sample": f"first {sample_ranks} of {s.n_ranks} ranks ({n_ev} events) of "
+                               "sample": f"first {k} of {s.n_ranks} ranks ({n_ev} events) of "
                                          f"'{s.name}', aggregate + phase_times + diagnose, {dt:.1f} s; "
                                          f"host has {os.cpu_count()} cores (generator used them, oracle 1)"}
+        # bit-exact check of this very run: the table rows of the sampled ranks (every byte of their
+        # records; the e2e leg above left the same table, see e2e.verified) against the oracle's
+        want = o.records()
+        rb = ctx.record_bytes
+        got = rec[: want.shape[0] * rb].cpu().numpy().reshape(want.shape)
+        out["parity_check"] = {"ranks": int(k), "records_equal_oracle": bool(np.array_equal(got, want)),
+                               "counters_equal_oracle": (n_valid, n_invalid) == (o.n_valid, o.n_invalid)
+                               if k == s.n_ranks else None}
     print(json.dumps(out))
     ctx.close()
+
+
+def relaunch_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` outside torchrun: spawn N ranks (one per GPU) or fail loudly."""
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        print(f"bench.py: --gpus {args.gpus} but this box has {have} CUDA device(s)", file=sys.stderr)
+        return 2
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -290,10 +386,13 @@ def main():
     ap.add_argument("--workload", default="production",
                     help="tiny | mid | scale | unsorted | production (BASELINE.json configs[0..4])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--variant", type=int, default=0, help="segmented-kernel geometry (tuning)")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = one job of the named size per GPU; strong = ONE job sharded by trace rank")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-baseline-ranks", type=int, default=-1,
+                    help="ranks of the workload the oracle is timed on: -1 = bounded sample (default), 0 = all")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
@@ -303,6 +402,8 @@ def main():
         if rank == 0:
             run_reference(args, D.World())
         return
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(relaunch_under_torchrun(args))
     world = D.init_world(args.gpus)
     try:
         run_ours(args, world)

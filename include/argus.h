@@ -34,8 +34,8 @@ extern "C" {
 /* ---- config flags ------------------------------------------------------------------------- */
 /* Performance hint (R18): records arrive grouped by (rank, step) — the segmented kernel reads them
  * in place.  Without the hint argus_aggregate first groups the n events of the call by (rank, step)
- * into a ctx-owned device workspace of n*32 bytes (allocated on first use, grown on demand; if it
- * cannot be allocated the slower global-table kernel is used instead).
+ * into the grouping area of the workspace (argus_config.max_ungrouped_events * 32 bytes); a call
+ * with more events than that area holds takes the slower global-table kernel instead.
  * Results never depend on the hint; a violated hint only costs time. */
 #define ARGUS_FLAG_SORTED 0x1u
 
@@ -113,13 +113,16 @@ typedef struct argus_record_header {
 
 typedef struct argus_config {
   uint32_t n_ranks;    /* R, 1..ARGUS_MAX_RANKS */
-  uint32_t n_steps;    /* T >= 1; a record is addressed by step - step_base in [0, T) (R19) */
+  uint32_t n_steps;    /* T >= 1; a record is addressed by step - step_base in [0, T) (R19);
+                          step_base + T <= 2^32 (ARGUS_ESIZE otherwise: step numbers do not wrap) */
   uint32_t n_sigs;     /* S >= 1 */
   uint32_t n_phases;   /* P, 1..ARGUS_MAX_PHASES */
   uint32_t step_base;
   uint32_t flags;      /* ARGUS_FLAG_* */
   int32_t  device;     /* CUDA device ordinal */
-  uint32_t reserved;   /* 0 */
+  uint32_t max_ungrouped_events; /* largest n of one argus_aggregate call on input WITHOUT the SORTED hint that
+                          is still grouped first (sizes the grouping area of the workspace: 32 B per event);
+                          0 = no grouping area, ungrouped input goes through the global-table kernel */
 } argus_config;
 
 /* Per-series result of the cross-rank rule (NS: "per (step, sig), the exact median and MAD over
@@ -145,9 +148,23 @@ typedef struct argus_diag_out {
 
 typedef struct argus_ctx argus_ctx;  /* opaque */
 
-/* Create a context for one table geometry.  Allocates only small device workspace (two u32 per
- * record slot, counters); see ARGUS_FLAG_SORTED for the grouping workspace.  [host] cfg, [host] out. */
-int argus_create(const argus_config* cfg, argus_ctx** out);
+/* Device workspace of a context, in bytes ("the caller owns every large buffer").  It holds,
+ * in this order, each area 256-byte aligned: the per-record state words (4 B per (rank, step)), the event
+ * counters, the group sizes of the grouping pass (4 B per (rank, step)), the SUM PLANE (8 B per cell: the
+ * u64 sum of every (rank, step, sig), sig-contiguous, kept in step with the table so that the cross-rank
+ * gather of argus_diagnose reads whole sectors: 134 MB at R = S = 4096), the per-CTA overflow lists of the
+ * segmented kernel (64 KB x 1024), one mark byte per diagnosed series, and — only when
+ * cfg->max_ungrouped_events > 0 — the per-CTA key histograms of the grouping pass and the grouping area
+ * itself (32 B per event).  Queries the device of cfg for its SM count.  0 if cfg is invalid. */
+size_t argus_workspace_bytes(const argus_config* cfg);
+
+/* Create a context for one table geometry.  [device] d_workspace: argus_workspace_bytes(cfg) bytes,
+ * 256-byte aligned, owned by the caller, borrowed until argus_destroy (ARGUS_EINVAL when misaligned or
+ * workspace_bytes is too small).  d_workspace == NULL: the library makes that one allocation itself, here
+ * (ARGUS_ENOMEM when it fails), and frees it in argus_destroy.  No other entry point allocates or frees
+ * device memory or synchronises the device.  Host-side the ctx owns an internal copy stream and a few CUDA
+ * events.  [host] cfg, [host] out. */
+int argus_create(const argus_config* cfg, void* d_workspace, size_t workspace_bytes, argus_ctx** out);
 int argus_destroy(argus_ctx* ctx);
 
 /* Bytes of one record = 64 + 32*(P+1) + 160*S, and of the whole [R][T] table.  0 if cfg is NULL. */
@@ -161,8 +178,10 @@ size_t argus_table_bytes(const argus_config* cfg);
 int argus_reset(argus_ctx* ctx, void* d_records, void* stream);
 
 /* NS (2) ingest: asynchronous copy of n events from [host] pinned memory h_src to [device] d_dst
- * on `copy_stream`, followed by an internal CUDA event that the next argus_aggregate on this ctx
- * waits for (so copy and compute overlap across chunks).  n may be 0. */
+ * on `copy_stream`, followed by an internal CUDA event that the next argus_aggregate (or
+ * argus_aggregate_host) on this ctx waits for, so copy and compute overlap across chunks.  Re-using d_dst
+ * while an earlier argus_aggregate may still read it is the caller's business (order copy_stream after
+ * the compute stream with an event of your own: see tests/test_ingest_gpu.py).  n may be 0. */
 int argus_ingest(argus_ctx* ctx, const argus_event* h_src, uint64_t n, argus_event* d_dst,
                  void* copy_stream);
 
@@ -175,9 +194,11 @@ int argus_aggregate(argus_ctx* ctx, const argus_event* d_events, uint64_t n, voi
                     void* stream);
 
 /* NS (2)+(3) streamed aggregate: copy n events from [host] pinned h_events in chunks of
- * chunk_events through a [device] ring of ring_slots slots (each chunk_events*32 bytes) on an
- * internal copy stream, overlapped with aggregation of earlier chunks on `stream`.
- * Equivalent to argus_ingest + argus_aggregate per chunk with ring-slot reuse ordered by events. */
+ * chunk_events through a [device] ring of ring_slots slots (each chunk_events*32 bytes; 1..64 slots) on
+ * an internal copy stream, overlapped with aggregation of earlier chunks on `stream`.
+ * Equivalent to argus_ingest + argus_aggregate per chunk with ring-slot reuse ordered by events: the
+ * copy into a slot waits for the aggregation that last read it, the aggregation waits for its copy (the
+ * paper's fixed buffer pool with back-pressure; nothing is dropped). */
 int argus_aggregate_host(argus_ctx* ctx, const argus_event* h_events, uint64_t n,
                          uint64_t chunk_events, argus_event* d_ring, uint32_t ring_slots,
                          void* d_records, void* stream);
@@ -185,23 +206,30 @@ int argus_aggregate_host(argus_ctx* ctx, const argus_event* h_events, uint64_t n
 /* Finalise (never re-reads events): materialise untouched records, set every span_ns, derive the
  * whole-iteration span (index P) from the phase spans, write the record headers (NS (5), R17).
  * If [device] d_spans_out is non-NULL also writes a compact copy argus_span[R][T][P+1].
- * Idempotent; may be followed by more argus_aggregate calls and another argus_phase_times. */
+ * Idempotent; may be followed by more argus_aggregate calls and another argus_phase_times (required
+ * again before argus_diagnose: ARGUS_ESTATE otherwise). */
 int argus_phase_times(argus_ctx* ctx, void* d_records, argus_span* d_spans_out, void* stream);
 
-/* NS (4) cross-rank diagnosis on a finalised table (call argus_phase_times first).  For every
+/* NS (4) cross-rank diagnosis on a finalised table (argus_phase_times must have run since the last
+ * argus_aggregate into it, else ARGUS_ESTATE; a table this ctx did not aggregate is read as is).  For every
  * step t and every series family (sigs, phases, whole iteration): exact median and MAD over the
  * R ranks, flag[r] = |x[r]-med| > sat3(MAD) ? (x[r] > med ? HIGH : LOW) : NONE  (R10-R14),
  * plus the roll-ups of R15.  [host] outs holds [device] pointers. */
 int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* outs, void* stream);
 
-/* Synchronises all streams the ctx has used and returns the event counters since argus_reset.
- * Asynchronous kernel faults surface here as ARGUS_ECUDA.  [host] outputs, may be NULL. */
+/* Synchronises the internal copy stream and every stream passed to this ctx since argus_create (the ctx
+ * remembers up to 8 distinct ones; the oldest is synchronised when a ninth appears) and returns the event
+ * counters since argus_reset.  Asynchronous kernel faults surface here as ARGUS_ECUDA.  [host] outputs,
+ * may be NULL. */
 int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid);
 
-/* Tuning knobs for measurement (not needed for correctness): which = ARGUS_TUNE_*.  */
-#define ARGUS_TUNE_GRID_CTAS   1  /* persistent CTAs of the segmented kernel (0 = #SMs)  */
+/* Kernels and memsets this ctx has launched since argus_create (what bench.py reports as gpu_launches).
+ * [host] outputs, may be NULL. */
+int argus_launch_count(const argus_ctx* ctx, uint64_t* kernels, uint64_t* memsets);
+
+/* Knobs for tests and measurement (not needed for correctness): which = ARGUS_TUNE_*.  */
+#define ARGUS_TUNE_GRID_CTAS   1  /* persistent CTAs of the segmented kernel (0 = by geometry; <= 1024) */
 #define ARGUS_TUNE_FORCE_PATH  2  /* 0 = by flags, 1 = segmented, 2 = global-table, 3 = group then segmented */
-#define ARGUS_TUNE_SEG_VARIANT 3  /* thread/unroll geometry of the segmented kernel (0 = default) */
 int argus_tune(argus_ctx* ctx, int which, int64_t value);
 
 const char* argus_strerror(int code);

@@ -15,7 +15,9 @@
  * (SURVEY.md §8(c)), a pure-Python dict brute force, bucket() against int.bit_length at every
  * power of two +-1, closed forms of median/MAD (constant series, one outlier, arithmetic
  * progression, translation invariance, odd-R scaling), permutation and chunk-split invariance,
- * histogram/count/min/max/span invariants, recovery of the injected faults.
+ * histogram/count/min/max/span invariants, recovery of the injected faults; every byte of the record
+ * header (R17) by the hand-worked H lines of tests/golden/handworked.txt and a Python-int brute force
+ * over the raw events (first start / last end per rank-step, zero reserved words).
  */
 #include <stdint.h>
 #include <stdlib.h>

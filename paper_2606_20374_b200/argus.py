@@ -14,7 +14,7 @@ from ._build import build_argus
 
 OK, EINVAL, ECUDA, ESIZE, ESTATE, ENOMEM = 0, -1, -2, -3, -4, -5
 FLAG_SORTED = 0x1
-TUNE_GRID_CTAS, TUNE_FORCE_PATH, TUNE_SEG_VARIANT = 1, 2, 3
+TUNE_GRID_CTAS, TUNE_FORCE_PATH = 1, 2
 PATH_AUTO, PATH_SEGMENTED, PATH_GLOBAL, PATH_GROUPED = 0, 1, 2, 3
 
 EVENT_DTYPE = np.dtype(
@@ -30,9 +30,10 @@ HEADER_DTYPE = np.dtype([("magic", "<u4"), ("version", "<u2"), ("n_phases", "<u2
                          ("n_events", "<u8"), ("min_start", "<i8"), ("max_end", "<i8"),
                          ("iter_ns", "<u8"), ("reserved1", "<u8")])
 
-EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes", "argus_reset",
-           "argus_ingest", "argus_aggregate", "argus_aggregate_host", "argus_phase_times",
-           "argus_diagnose", "argus_stats", "argus_tune", "argus_strerror", "argus_last_cuda_error",
+EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes",
+           "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
+           "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_stats",
+           "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
 
 
@@ -40,7 +41,7 @@ class ArgusConfig(ctypes.Structure):
     _fields_ = [("n_ranks", ctypes.c_uint32), ("n_steps", ctypes.c_uint32),
                 ("n_sigs", ctypes.c_uint32), ("n_phases", ctypes.c_uint32),
                 ("step_base", ctypes.c_uint32), ("flags", ctypes.c_uint32),
-                ("device", ctypes.c_int32), ("reserved", ctypes.c_uint32)]
+                ("device", ctypes.c_int32), ("max_ungrouped_events", ctypes.c_uint32)]
 
 
 class ArgusDiagOut(ctypes.Structure):
@@ -67,7 +68,9 @@ def load() -> ctypes.CDLL:
     vp, u64, i32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int
     cfgp = ctypes.POINTER(ArgusConfig)
     lib.argus_create.restype = i32
-    lib.argus_create.argtypes = [cfgp, ctypes.POINTER(vp)]
+    lib.argus_create.argtypes = [cfgp, vp, ctypes.c_size_t, ctypes.POINTER(vp)]
+    lib.argus_workspace_bytes.restype = ctypes.c_size_t
+    lib.argus_workspace_bytes.argtypes = [cfgp]
     lib.argus_destroy.restype = i32
     lib.argus_destroy.argtypes = [vp]
     lib.argus_record_bytes.restype = ctypes.c_size_t
@@ -88,6 +91,8 @@ def load() -> ctypes.CDLL:
     lib.argus_diagnose.argtypes = [vp, vp, ctypes.POINTER(ArgusDiagOut), vp]
     lib.argus_stats.restype = i32
     lib.argus_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    lib.argus_launch_count.restype = i32
+    lib.argus_launch_count.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_tune.restype = i32
     lib.argus_tune.argtypes = [vp, i32, ctypes.c_int64]
     lib.argus_strerror.restype = ctypes.c_char_p
@@ -126,14 +131,30 @@ class Argus:
     names of the C entry points; all work is queued on CUDA streams."""
 
     def __init__(self, n_ranks: int, n_steps: int, n_sigs: int, n_phases: int, step_base: int = 0,
-                 sorted_hint: bool = True, device: int = 0):
+                 sorted_hint: bool = True, device: int = 0, max_ungrouped_events: int = 0,
+                 workspace="torch"):
+        """workspace: "torch" = a caller-owned torch uint8 tensor of argus_workspace_bytes (kept in
+        self.workspace); None = the library allocates it itself in argus_create; or a tensor."""
         self.lib = load()
         self.cfg = ArgusConfig(n_ranks, n_steps, n_sigs, n_phases, step_base,
-                               FLAG_SORTED if sorted_hint else 0, device, 0)
+                               FLAG_SORTED if sorted_hint else 0, device, max_ungrouped_events)
         self.R, self.T, self.S, self.P = n_ranks, n_steps, n_sigs, n_phases
         self.device = device
+        self.workspace = None
+        self._h = None
+        if isinstance(workspace, str):
+            if workspace != "torch":
+                raise ValueError(workspace)
+            import torch
+            nbytes = self.workspace_bytes
+            if nbytes:          # 0: invalid config or no device; argus_create reports which
+                workspace = torch.empty(nbytes, dtype=torch.uint8, device=f"cuda:{device}")
+            else:
+                workspace = None
+        self.workspace = workspace
         h = ctypes.c_void_p()
-        rc = self.lib.argus_create(ctypes.byref(self.cfg), ctypes.byref(h))
+        rc = self.lib.argus_create(ctypes.byref(self.cfg), _ptr(workspace),
+                                   0 if workspace is None else workspace.numel(), ctypes.byref(h))
         self._h = h if rc == OK else None
         self._check(rc)
 
@@ -163,6 +184,10 @@ class Argus:
     @property
     def table_bytes(self) -> int:
         return int(self.lib.argus_table_bytes(ctypes.byref(self.cfg)))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(self.lib.argus_workspace_bytes(ctypes.byref(self.cfg)))
 
     def alloc_records(self):
         import torch
@@ -210,6 +235,11 @@ class Argus:
     def stats(self):
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         self._check(self.lib.argus_stats(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return int(a.value), int(b.value)
+
+    def launch_count(self):
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self.lib.argus_launch_count(self._h, ctypes.byref(a), ctypes.byref(b)))
         return int(a.value), int(b.value)
 
     def tune(self, which: int, value: int) -> None:

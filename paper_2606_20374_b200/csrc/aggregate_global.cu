@@ -76,6 +76,7 @@ cudaError_t argus_launch_materialise_all(argus_ctx* ctx, void* d_records, cudaSt
   const uint32_t n_rec = ctx->dims.R * ctx->dims.T;
   uint32_t grid = n_rec < (uint32_t)ctx->sm_count * 8u ? n_rec : (uint32_t)ctx->sm_count * 8u;
   materialise_kernel<<<grid, 256, 0, s>>>(static_cast<uint8_t*>(d_records), ctx->d_state, ctx->dims, n_rec);
+  ctx->n_kernels += 1;
   return cudaGetLastError();
 }
 
@@ -90,5 +91,6 @@ cudaError_t argus_launch_aggregate_global(argus_ctx* ctx, const argus_event* ev,
   aggregate_global_kernel<<<(unsigned)blocks, 256, 0, s>>>(reinterpret_cast<const uint4*>(ev), n,
                                                            static_cast<uint8_t*>(d_records),
                                                            ctx->d_counters, ctx->dims);
+  ctx->n_kernels += 1;
   return cudaGetLastError();
 }

@@ -3,10 +3,11 @@
 // shared-memory-privatised per-block histograms and min/max/sum ... warp-shuffle segmented
 // reductions where a block spans rank-step boundaries, and flush to global in one pass").
 //
-// One persistent CTA per SM walks a contiguous span of the event buffer.  Events arrive through a
-// ring of shared-memory stages filled by 1-D TMA bulk copies (cp.async.bulk + mbarrier
+// Persistent CTAs (one, two or three per SM by table size) each walk a contiguous span of the event
+// buffer.  Events arrive through a ring of shared-memory stages filled by 2-D tiled TMA loads
+// (cp.async.bulk.tensor.2d over whole 128-byte rows of four events, 128-byte swizzle, mbarrier
 // complete_tx, L2 evict-first) issued by a producer warp; each consumer lane takes one event per
-// iteration into registers and releases the stage at once.
+// iteration into registers with two conflict-free LDS.128.
 // The CTA keeps ONE (rank, step) table in shared memory at a time, 32 bytes per sig, laid out as
 // structure-of-arrays so that random sigs spread over all 32 banks:
 //   slots[S]  uint4: four histogram counters, DIRECT-MAPPED by bucket & 3
@@ -19,33 +20,20 @@
 // extension when the invariant would break.  Only native 32-bit shared atomics are used on the
 // hot path (64-bit shared atomic adds are CAS loops on sm_100a).
 // An event the compact cell cannot take (duration >= 2^32 ns, or a range wider than four buckets)
-// goes straight to the global record with L2 atomics.  When the (rank, step) key changes the
-// table is flushed: the first CTA to reach a record claims it and writes the whole 160-byte cells
-// with coalesced 128-bit stores (no read-modify-write, no separate identity fill); any later
-// contribution to the same record merges with L2 reductions.  Correct for ANY event order; fast
-// when events are grouped by (rank, step) (R18).
+// is parked in the CTA's overflow list (global memory, workspace) and applied to the record with L2
+// reductions at the flush; when the record is already live it goes there at once.  When the
+// (rank, step) key changes the table is flushed: the first CTA to reach a record claims it and
+// writes the whole 160-byte cells with coalesced 128-bit stores (no read-modify-write, no separate
+// identity fill); any later contribution to the same record merges with L2 reductions.  Correct
+// for ANY event order; fast when events are grouped by (rank, step) (R18).
 #include <cuda.h>
 #include <stddef.h>
-#include <stdio.h>
 
 #include <type_traits>
 
 #include "argus_internal.cuh"
 
 namespace {
-
-// Optional cycle accounting (build with -DARGUS_SEG_PROF; prints from a few CTAs): where consumer
-// warp 0 spends its time — waiting for data, in rendezvous (park), of which flushing.
-#ifdef ARGUS_SEG_PROF
-#define PROF_DECL long long prof_wait = 0, prof_park = 0, prof_t0 = clock64()
-#define PROF_BEGIN(v) const long long v = clock64()
-#define PROF_END(acc, v) acc += clock64() - v
-__device__ long long g_prof_flush[148];
-#else
-#define PROF_DECL
-#define PROF_BEGIN(v)
-#define PROF_END(acc, v)
-#endif
 
 constexpr int MAXK = 48;             // ring stages (bounded by shared memory at launch)
 constexpr uint32_t KEY_NONE = 0xFFFFFFFFu;
@@ -68,7 +56,7 @@ struct Hdr {
   uint32_t n_finished;                // consumer warps that ran out of events
   uint32_t ovf_n;                     // events parked in this CTA's overflow list since the last flush
 };
-constexpr uint32_t OVF_CAP = 4096;    // entries of a CTA's overflow list (16 bytes each, global memory)
+constexpr uint32_t OVF_CAP = ARGUS_OVF_CAP;   // entries of a CTA's overflow list (16 bytes each, workspace)
 constexpr unsigned long long NEXT_NONE = ~0ull;
 static_assert(sizeof(Hdr) <= HDR_BYTES, "header");
 
@@ -285,9 +273,6 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
   const Table tb{SCAP};
   Hdr* H = hdr();
   SpanAcc* spans = span_tab();
-#ifdef ARGUS_SEG_PROF
-  const long long tf0 = clock64();
-#endif
   uint32_t mode = *reinterpret_cast<volatile uint32_t*>(&H->mode);
   uint32_t n_ovf = *reinterpret_cast<volatile uint32_t*>(&H->ovf_n);
   n_ovf = n_ovf < OVF_CAP ? n_ovf : OVF_CAP;
@@ -408,9 +393,6 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
   for (uint32_t k = tid; k < D.P; k += NC) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
   }
-#ifdef ARGUS_SEG_PROF
-  if (tid == 0) g_prof_flush[blockIdx.x] += clock64() - tf0;
-#endif
 }
 
 // Rendezvous of all consumer warps (the only CTA-wide synchronisation of the steady state, taken
@@ -549,7 +531,6 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   constexpr uint32_t EMPTY_OFF = MAXK * 8u;          // empty[k] sits MAXK*8 bytes after full[k]
   WarpSpan ws;
   ws.reset();
-  PROF_DECL;
   uint32_t cur_key = KEY_NONE, live = 0u;
   uint32_t cur_rank = 0u, cur_step = 0u, s_eff = 0u;   // s_eff = 0 while no key is current: nothing is accepted
   uint32_t n_invalid = 0;
@@ -617,35 +598,18 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     // stage unreleased, which may stall the in-order producer, so nobody may wait for data while
     // others wait for him).  Warps before that position go on: their stages are always issued.
     if (have && !mbar_try_wait(a_bar, par)) {
-      PROF_BEGIN(tw);
       do {
         if (lds32(a_nextidx) < my_pos) {
           ws.flush(lane);
-          PROF_BEGIN(tp);
           const unsigned long long r = park<NC, SCAP>(gl, false, KEY_NONE, KEY_NONE, cur_key, live);
-          PROF_END(prof_park, tp);
           ARGUS_ADOPT(r);
         }
       } while (!mbar_try_wait(a_bar, par));
-      PROF_END(prof_wait, tw);
     }
     uint4 lo, hi;
     if (have) {
       lo = lds128(a_ev);
       hi = lds128(a_ev ^ 16u);
-#ifdef ARGUS_SEG_CHECK
-      {   // debug: the staged record must equal the record in global memory
-        const uint64_t gc = e0 + my_pos + (uint32_t)lane;
-        if (gc < (n & ~3ull) && gc < e1) {
-          const uint4 gl0 = ev[2 * gc], gl1 = ev[2 * gc + 1];
-          const bool bad_lo = gl0.x != lo.x || gl0.y != lo.y || gl0.z != lo.z || gl0.w != lo.w;
-          const bool bad_hi = gl1.x != hi.x || gl1.y != hi.y || gl1.z != hi.z || gl1.w != hi.w;
-          if (bad_lo || bad_hi)
-            printf("stage mismatch cta %d warp %d lane %d ev %llu lo %d hi %d (smem %08x %08x | glob %08x %08x)\n",
-                   blockIdx.x, warp, lane, (unsigned long long)gc, (int)bad_lo, (int)bad_hi, hi.x, hi.z, gl1.x, gl1.z);
-        }
-      }
-#endif
       if (TAIL) {
         // the last n % 4 events of the buffer are not part of the tensor (whole 128-byte rows only)
         const uint64_t g = e0 + my_pos + (uint32_t)lane;
@@ -659,14 +623,6 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     if (a_bar >= a_bar_end) { a_bar -= bar_ring; par ^= 1u; a_ev -= ring_bytes; }
     if (TAIL) s += SPI;
     my_pos += NC;
-#ifdef ARGUS_SEG_NOCOMPUTE
-    {
-      const bool odd = ((lo.x ^ hi.x) == 0x12345u);   // experiment: stream only (results are wrong)
-      n_invalid += __all_sync(FULL, odd) ? 1u : 0u;
-      if (have && lane == 0) mbar_arrive(a_rel);
-    }
-    return;
-#endif
 
     // ---- decode.  Fast test first: the event belongs to the current key and fits a compact cell
     // (same rank and step words as the current key, sig and phase in range, both timestamps
@@ -746,9 +702,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       if (ok) { pending = false; fast = false; }
       if (!__any_sync(FULL, pending)) break;
       ws.flush(lane);
-      PROF_BEGIN(tp2);
       const unsigned long long r = park<NC, SCAP>(gl, pending, key, idx, cur_key, live);
-      PROF_END(prof_park, tp2);
       ARGUS_ADOPT(r);
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
@@ -766,44 +720,39 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     cur_key = (uint32_t)r; live = (uint32_t)(r >> 32) & 1u;
   }
 #undef ARGUS_ADOPT
-#ifdef ARGUS_SEG_PROF
-  if ((warp == 0 || warp == CW - 1) && lane == 0 && (blockIdx.x % 37) == 0)
-    printf("cta %3d warp %2d: total %lld  wait-data %lld  park %lld (flush %lld)  iters %u\n", blockIdx.x, warp,
-           clock64() - prof_t0, prof_wait, prof_park, g_prof_flush[blockIdx.x], n_iter);
-#endif
 
   n_invalid = __reduce_add_sync(FULL, n_invalid);
   if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
   if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
 }
 
+// shared-memory bytes of one geometry
+template <int CW, int WPSTG, uint32_t SCAP, int MINB>
+constexpr size_t geom_smem() {
+  return ((TAB_OFF + 32u * SCAP + 127u) & ~127u) +
+         (size_t)ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG, MINB) * ((size_t)WPSTG * 1024u);
+}
+
+template <int CW, int WPSTG, uint32_t SCAP, int MINB>
+cudaError_t configure_cap() {
+  static_assert(geom_smem<CW, WPSTG, SCAP, MINB>() <= smem_budget(MINB), "shared memory");
+  return cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB>,
+                              cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)geom_smem<CW, WPSTG, SCAP, MINB>());
+}
+
 template <int CW, int WPSTG, uint32_t SCAP, int MINB>
 cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records, cudaStream_t s) {
-  constexpr size_t STAGE_BYTES = (size_t)WPSTG * 32 * 32;
-  constexpr int K = ring_depth(SCAP, (uint32_t)STAGE_BYTES, CW / WPSTG, MINB);
-  constexpr size_t smem_bytes = ((TAB_OFF + 32u * SCAP + 127u) & ~127u) + (size_t)K * STAGE_BYTES;
-  static_assert(smem_bytes <= smem_budget(MINB), "shared memory");
-  if ((size_t)ctx->max_smem_optin < smem_bytes) return cudaErrorInvalidConfiguration;
-  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB>,
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
-  if (e != cudaSuccess) return e;
+  constexpr size_t smem_bytes = geom_smem<CW, WPSTG, SCAP, MINB>();
   int grid = ctx->tune_grid > 0 ? ctx->tune_grid : ctx->sm_count * MINB;
+  if (grid > (int)ARGUS_MAX_SEG_CTAS) grid = (int)ARGUS_MAX_SEG_CTAS;
   // the u32 histogram counters of a CTA must not wrap between flushes: bound the span of one CTA
   const uint64_t tile = (uint64_t)CW * 32;
   const uint64_t cap = (1ull << 26) - tile;
   uint64_t per_cta = (n + grid - 1) / grid;
   if (per_cta > cap) per_cta = cap;
   per_cta = (per_cta + tile - 1) / tile * tile;
-  const uint64_t ctas = (n + per_cta - 1) / per_cta;
-  if (ctx->ovf_ctas < ctas) {          // overflow lists, one per CTA (grow-only; 64 KB each)
-    e = cudaDeviceSynchronize();
-    if (e != cudaSuccess) return e;
-    if (ctx->d_ovf) cudaFree(ctx->d_ovf);
-    ctx->d_ovf = nullptr; ctx->ovf_ctas = 0;
-    e = cudaMalloc(&ctx->d_ovf, ctas * OVF_CAP * sizeof(uint4));
-    if (e != cudaSuccess) return e;
-    ctx->ovf_ctas = ctas;
-  }
+  const uint64_t ctas = (n + per_cta - 1) / per_cta;     // <= max(grid, 2^32 / 2^26 + 1) <= ARGUS_MAX_SEG_CTAS
   // the events as a 2-D tensor of whole 128-byte rows (4 events), loaded a stage (WPSTG * 8 rows) at a
   // time with the 128-byte shared-memory swizzle; the last n % 4 events are read by the consumers
   CUtensorMap tmap;
@@ -828,42 +777,35 @@ cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* 
   }
   aggregate_seg_kernel<CW, WPSTG, SCAP, MINB><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       tmap, reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
-      ctx->d_counters, static_cast<uint4*>(ctx->d_ovf), ctx->dims);
+      ctx->d_counters, ctx->d_ovf, ctx->dims);
+  ctx->n_kernels += 1;
   return cudaGetLastError();
-}
-
-// The table layout is compiled for a few capacities; S picks the smallest that holds it.
-template <int CW, int WPSTG>
-cudaError_t launch_variant(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records,
-                           cudaStream_t s) {
-  const uint32_t S = ctx->dims.S;
-  if (S <= 1024u) return launch_cap<CW, WPSTG, 1024u, 1>(ctx, ev, n, d_records, s);
-  if (S <= 2048u) return launch_cap<CW, WPSTG, 2048u, 1>(ctx, ev, n, d_records, s);
-  if (S <= 4096u) return launch_cap<CW, WPSTG, 4096u, 1>(ctx, ev, n, d_records, s);
-  if (S <= ARGUS_SEG_MAX_SIGS) return launch_cap<CW, WPSTG, ARGUS_SEG_MAX_SIGS, 1>(ctx, ev, n, d_records, s);
-  return cudaErrorInvalidConfiguration;
-}
-
-// Default geometry: as many CTAs per SM as the table leaves room for.
-cudaError_t launch_default(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* d_records, cudaStream_t s) {
-  const uint32_t S = ctx->dims.S;
-  if (S <= 1024u) return launch_cap<9, 3, 1024u, 3>(ctx, ev, n, d_records, s);
-  if (S <= 2048u) return launch_cap<15, 5, 2048u, 2>(ctx, ev, n, d_records, s);
-  return launch_variant<30, 10>(ctx, ev, n, d_records, s);
 }
 
 }  // namespace
 
+// Geometry by table size: as many CTAs per SM as the table leaves room for (three 9-warp CTAs for
+// S <= 1024, two 15-warp CTAs for S <= 2048, else one 30-warp CTA), compiled per table capacity.
 bool argus_seg_supported(const argus_ctx* ctx) {
   return ctx->dims.S <= ARGUS_SEG_MAX_SIGS && (size_t)ctx->max_smem_optin >= SMEM_MAX && ctx->fn_tmap_encode != nullptr;
+}
+
+cudaError_t argus_configure_seg(argus_ctx* ctx) {
+  if (!argus_seg_supported(ctx)) return cudaSuccess;
+  const uint32_t S = ctx->dims.S;
+  if (S <= 1024u) return configure_cap<9, 3, 1024u, 3>();
+  if (S <= 2048u) return configure_cap<15, 5, 2048u, 2>();
+  if (S <= 4096u) return configure_cap<30, 10, 4096u, 1>();
+  return configure_cap<30, 10, ARGUS_SEG_MAX_SIGS, 1>();
 }
 
 cudaError_t argus_launch_aggregate_seg(argus_ctx* ctx, const argus_event* ev, uint64_t n,
                                        void* d_records, cudaStream_t s) {
   if (n == 0) return cudaSuccess;
-  switch (ctx->tune_variant) {
-    case 1: return launch_variant<30, 10>(ctx, ev, n, d_records, s);   // one CTA per SM whatever S
-    case 2: return launch_variant<30, 6>(ctx, ev, n, d_records, s);
-    default: return launch_default(ctx, ev, n, d_records, s);
-  }
+  const uint32_t S = ctx->dims.S;
+  if (S <= 1024u) return launch_cap<9, 3, 1024u, 3>(ctx, ev, n, d_records, s);
+  if (S <= 2048u) return launch_cap<15, 5, 2048u, 2>(ctx, ev, n, d_records, s);
+  if (S <= 4096u) return launch_cap<30, 10, 4096u, 1>(ctx, ev, n, d_records, s);
+  if (S <= ARGUS_SEG_MAX_SIGS) return launch_cap<30, 10, ARGUS_SEG_MAX_SIGS, 1>(ctx, ev, n, d_records, s);
+  return cudaErrorInvalidConfiguration;
 }

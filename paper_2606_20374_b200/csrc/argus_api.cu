@@ -1,4 +1,6 @@
-// argus_api.cu — the C ABI of include/argus.h: argument checks, stream/event plumbing, launches.
+// argus_api.cu — the C ABI of include/argus.h: argument checks, workspace carving, stream/event
+// plumbing, launches.  Device memory is allocated in argus_create only (and only when the caller
+// passes no workspace); nothing here synchronises the device.
 #include <new>
 #include <string.h>
 
@@ -21,6 +23,15 @@ static bool cfg_ok(const argus_config* c) {
   return true;
 }
 
+// dims the kernels cannot address (ARGUS_ESIZE); cfg_ok(c) holds
+static bool cfg_too_large(const argus_config* c) {
+  if ((uint64_t)c->n_ranks * c->n_steps >= (1ull << 31)) return true;
+  if (argus_record_bytes(c) >= (1ull << 32)) return true;
+  if ((uint64_t)c->step_base + c->n_steps > (1ull << 32)) return true;   // step numbers do not wrap (R19)
+  if ((uint64_t)c->n_steps * ((uint64_t)c->n_sigs + c->n_phases + 1u) > 0x7FFFFFFFull) return true;   // one CTA per series
+  return false;
+}
+
 extern "C" size_t argus_record_bytes(const argus_config* c) {
   if (!c) return 0;
   return 64u + 32u * ((size_t)c->n_phases + 1u) + 160u * (size_t)c->n_sigs;
@@ -31,12 +42,48 @@ extern "C" size_t argus_table_bytes(const argus_config* c) {
   return argus_record_bytes(c) * (size_t)c->n_ranks * (size_t)c->n_steps;
 }
 
-extern "C" int argus_create(const argus_config* cfg, argus_ctx** out) {
+static size_t up256(size_t v) { return (v + 255u) & ~(size_t)255u; }
+
+void argus_ws_plan(const argus_config* c, int sm_count, int max_smem_optin, argus_ws_layout* L) {
+  const size_t RT = (size_t)c->n_ranks * c->n_steps;
+  size_t o = 0;
+  L->state = o;     o += up256(sizeof(uint32_t) * RT);
+  L->counters = o;  o += up256(2 * sizeof(unsigned long long));
+  L->hist = o;      o += up256(sizeof(uint32_t) * (RT + 1u));
+  L->sums = o;      o += up256(sizeof(unsigned long long) * RT * c->n_sigs);
+  L->ovf = o;       o += up256((size_t)ARGUS_MAX_SEG_CTAS * ARGUS_OVF_CAP * sizeof(uint4));
+  L->diag_todo = o; o += up256((size_t)c->n_steps * ((size_t)c->n_sigs + c->n_phases + 1u));
+  L->part = o; L->group = o; L->part_ctas = 0; L->part_smem = false;
+  if (c->max_ungrouped_events) {
+    argus_partition_plan(c, sm_count, max_smem_optin, &L->part_ctas, &L->part_smem);
+    if (L->part_smem) o += up256(sizeof(uint32_t) * (size_t)L->part_ctas * (RT + 1u));
+    L->group = o;
+    o += up256((size_t)c->max_ungrouped_events * sizeof(argus_event));
+  }
+  L->total = o;
+}
+
+static cudaError_t device_shape(int device, int* sm_count, int* max_smem_optin) {
+  cudaError_t e = cudaDeviceGetAttribute(sm_count, cudaDevAttrMultiProcessorCount, device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+  return e;
+}
+
+extern "C" size_t argus_workspace_bytes(const argus_config* cfg) {
+  if (!cfg_ok(cfg) || cfg_too_large(cfg)) return 0;
+  int sms = 0, smem = 0;
+  if (device_shape(cfg->device, &sms, &smem) != cudaSuccess) { (void)cudaGetLastError(); return 0; }
+  argus_ws_layout L;
+  argus_ws_plan(cfg, sms, smem, &L);
+  return L.total;
+}
+
+extern "C" int argus_create(const argus_config* cfg, void* d_workspace, size_t workspace_bytes, argus_ctx** out) {
   if (!out) return ARGUS_EINVAL;
   *out = nullptr;
   if (!cfg_ok(cfg)) return ARGUS_EINVAL;
-  if ((uint64_t)cfg->n_ranks * cfg->n_steps >= (1ull << 31)) return ARGUS_ESIZE;
-  if (argus_record_bytes(cfg) >= (1ull << 32)) return ARGUS_ESIZE;
+  if (cfg_too_large(cfg)) return ARGUS_ESIZE;
+  if (d_workspace && ((uintptr_t)d_workspace & 255u)) return ARGUS_EINVAL;
   argus_ctx* ctx = new (std::nothrow) argus_ctx();
   if (!ctx) return ARGUS_ENOMEM;
   memset(ctx, 0, sizeof *ctx);
@@ -47,36 +94,49 @@ extern "C" int argus_create(const argus_config* cfg, argus_ctx** out) {
   D.rec_bytes = (uint32_t)argus_record_bytes(cfg);
   D.span_off = 64u;
   D.cell_off = 64u + 32u * (D.P + 1u);
+  int code = ARGUS_OK;
   cudaError_t e = cudaSetDevice(cfg->device);
-  cudaDeviceProp prop;
-  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, cfg->device);
+  if (e == cudaSuccess) e = device_shape(cfg->device, &ctx->sm_count, &ctx->max_smem_optin);
   if (e == cudaSuccess) {
-    ctx->sm_count = prop.multiProcessorCount;
-    ctx->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
-    e = cudaMalloc(&ctx->d_state, sizeof(uint32_t) * (size_t)D.R * D.T);
+    argus_ws_plan(cfg, ctx->sm_count, ctx->max_smem_optin, &ctx->ws);
+    if (d_workspace) {
+      if (workspace_bytes < ctx->ws.total) code = ARGUS_EINVAL;
+      ctx->d_ws = static_cast<uint8_t*>(d_workspace);
+    } else {
+      void* p = nullptr;
+      e = cudaMalloc(&p, ctx->ws.total);     // the library's only device allocation
+      ctx->d_ws = static_cast<uint8_t*>(p);
+      ctx->ws_owned = e == cudaSuccess;
+    }
   }
-  if (e == cudaSuccess) {
+  if (e == cudaSuccess && code == ARGUS_OK) {
+    const argus_ws_layout& L = ctx->ws;
+    ctx->d_state = reinterpret_cast<uint32_t*>(ctx->d_ws + L.state);
+    ctx->d_counters = reinterpret_cast<unsigned long long*>(ctx->d_ws + L.counters);
+    ctx->d_hist = reinterpret_cast<uint32_t*>(ctx->d_ws + L.hist);
+    D.sums = reinterpret_cast<unsigned long long*>(ctx->d_ws + L.sums);
+    ctx->d_ovf = reinterpret_cast<uint4*>(ctx->d_ws + L.ovf);
+    ctx->d_diag_todo = ctx->d_ws + L.diag_todo;
+    if (cfg->max_ungrouped_events) {
+      ctx->d_part = L.part_smem ? reinterpret_cast<uint32_t*>(ctx->d_ws + L.part) : nullptr;
+      ctx->d_group = reinterpret_cast<argus_event*>(ctx->d_ws + L.group);
+    }
     cudaDriverEntryPointQueryResult q;
     void* fn = nullptr;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) == cudaSuccess &&
         q == cudaDriverEntryPointSuccess)
       ctx->fn_tmap_encode = fn;
     (void)cudaGetLastError();
+    e = cudaEventCreateWithFlags(&ctx->ingest_event, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->order_event, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = argus_configure_kernels(ctx);   // opt-in shared-memory sizes, once
   }
-  if (e == cudaSuccess) {
-    // the sum plane (8 bytes per cell, 5 % of the table) is an accelerator of argus_diagnose only:
-    // without it the gather falls back to the records
-    if (cudaMalloc(&D.sums, sizeof(unsigned long long) * (size_t)D.R * D.T * D.S) != cudaSuccess) {
-      D.sums = nullptr;
+  if (e != cudaSuccess || code != ARGUS_OK) {
+    if (e != cudaSuccess) {
+      code = (e == cudaErrorMemoryAllocation) ? ARGUS_ENOMEM : ARGUS_ECUDA;
       (void)cudaGetLastError();
     }
-  }
-  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_counters, 2 * sizeof(unsigned long long));
-  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_hist, sizeof(uint32_t) * ((size_t)D.R * D.T + 1u));
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ingest_event, cudaEventDisableTiming);
-  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
-  if (e != cudaSuccess) {
-    int code = (e == cudaErrorMemoryAllocation) ? ARGUS_ENOMEM : ARGUS_ECUDA;
     argus_destroy(ctx);
     return code;
   }
@@ -87,15 +147,9 @@ extern "C" int argus_create(const argus_config* cfg, argus_ctx** out) {
 extern "C" int argus_destroy(argus_ctx* ctx) {
   if (!ctx) return ARGUS_EINVAL;
   cudaSetDevice(ctx->cfg.device);
-  if (ctx->d_state) cudaFree(ctx->d_state);
-  if (ctx->d_counters) cudaFree(ctx->d_counters);
-  if (ctx->dims.sums) cudaFree(ctx->dims.sums);
-  if (ctx->d_hist) cudaFree(ctx->d_hist);
-  if (ctx->d_group) cudaFree(ctx->d_group);
-  if (ctx->d_ovf) cudaFree(ctx->d_ovf);
-  if (ctx->d_diag_todo) cudaFree(ctx->d_diag_todo);
-  if (ctx->d_part) cudaFree(ctx->d_part);
+  if (ctx->ws_owned && ctx->d_ws) cudaFree(ctx->d_ws);
   if (ctx->ingest_event) cudaEventDestroy(ctx->ingest_event);
+  if (ctx->order_event) cudaEventDestroy(ctx->order_event);
   for (uint32_t i = 0; i < ctx->n_slot_events; ++i) {
     cudaEventDestroy(ctx->slot_free[i]);
     cudaEventDestroy(ctx->slot_full[i]);
@@ -109,15 +163,30 @@ extern "C" int argus_destroy(argus_ctx* ctx) {
 
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
+// argus_stats synchronises every stream the ctx was given; remember the distinct ones
+static int note_stream(argus_ctx* ctx, cudaStream_t s) {
+  for (uint32_t i = 0; i < ctx->n_streams; ++i)
+    if (ctx->streams[i] == s) return ARGUS_OK;
+  if (ctx->n_streams == 8u) {
+    CU(ctx, cudaStreamSynchronize(ctx->streams[0]));
+    memmove(&ctx->streams[0], &ctx->streams[1], 7 * sizeof(cudaStream_t));
+    ctx->n_streams = 7u;
+  }
+  ctx->streams[ctx->n_streams++] = s;
+  return ARGUS_OK;
+}
+
 extern "C" int argus_reset(argus_ctx* ctx, void* d_records, void* stream) {
   if (!ctx || !d_records || !aligned16(d_records)) return ARGUS_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
+  int rc = note_stream(ctx, s);
+  if (rc != ARGUS_OK) return rc;
   CU(ctx, cudaMemsetAsync(ctx->d_state, 0, sizeof(uint32_t) * (size_t)ctx->dims.R * ctx->dims.T, s));
   CU(ctx, cudaMemsetAsync(ctx->d_counters, 0, 2 * sizeof(unsigned long long), s));
+  ctx->n_memsets += 2;
   ctx->d_records = d_records;
   ctx->finalized = false;
-  ctx->last_stream = s;
   return ARGUS_OK;
 }
 
@@ -128,6 +197,8 @@ extern "C" int argus_ingest(argus_ctx* ctx, const argus_event* h_src, uint64_t n
   if (!h_src || !d_dst || !aligned16(d_dst)) return ARGUS_EINVAL;
   cudaStream_t cs = (cudaStream_t)copy_stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
+  int rc = note_stream(ctx, cs);
+  if (rc != ARGUS_OK) return rc;
   CU(ctx, cudaMemcpyAsync(d_dst, h_src, n * sizeof(argus_event), cudaMemcpyHostToDevice, cs));
   CU(ctx, cudaEventRecord(ctx->ingest_event, cs));
   ctx->ingest_pending = true;
@@ -136,23 +207,29 @@ extern "C" int argus_ingest(argus_ctx* ctx, const argus_event* h_src, uint64_t n
 
 // Path choice: grouped input (ARGUS_FLAG_SORTED) -> segmented kernel; ungrouped input -> group the
 // events by (rank, step) first, then the segmented kernel; the global-table kernel is what is left
-// when the table does not fit the segmented kernel or the grouping workspace cannot be allocated.
+// when the table does not fit the segmented kernel or the call exceeds the grouping area.
 static int aggregate_impl(argus_ctx* ctx, const argus_event* d_events, uint64_t n, void* d_records,
                           cudaStream_t s) {
   int path = ctx->tune_path;
   if (path == 0) path = (ctx->cfg.flags & ARGUS_FLAG_SORTED) ? 1 : 3;
   if ((path == 1 || path == 3) && !argus_seg_supported(ctx)) path = 2;
+  if (path == 3 && n > ctx->cfg.max_ungrouped_events) path = 2;
   if (path == 3) {
-    cudaError_t e = argus_launch_partition(ctx, d_events, n, s);
-    if (e == cudaErrorMemoryAllocation) path = 2;
-    else {
-      CU(ctx, e);
-      d_events = ctx->d_group;
-      path = 1;
-    }
+    CU(ctx, argus_launch_partition(ctx, d_events, n, s));
+    d_events = ctx->d_group;
+    path = 1;
   }
   if (path == 1) CU(ctx, argus_launch_aggregate_seg(ctx, d_events, n, d_records, s));
   else CU(ctx, argus_launch_aggregate_global(ctx, d_events, n, d_records, s));
+  return ARGUS_OK;
+}
+
+// the next kernel on `s` must see the bytes of the last argus_ingest
+static int wait_ingest(argus_ctx* ctx, cudaStream_t s) {
+  if (ctx->ingest_pending) {
+    CU(ctx, cudaStreamWaitEvent(s, ctx->ingest_event, 0));
+    ctx->ingest_pending = false;
+  }
   return ARGUS_OK;
 }
 
@@ -164,13 +241,32 @@ extern "C" int argus_aggregate(argus_ctx* ctx, const argus_event* d_events, uint
   if (n != 0 && (!d_events || !aligned16(d_events))) return ARGUS_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
-  if (ctx->ingest_pending) {
-    CU(ctx, cudaStreamWaitEvent(s, ctx->ingest_event, 0));
-    ctx->ingest_pending = false;
-  }
-  ctx->last_stream = s;
-  if (n == 0) return ARGUS_OK;
+  int rc = note_stream(ctx, s);
+  if (rc == ARGUS_OK) rc = wait_ingest(ctx, s);
+  if (rc != ARGUS_OK || n == 0) return rc;
+  ctx->finalized = false;
   return aggregate_impl(ctx, d_events, n, d_records, s);
+}
+
+static int ensure_slot_events(argus_ctx* ctx, uint32_t ring_slots) {
+  if (ctx->n_slot_events >= ring_slots) return ARGUS_OK;
+  cudaEvent_t* f = new (std::nothrow) cudaEvent_t[ring_slots];
+  cudaEvent_t* u = new (std::nothrow) cudaEvent_t[ring_slots];
+  if (!f || !u) { delete[] f; delete[] u; return ARGUS_ENOMEM; }
+  for (uint32_t i = 0; i < ctx->n_slot_events; ++i) { f[i] = ctx->slot_free[i]; u[i] = ctx->slot_full[i]; }
+  uint32_t made = ctx->n_slot_events;
+  for (; made < ring_slots; ++made) {
+    if (cudaEventCreateWithFlags(&f[made], cudaEventDisableTiming) != cudaSuccess) break;
+    if (cudaEventCreateWithFlags(&u[made], cudaEventDisableTiming) != cudaSuccess) {
+      cudaEventDestroy(f[made]);
+      break;
+    }
+  }
+  delete[] ctx->slot_free;
+  delete[] ctx->slot_full;
+  ctx->slot_free = f; ctx->slot_full = u; ctx->n_slot_events = made;
+  if (made < ring_slots) { ctx->last_cuda_error = (int)cudaGetLastError(); return ARGUS_ECUDA; }
+  return ARGUS_OK;
 }
 
 extern "C" int argus_aggregate_host(argus_ctx* ctx, const argus_event* h_events, uint64_t n,
@@ -178,49 +274,36 @@ extern "C" int argus_aggregate_host(argus_ctx* ctx, const argus_event* h_events,
                                     void* d_records, void* stream) {
   if (!ctx || !d_records) return ARGUS_EINVAL;
   if (d_records != ctx->d_records) return ARGUS_ESTATE;
-  if (n == 0) return ARGUS_OK;
-  if (!h_events || !d_ring || !aligned16(d_ring) || ring_slots == 0 || chunk_events == 0)
-    return ARGUS_EINVAL;
-  if (chunk_events >= (1ull << 32)) return ARGUS_ESIZE;
   cudaStream_t s = (cudaStream_t)stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
-  if (ctx->n_slot_events < ring_slots) {
-    cudaEvent_t* f = new (std::nothrow) cudaEvent_t[ring_slots];
-    cudaEvent_t* u = new (std::nothrow) cudaEvent_t[ring_slots];
-    if (!f || !u) { delete[] f; delete[] u; return ARGUS_ENOMEM; }
-    for (uint32_t i = 0; i < ctx->n_slot_events; ++i) { f[i] = ctx->slot_free[i]; u[i] = ctx->slot_full[i]; }
-    uint32_t made = ctx->n_slot_events;
-    for (; made < ring_slots; ++made) {
-      if (cudaEventCreateWithFlags(&f[made], cudaEventDisableTiming) != cudaSuccess) break;
-      if (cudaEventCreateWithFlags(&u[made], cudaEventDisableTiming) != cudaSuccess) {
-        cudaEventDestroy(f[made]);
-        break;
-      }
-    }
-    delete[] ctx->slot_free;
-    delete[] ctx->slot_full;
-    ctx->slot_free = f; ctx->slot_full = u; ctx->n_slot_events = made;
-    if (made < ring_slots) { ctx->last_cuda_error = (int)cudaGetLastError(); return ARGUS_ECUDA; }
-  }
+  int rc = note_stream(ctx, s);
+  if (rc == ARGUS_OK) rc = wait_ingest(ctx, s);    // an argus_ingest the caller queued before us stays ordered
+  if (rc != ARGUS_OK || n == 0) return rc;
+  if (!h_events || !d_ring || !aligned16(d_ring) || ring_slots == 0 || ring_slots > 64u || chunk_events == 0)
+    return ARGUS_EINVAL;
+  if (chunk_events >= (1ull << 32)) return ARGUS_ESIZE;
+  rc = ensure_slot_events(ctx, ring_slots);
+  if (rc != ARGUS_OK) return rc;
+  ctx->finalized = false;
   // the copy stream must not run ahead of work already queued on `stream` that may still read the
   // ring (an earlier call): order it after the compute stream's current tail
-  CU(ctx, cudaEventRecord(ctx->ingest_event, s));
-  CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ingest_event, 0));
+  CU(ctx, cudaEventRecord(ctx->order_event, s));
+  CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->order_event, 0));
   const uint64_t n_chunks = (n + chunk_events - 1) / chunk_events;
   for (uint64_t c = 0; c < n_chunks; ++c) {
     const uint32_t slot = (uint32_t)(c % ring_slots);
     const uint64_t cnt = (c + 1 == n_chunks) ? n - c * chunk_events : chunk_events;
     argus_event* dst = d_ring + (size_t)slot * chunk_events;
+    // slot reuse: the copy of chunk c waits for the aggregation of chunk c - ring_slots
     if (c >= ring_slots) CU(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->slot_free[slot], 0));
     CU(ctx, cudaMemcpyAsync(dst, h_events + c * chunk_events, cnt * sizeof(argus_event),
                             cudaMemcpyHostToDevice, ctx->copy_stream));
     CU(ctx, cudaEventRecord(ctx->slot_full[slot], ctx->copy_stream));
     CU(ctx, cudaStreamWaitEvent(s, ctx->slot_full[slot], 0));
-    int rc = aggregate_impl(ctx, dst, cnt, d_records, s);
+    rc = aggregate_impl(ctx, dst, cnt, d_records, s);
     if (rc != ARGUS_OK) return rc;
     CU(ctx, cudaEventRecord(ctx->slot_free[slot], s));
   }
-  ctx->last_stream = s;
   return ARGUS_OK;
 }
 
@@ -230,7 +313,8 @@ extern "C" int argus_phase_times(argus_ctx* ctx, void* d_records, argus_span* d_
   if (d_spans_out && !aligned16(d_spans_out)) return ARGUS_EINVAL;
   cudaStream_t s = (cudaStream_t)stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
-  ctx->last_stream = s;
+  int rc = note_stream(ctx, s);
+  if (rc != ARGUS_OK) return rc;
   CU(ctx, argus_launch_finalize(ctx, d_records, d_spans_out, s));
   ctx->finalized = true;
   return ARGUS_OK;
@@ -240,12 +324,16 @@ extern "C" int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus
   if (!ctx || !d_records || !outs || !aligned16(d_records)) return ARGUS_EINVAL;
   if ((outs->sig_stats && !aligned16(outs->sig_stats)) || (outs->span_stats && !aligned16(outs->span_stats)))
     return ARGUS_EINVAL;
+  if (((uintptr_t)outs->rank_score & 3u) || ((uintptr_t)outs->step_anomalous & 3u)) return ARGUS_EINVAL;
+  // our own table must be finalised (span_ns, headers, identities of untouched records); a foreign
+  // finalised table (e.g. one read back from storage) is gathered from its records
+  const bool own = d_records == ctx->d_records;
+  if (own && !ctx->finalized) return ARGUS_ESTATE;
   cudaStream_t s = (cudaStream_t)stream;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
-  ctx->last_stream = s;
-  // the sum plane mirrors the table given to argus_reset, finalised by argus_phase_times
-  const bool use_sums = ctx->dims.sums != nullptr && d_records == ctx->d_records && ctx->finalized;
-  CU(ctx, argus_launch_diagnose(ctx, d_records, outs, use_sums, s));
+  int rc = note_stream(ctx, s);
+  if (rc != ARGUS_OK) return rc;
+  CU(ctx, argus_launch_diagnose(ctx, d_records, outs, /*use_sums=*/own, s));
   return ARGUS_OK;
 }
 
@@ -253,7 +341,7 @@ extern "C" int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invali
   if (!ctx) return ARGUS_EINVAL;
   CU(ctx, cudaSetDevice(ctx->cfg.device));
   CU(ctx, cudaStreamSynchronize(ctx->copy_stream));
-  CU(ctx, cudaStreamSynchronize(ctx->last_stream));
+  for (uint32_t i = 0; i < ctx->n_streams; ++i) CU(ctx, cudaStreamSynchronize(ctx->streams[i]));
   unsigned long long h[2] = {0, 0};
   CU(ctx, cudaMemcpy(h, ctx->d_counters, sizeof h, cudaMemcpyDeviceToHost));
   h[0] -= h[1];  // kernels count events seen and events rejected
@@ -262,15 +350,19 @@ extern "C" int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invali
   return ARGUS_OK;
 }
 
+extern "C" int argus_launch_count(const argus_ctx* ctx, uint64_t* kernels, uint64_t* memsets) {
+  if (!ctx) return ARGUS_EINVAL;
+  if (kernels) *kernels = ctx->n_kernels;
+  if (memsets) *memsets = ctx->n_memsets;
+  return ARGUS_OK;
+}
+
 extern "C" int argus_tune(argus_ctx* ctx, int which, int64_t value) {
   if (!ctx) return ARGUS_EINVAL;
   switch (which) {
     case ARGUS_TUNE_GRID_CTAS:
-      if (value < 0 || value > 65535) return ARGUS_EINVAL;
+      if (value < 0 || value > (int64_t)ARGUS_MAX_SEG_CTAS) return ARGUS_EINVAL;
       ctx->tune_grid = (int)value;
-      return ARGUS_OK;
-    case ARGUS_TUNE_SEG_VARIANT:
-      ctx->tune_variant = (int)value;
       return ARGUS_OK;
     case ARGUS_TUNE_FORCE_PATH:
       if (value < 0 || value > 3) return ARGUS_EINVAL;
@@ -294,4 +386,4 @@ extern "C" const char* argus_strerror(int code) {
 }
 
 extern "C" int argus_last_cuda_error(const argus_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
-extern "C" const char* argus_version(void) { return "argus-b200 0.1.0 (sm_100a)"; }
+extern "C" const char* argus_version(void) { return "argus-b200 0.2.0 (sm_100a)"; }

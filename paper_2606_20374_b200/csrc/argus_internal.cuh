@@ -18,43 +18,55 @@ struct argus_dims {
   uint32_t rec_bytes;   // 64 + 32*(P+1) + 160*S
   uint32_t span_off;    // 64
   uint32_t cell_off;    // 64 + 32*(P+1)
-  // Sum plane (ctx workspace, may be null): sums[(rank*T + t)*S + sig] mirrors cell.sum_ns of the table
+  // Sum plane (workspace; null in kernels that must not touch it): sums[(rank*T + t)*S + sig] mirrors cell.sum_ns of the table
   // given to argus_reset, sig-contiguous, so that the cross-rank gather of argus_diagnose reads whole
   // sectors of neighbouring sigs instead of one 32-byte sector per 160-byte cell.  Every kernel that
   // writes a cell's sum (flush, merge, global path, identity fill) keeps it in step.
   unsigned long long* sums;
 };
 
+// Areas of the device workspace (argus_workspace_bytes): byte offsets from its base, each 256-byte
+// aligned; computed by one function so that argus_workspace_bytes and argus_create cannot disagree.
+#define ARGUS_MAX_SEG_CTAS 1024u      // CTAs of one segmented launch (bounds the overflow-list area)
+#define ARGUS_OVF_CAP 4096u           // entries (16 B) of one CTA's overflow list
+struct argus_ws_layout {
+  size_t state, counters, hist, sums, ovf, diag_todo, part, group, total;
+  uint32_t part_ctas;                 // CTAs of the grouping pass (0: no grouping area)
+  bool part_smem;                     // its key histograms fit shared memory
+};
+void argus_ws_plan(const argus_config* cfg, int sm_count, int max_smem_optin, argus_ws_layout* out);
+
 struct argus_ctx {
   argus_config cfg;
   argus_dims dims;
   int sm_count;
   int max_smem_optin;
+  argus_ws_layout ws;
+  uint8_t* d_ws;              // the workspace (caller's, or ours when ws_owned)
+  bool ws_owned;
   uint32_t* d_state;          // [R*T]
-  unsigned long long* d_counters;  // [2] n_valid, n_invalid
-  uint32_t* d_hist;           // [R*T + 1] group sizes / cursors of the partition pass
-  argus_event* d_group;       // grouping workspace of the partition pass (grown on demand)
-  uint64_t group_capacity;    // events d_group can hold
+  unsigned long long* d_counters;  // [2] events seen, events rejected
+  uint32_t* d_hist;           // [R*T + 1] group sizes / cursors of the grouping pass
+  argus_event* d_group;       // grouping area [cfg.max_ungrouped_events] (null when 0)
   void* fn_tmap_encode;       // cuTensorMapEncodeTiled, resolved through the runtime (no libcuda link)
-  void* d_part;               // per-CTA key histograms of the partition pass [n_cta][R*T + 1]
-  uint64_t part_rows;         // u32 entries d_part holds
-  void* d_diag_todo;          // argus_diagnose: one byte per series, set by the 32-bit pass for the 64-bit pass
-  uint64_t diag_todo_len;
-  void* d_ovf;                // per-CTA overflow lists of the segmented kernel (grown on demand)
-  uint64_t ovf_ctas;          // CTAs d_ovf can serve
+  uint32_t* d_part;           // per-CTA key histograms of the grouping pass [part_ctas][R*T + 1]
+  uint8_t* d_diag_todo;       // argus_diagnose: one byte per series, set by the 32-bit pass for the 64-bit pass
+  uint4* d_ovf;               // per-CTA overflow lists of the segmented kernel [ARGUS_MAX_SEG_CTAS][ARGUS_OVF_CAP]
   void* d_records;            // table given to the last argus_reset
   cudaEvent_t ingest_event;   // recorded after every argus_ingest copy
+  cudaEvent_t order_event;    // argus_aggregate_host: orders the copy stream after the compute stream's tail
   bool ingest_pending;
   bool finalized;             // argus_phase_times ran since the last argus_reset / argus_aggregate
   cudaStream_t copy_stream;   // internal, for argus_aggregate_host
   cudaEvent_t* slot_free;     // ring-slot reuse events (argus_aggregate_host)
   cudaEvent_t* slot_full;
   uint32_t n_slot_events;
-  cudaStream_t last_stream;
+  cudaStream_t streams[8];    // distinct streams seen since argus_create (argus_stats synchronises them)
+  uint32_t n_streams;
   int last_cuda_error;
   int tune_grid;
   int tune_path;
-  int tune_variant;
+  uint64_t n_kernels, n_memsets;   // launches since argus_create (argus_launch_count)
 };
 
 // kernels' host-side launchers (each returns cudaError_t of the launch)
@@ -69,6 +81,15 @@ cudaError_t argus_launch_finalize(argus_ctx* ctx, void* d_records, argus_span* d
 cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
                                   bool use_sums, cudaStream_t s);
 bool argus_seg_supported(const argus_ctx* ctx);
+void argus_partition_plan(const argus_config* cfg, int sm_count, int max_smem_optin, uint32_t* n_cta,
+                          bool* smem);
+// opt-in shared-memory sizes of the kernels this ctx will launch (argus_create, once)
+cudaError_t argus_configure_seg(argus_ctx* ctx);
+cudaError_t argus_configure_partition(argus_ctx* ctx);
+inline cudaError_t argus_configure_kernels(argus_ctx* ctx) {
+  cudaError_t e = argus_configure_seg(ctx);
+  return e == cudaSuccess ? argus_configure_partition(ctx) : e;
+}
 
 // ---- device helpers shared by the kernels ------------------------------------------------------
 #ifdef __CUDACC__

@@ -254,20 +254,12 @@ cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const a
   if (o->rank_score) {
     cudaError_t e = cudaMemsetAsync(o->rank_score, 0, (size_t)D.T * D.R * sizeof(uint32_t), s);
     if (e != cudaSuccess) return e;
+    ctx->n_memsets += 1;
   }
   const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);
   if (blocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
   const uint8_t* rec = static_cast<const uint8_t*>(d_records);
-  if (ctx->diag_todo_len < blocks) {       // one byte per series (grow-only)
-    cudaError_t e = cudaDeviceSynchronize();
-    if (e != cudaSuccess) return e;
-    if (ctx->d_diag_todo) cudaFree(ctx->d_diag_todo);
-    ctx->d_diag_todo = nullptr; ctx->diag_todo_len = 0;
-    e = cudaMalloc(&ctx->d_diag_todo, blocks);
-    if (e != cudaSuccess) return e;
-    ctx->diag_todo_len = blocks;
-  }
-  uint8_t* todo = static_cast<uint8_t*>(ctx->d_diag_todo);
+  uint8_t* todo = ctx->d_diag_todo;        // one mark byte per series (workspace)
   const unsigned nb = (unsigned)blocks;
   if (D.R <= 64u * EPT) {
     diagnose_kernel<64, uint32_t><<<nb, 64, 0, s>>>(rec, D, *o, use_sums, todo);
@@ -279,5 +271,6 @@ cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const a
     diagnose_kernel<1024, uint32_t><<<nb, 1024, 0, s>>>(rec, D, *o, use_sums, todo);
     diagnose_kernel<1024, unsigned long long><<<nb, 1024, 0, s>>>(rec, D, *o, use_sums, todo);
   }
+  ctx->n_kernels += 2;
   return cudaGetLastError();
 }

@@ -61,5 +61,6 @@ cudaError_t argus_launch_finalize(argus_ctx* ctx, void* d_records, argus_span* d
   uint32_t grid = n_rec < (uint32_t)ctx->sm_count * 8u ? n_rec : (uint32_t)ctx->sm_count * 8u;
   finalize_kernel<<<grid, 256, 0, s>>>(static_cast<uint8_t*>(d_records), ctx->d_state, d_spans_out,
                                        ctx->dims, n_rec);
+  ctx->n_kernels += 1;
   return cudaGetLastError();
 }

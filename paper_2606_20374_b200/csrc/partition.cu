@@ -16,7 +16,7 @@
 //   scatter : the same CTA re-reads its chunk with cursor[key] = total[key] + H[cta][key] in shared
 //             memory: pos = atomicAdd(&cursor[key], 1); grouped[pos] = event
 // When R*T + 1 counters do not fit shared memory, count and scatter use L2 atomics on one global
-// counter array instead (same results, slower).
+// counter array instead (same results, slower).  All buffers are areas of the ctx workspace.
 // Events whose key fields are out of range travel in the last bin, so that the segmented kernel
 // still sees (and counts) every event; sig / phase / timestamp validity is its business.
 #include "argus_internal.cuh"
@@ -143,51 +143,44 @@ partition_scatter_smem_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t
 
 }  // namespace
 
-// Group n events by (rank, step) into ctx->d_group (grown on demand).  Returns cudaErrorMemoryAllocation
-// if the workspace cannot be had (the caller then falls back to the global-table kernel).
+// CTAs of the grouping pass and whether their key histograms (R*T + 1 counters) fit shared memory.
+void argus_partition_plan(const argus_config* cfg, int sm_count, int max_smem_optin, uint32_t* n_cta,
+                          bool* smem) {
+  const size_t bin_bytes = sizeof(uint32_t) * ((size_t)cfg->n_ranks * cfg->n_steps + 1u);
+  *smem = bin_bytes <= 200u * 1024u && bin_bytes + 1024u <= (size_t)max_smem_optin;
+  *n_cta = *smem ? (uint32_t)sm_count * (bin_bytes <= 100u * 1024u ? 2u : 1u) : 0u;
+}
+
+cudaError_t argus_configure_partition(argus_ctx* ctx) {
+  if (!ctx->ws.part_smem) return cudaSuccess;
+  const int bin_bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->dims.R * ctx->dims.T + 1u));
+  cudaError_t e = cudaFuncSetAttribute(partition_count_smem_kernel,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, bin_bytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(partition_scatter_smem_kernel,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, bin_bytes);
+  return e;
+}
+
+// Group n <= cfg.max_ungrouped_events events by (rank, step) into the grouping area ctx->d_group.
 cudaError_t argus_launch_partition(argus_ctx* ctx, const argus_event* ev, uint64_t n, cudaStream_t s) {
   const argus_dims& D = ctx->dims;
   const uint32_t m = D.R * D.T + 1u;
-  if (ctx->group_capacity < n) {
-    // grow-only; the old buffer may still be read by work queued on a stream: drain first
-    cudaError_t e = cudaDeviceSynchronize();
-    if (e != cudaSuccess) return e;
-    if (ctx->d_group) cudaFree(ctx->d_group);
-    ctx->d_group = nullptr; ctx->group_capacity = 0;
-    e = cudaMalloc(&ctx->d_group, n * sizeof(argus_event));
-    if (e != cudaSuccess) { (void)cudaGetLastError(); return cudaErrorMemoryAllocation; }
-    ctx->group_capacity = n;
-  }
   const uint4* src = reinterpret_cast<const uint4*>(ev);
   const size_t bin_bytes = sizeof(uint32_t) * (size_t)m;
-  if (bin_bytes <= 200u * 1024u && bin_bytes + 1024u <= (size_t)ctx->max_smem_optin) {
+  if (ctx->ws.part_smem) {
     // per-CTA shared-memory histograms
-    const uint32_t per_sm = bin_bytes <= 100u * 1024u ? 2u : 1u;
-    uint32_t n_cta = (uint32_t)ctx->sm_count * per_sm;
+    uint32_t n_cta = ctx->ws.part_ctas;
     uint64_t chunk = (n + n_cta - 1) / n_cta;
     chunk = (chunk + 1023) / 1024 * 1024;
     n_cta = (uint32_t)((n + chunk - 1) / chunk);
-    if (ctx->part_rows < (uint64_t)n_cta * m) {
-      cudaError_t e = cudaDeviceSynchronize();
-      if (e != cudaSuccess) return e;
-      if (ctx->d_part) cudaFree(ctx->d_part);
-      ctx->d_part = nullptr; ctx->part_rows = 0;
-      e = cudaMalloc(&ctx->d_part, sizeof(uint32_t) * (size_t)n_cta * m);
-      if (e != cudaSuccess) { (void)cudaGetLastError(); return cudaErrorMemoryAllocation; }
-      ctx->part_rows = (uint64_t)n_cta * m;
-    }
-    cudaError_t e = cudaFuncSetAttribute(partition_count_smem_kernel,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bin_bytes);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(partition_scatter_smem_kernel,
-                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bin_bytes);
-    if (e != cudaSuccess) return e;
-    uint32_t* H = static_cast<uint32_t*>(ctx->d_part);
+    uint32_t* H = ctx->d_part;
     partition_count_smem_kernel<<<n_cta, 1024, bin_bytes, s>>>(src, n, chunk, D, m, H);
     partition_offsets_kernel<<<(m + 255u) / 256u, 256, 0, s>>>(H, n_cta, m, ctx->d_hist);
     partition_scan_kernel<<<1, 1024, 0, s>>>(ctx->d_hist, m);
     partition_scatter_smem_kernel<<<n_cta, 1024, bin_bytes, s>>>(src, n, chunk, D, m, H, ctx->d_hist,
                                                                  reinterpret_cast<uint4*>(ctx->d_group));
+    ctx->n_kernels += 4;
     return cudaGetLastError();
   }
   // too many groups for shared memory: one global counter array, L2 atomics
@@ -200,5 +193,7 @@ cudaError_t argus_launch_partition(argus_ctx* ctx, const argus_event* ev, uint64
   partition_scan_kernel<<<1, 1024, 0, s>>>(ctx->d_hist, m);
   partition_scatter_kernel<<<(unsigned)blocks, 512, 0, s>>>(src, n, D, ctx->d_hist,
                                                             reinterpret_cast<uint4*>(ctx->d_group));
+  ctx->n_memsets += 1;
+  ctx->n_kernels += 3;
   return cudaGetLastError();
 }

@@ -23,6 +23,8 @@ def init_world(n_gpus: int, backend: Optional[str] = None) -> World:
     """Join the process group torchrun set up (RANK / WORLD_SIZE / MASTER_* in the environment).
     A plain `python bench.py` run (no WORLD_SIZE) is a world of one and needs no group."""
     size = int(os.environ.get("WORLD_SIZE", "1"))
+    if n_gpus not in (0, size):
+        raise RuntimeError(f"--gpus {n_gpus} but WORLD_SIZE={size}: launch one rank per GPU (torchrun)")
     if size == 1:
         return World()
     rank = int(os.environ["RANK"])
@@ -32,8 +34,6 @@ def init_world(n_gpus: int, backend: Optional[str] = None) -> World:
         torch.cuda.set_device(local_rank)
     if not dist.is_initialized():
         dist.init_process_group(backend=backend, rank=rank, world_size=size)
-    if n_gpus not in (0, size):
-        raise RuntimeError(f"--gpus {n_gpus} but WORLD_SIZE={size}")
     return World(rank, size, local_rank, backend)
 
 

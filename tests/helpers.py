@@ -97,7 +97,7 @@ def check_against_bruteforce(cells_arr, spans_arr, ev, R, T, S, P, step_base):
 
 
 def parse_handworked():
-    ev, cells, spans, ds, dp = [], [], [], [], []
+    ev, cells, spans, ds, dp, hdrs = [], [], [], [], [], []
     n = rs = sa = None
     with open(os.path.join(GOLDEN, "handworked.txt")) as f:
         for line in f:
@@ -117,6 +117,8 @@ def parse_handworked():
                 cells.append((int(a[0]), int(a[1]), [int(v) for v in a[2:6]], hist))
             elif k == "S":
                 spans.append((int(a[0]), int(a[1]), [int(v) for v in a[2:6]]))
+            elif k == "H":
+                hdrs.append(tuple(int(v) for v in a))
             elif k == "DS":
                 ds.append((int(a[0]), int(a[1]), int(a[2]), [int(v) for v in a[3:]]))
             elif k == "DP":
@@ -125,7 +127,20 @@ def parse_handworked():
                 rs = [int(v) for v in a]
             elif k == "SA":
                 sa = [int(v) for v in a]
-    return dict(events=make_events(ev), n=n, cells=cells, spans=spans, ds=ds, dp=dp, rs=rs, sa=sa)
+    return dict(events=make_events(ev), n=n, cells=cells, spans=spans, ds=ds, dp=dp, rs=rs, sa=sa,
+                headers=hdrs)
+
+
+def check_handworked_headers(g, hdr, n_sigs=2, n_phases=2):
+    """hdr: HEADER-like structured array [R][T] of any implementation vs the golden H lines."""
+    assert len(g["headers"]) == hdr.size
+    for r, t, n, mn, mx, it in g["headers"]:
+        h = hdr[r, t]
+        assert int(h["magic"]) == int.from_bytes(b"ARGS", "little") and int(h["version"]) == 1
+        assert (int(h["n_phases"]), int(h["n_sigs"])) == (n_phases, n_sigs)
+        assert (int(h["rank"]), int(h["step"])) == (r, t)
+        assert (int(h["n_events"]), int(h["min_start"]), int(h["max_end"]), int(h["iter_ns"])) == (n, mn, mx, it), (r, t)
+        assert int(h["reserved0"]) == 0 and int(h["reserved1"]) == 0
 
 
 def parse_series_cases():

@@ -45,9 +45,17 @@ def test_create_rejects_bad_config_without_touching_cuda():
     for cfg in (A.ArgusConfig(0, 1, 1, 1, 0, 0, 0, 0), A.ArgusConfig(1, 0, 1, 1, 0, 0, 0, 0),
                 A.ArgusConfig(1, 1, 0, 1, 0, 0, 0, 0), A.ArgusConfig(1, 1, 1, 0, 0, 0, 0, 0),
                 A.ArgusConfig(1, 1, 1, 65, 0, 0, 0, 0), A.ArgusConfig(16385, 1, 1, 1, 0, 0, 0, 0)):
-        assert lib.argus_create(ctypes.byref(cfg), ctypes.byref(h)) == A.EINVAL
-    assert lib.argus_create(None, ctypes.byref(h)) == A.EINVAL
-    assert lib.argus_create(ctypes.byref(A.ArgusConfig(16384, 1 << 20, 1, 1, 0, 0, 0, 0)), ctypes.byref(h)) == A.ESIZE
+        assert lib.argus_create(ctypes.byref(cfg), None, 0, ctypes.byref(h)) == A.EINVAL
+        assert lib.argus_workspace_bytes(ctypes.byref(cfg)) == 0
+    assert lib.argus_create(None, None, 0, ctypes.byref(h)) == A.EINVAL
+    assert lib.argus_workspace_bytes(None) == 0
+    for cfg in (A.ArgusConfig(16384, 1 << 20, 1, 1, 0, 0, 0, 0),        # R*T >= 2^31
+                A.ArgusConfig(1, 1, 1 << 25, 1, 0, 0, 0, 0),            # record >= 4 GiB
+                A.ArgusConfig(2, 4, 2, 1, 0xFFFFFFFE, 0, 0, 0),         # step_base + T wraps (R19)
+                A.ArgusConfig(1, 1 << 12, 1 << 20, 1, 0, 0, 0, 0)):     # more series than one grid
+        assert lib.argus_create(ctypes.byref(cfg), None, 0, ctypes.byref(h)) == A.ESIZE
+    ok = A.ArgusConfig(2, 4, 2, 1, 0xFFFFFFFC, 0, 0, 0)                 # step_base + T == 2^32 is fine
+    assert lib.argus_create(ctypes.byref(ok), ctypes.c_void_p(128), 1 << 30, ctypes.byref(h)) == A.EINVAL  # misaligned workspace
     assert lib.argus_destroy(None) == A.EINVAL
     assert lib.argus_aggregate(None, None, 0, None, None) == A.EINVAL
 
@@ -60,5 +68,8 @@ def test_no_cpu_fallback():
     lib = A.load()
     h = ctypes.c_void_p()
     cfg = A.ArgusConfig(2, 1, 2, 1, 0, 1, 0, 0)
-    assert lib.argus_create(ctypes.byref(cfg), ctypes.byref(h)) in (A.ECUDA, A.ENOMEM)
+    assert lib.argus_create(ctypes.byref(cfg), None, 0, ctypes.byref(h)) in (A.ECUDA, A.ENOMEM)
     assert not h.value
+    import pytest
+    with pytest.raises(A.ArgusError):
+        A.Argus(2, 1, 2, 1)

@@ -228,6 +228,40 @@ def test_record_layout(tiny):
     assert (ce.reshape(s.n_ranks, s.n_steps, -1) == o.cells()).all()
     assert (hdr["n_events"] == s.n_events).all()
     assert (hdr["iter_ns"] == o.spans()["span"][:, :, s.n_phases].reshape(-1)).all()
+    # every header byte is pinned: the two timestamps against a Python-int brute force over the raw
+    # events (first start / last end of each rank-step; swapping them in the oracle fails here), the
+    # reserved words are zero, and nothing else lives in the 64 bytes
+    assert (hdr["reserved0"] == 0).all() and (hdr["reserved1"] == 0).all()
+    for i, h in enumerate(hdr):
+        r, t = divmod(i, s.n_steps)
+        sel = ev[(ev["rank"] == r) & (ev["step"] == s.step_base + t)]
+        mn = min(int(v) for v in sel["start_ns"])
+        mx = max(int(v) for v in sel["end_ns"])
+        assert (int(h["min_start"]), int(h["max_end"]), int(h["iter_ns"])) == (mn, mx, mx - mn), (r, t)
+        assert int(h["min_start"]) < int(h["max_end"])
+    want = np.zeros(hdr.size, dtype=HEADER_DTYPE)
+    for f in HEADER_DTYPE.names:
+        want[f] = hdr[f]
+    assert (want.view(np.uint8) == rec[:, :64].reshape(-1)).all()      # no byte outside the named fields
+
+
+def test_record_header_handworked():
+    """The H lines of tests/golden/handworked.txt (worked by hand) pin the oracle's header fields, and
+    an untouched record's header carries the empty-span identities (R7, R17)."""
+    from helpers import check_handworked_headers
+    from oracle import HEADER_DTYPE
+    g = parse_handworked()
+    o = Oracle(3, 1, 2, 2, 0)
+    o.aggregate(g["events"])
+    rec = o.records()
+    check_handworked_headers(g, rec[:, :64].copy().view(HEADER_DTYPE).reshape(3, 1))
+    o2 = Oracle(2, 2, 3, 1, 50)
+    o2.aggregate(make_events([(1, 51, 2, 0, 0, 10, 30)]))
+    h = o2.records()[:, :64].copy().view(HEADER_DTYPE).reshape(2, 2)
+    assert [int(h[1, 1][f]) for f in ("rank", "step", "n_events", "min_start", "max_end", "iter_ns")] == [1, 51, 1, 10, 30, 20]
+    for r, t in ((0, 0), (0, 1), (1, 0)):
+        assert [int(h[r, t][f]) for f in ("rank", "step", "n_events", "min_start", "max_end", "iter_ns")] == \
+            [r, 50 + t, 0, 2**63 - 1, -2**63, 0]
 
 
 # ---- detection: injected faults are recovered (recall only; precision is not asserted) --------

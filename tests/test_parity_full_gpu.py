@@ -22,12 +22,14 @@ def _full_parity(name, chunk_ranks):
     wl = build_workload(name)
     s = wl.spec
     free, _ = torch.cuda.mem_get_info()
-    need = s.total_events * 32 + s.n_ranks * s.n_steps * (64 + 32 * (s.n_phases + 1) + 160 * s.n_sigs)
+    need = s.total_events * 32 * (2 if s.shuffle else 1) + \
+        s.n_ranks * s.n_steps * (64 + 32 * (s.n_phases + 1) + 168 * s.n_sigs)
     if free < need * 1.05:
         pytest.skip(f"{name}: needs {need / 1e9:.1f} GB of HBM, {free / 1e9:.1f} GB free")
     # ---- CUDA path, as bench.py runs it ----------------------------------------------------------
     d_ev = wl.expand_device()
-    ctx = A.Argus(s.n_ranks, s.n_steps, s.n_sigs, s.n_phases, s.step_base, sorted_hint=not s.shuffle)
+    ctx = A.Argus(s.n_ranks, s.n_steps, s.n_sigs, s.n_phases, s.step_base, sorted_hint=not s.shuffle,
+                  max_ungrouped_events=s.total_events if s.shuffle else 0)
     rec = ctx.alloc_records()
     outs = ctx.alloc_diag()
     ctx.reset(rec)
