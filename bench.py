@@ -296,6 +296,8 @@ def run_ours(args, world):
             g1.record()
             torch.cuda.synchronize()
             t_total = g0.elapsed_time(g1)
+            ctx.phase_times(rec)                  # leave a finalised table behind (parity_check below)
+            torch.cuda.synchronize()
             e2e = {"value": total_events / (e_ms * 1e-3), "unit": "events/s", "ms_per_step": e_ms,
                    "steps": e2e_steps, "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": d2h,
                    "h2d_gbs": 32 * n / (e_ms * 1e-3) / 1e9, "chunk_bytes": chunk * 32,

@@ -217,6 +217,41 @@ int argus_phase_times(argus_ctx* ctx, void* d_records, argus_span* d_spans_out, 
  * plus the roll-ups of R15.  [host] outs holds [device] pointers. */
 int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* outs, void* stream);
 
+/* ---- one job sharded by trace rank over several GPUs (the paper's comparison of "the same
+ * kernel across different ranks", when the ranks' events live on different devices) --------
+ * Every GPU g aggregates its own ranks [r0_g, r0_g + R_g) with a ctx of n_ranks = R_g (events carry
+ * rank - r0_g).  Aggregation and spans need no exchange.  The cross-rank rule needs, per (step, series),
+ * the value of EVERY rank: the one exchange is the 8-byte-per-cell sum plane (and the tiny span plane),
+ * transposed so that GPU d owns a slice of the sigs for ALL ranks:
+ *     sig plane  of a slice [s0, s1):  x[r] of series (t, s) at  plane[((t*(s1-s0) + (s-s0)) * rank_stride + r]
+ *     span plane:                      x[r] of series (t, k) at  plane[((t*(P+1) + k) * rank_stride + r]
+ * argus_pack_planes writes this ctx's ranks into columns [rank_offset, rank_offset + R_g) of such planes;
+ * the destination may be local memory (a send buffer for an all-to-all: rank_stride = R_g, rank_offset = 0)
+ * or the owning peer's plane mapped over NVLink (rank_stride = R, rank_offset = r0_g: the exchange is then
+ * the kernel's own coalesced stores, rows of R_g contiguous u64).  argus_diagnose_planes runs the rule
+ * of argus_diagnose on planes; rank_score comes out as the partial count over the slice's sigs (sum the
+ * partials of all slices), every other output is final for the series of the slice. */
+typedef struct argus_planes {
+  const uint64_t* sig_sums;    /* [device] [T][n_sigs][rank_stride] u64 summed durations (0 = empty cell, R11), or NULL */
+  const uint64_t* span_ns;     /* [device] [T][P+1][rank_stride]    u64 span_ns, or NULL */
+  uint32_t n_ranks;            /* R of the whole job, 1..ARGUS_MAX_RANKS */
+  uint32_t rank_stride;        /* >= n_ranks, in elements */
+  uint32_t n_sigs;             /* sigs of this slice (0 with sig_sums == NULL); <= cfg.n_sigs of the ctx */
+  uint32_t reserved;           /* 0 */
+} argus_planes;
+
+/* Export sigs [sig_lo, sig_hi) of this ctx's finalised table (argus_phase_times ran; ARGUS_ESTATE otherwise)
+ * into [device] planes as laid out above.  d_sig_plane and/or d_span_plane may be NULL to skip.
+ * 8-byte aligned; rank_offset + cfg.n_ranks <= rank_stride.  Asynchronous on `stream`. */
+int argus_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t sig_lo, uint32_t sig_hi,
+                      uint64_t* d_sig_plane, uint64_t* d_span_plane, uint32_t rank_stride,
+                      uint32_t rank_offset, void* stream);
+
+/* The cross-rank rule (R10-R15) on planes: outs->sig_stats [T][n_sigs], sig_flags [T][n_sigs][R],
+ * span_stats [T][P+1], span_flags [T][P+1][R], rank_score [T][R] (partial: this slice's sigs),
+ * step_anomalous [T]; T and P are the ctx's, R = planes->n_ranks.  [host] planes, [host] outs. */
+int argus_diagnose_planes(argus_ctx* ctx, const argus_planes* planes, const argus_diag_out* outs, void* stream);
+
 /* Synchronises the internal copy stream and every stream passed to this ctx since argus_create (the ctx
  * remembers up to 8 distinct ones; the oldest is synchronised when a ninth appears) and returns the event
  * counters since argus_reset.  Asynchronous kernel faults surface here as ARGUS_ECUDA.  [host] outputs,

@@ -32,7 +32,8 @@ HEADER_DTYPE = np.dtype([("magic", "<u4"), ("version", "<u2"), ("n_phases", "<u2
 
 EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes",
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
-           "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_stats",
+           "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
+           "argus_diagnose_planes", "argus_stats",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
 
@@ -48,6 +49,12 @@ class ArgusDiagOut(ctypes.Structure):
     _fields_ = [("sig_stats", ctypes.c_void_p), ("sig_flags", ctypes.c_void_p),
                 ("span_stats", ctypes.c_void_p), ("span_flags", ctypes.c_void_p),
                 ("rank_score", ctypes.c_void_p), ("step_anomalous", ctypes.c_void_p)]
+
+
+class ArgusPlanes(ctypes.Structure):
+    _fields_ = [("sig_sums", ctypes.c_void_p), ("span_ns", ctypes.c_void_p),
+                ("n_ranks", ctypes.c_uint32), ("rank_stride", ctypes.c_uint32),
+                ("n_sigs", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
 
 
 class ArgusError(RuntimeError):
@@ -89,6 +96,11 @@ def load() -> ctypes.CDLL:
     lib.argus_phase_times.argtypes = [vp, vp, vp, vp]
     lib.argus_diagnose.restype = i32
     lib.argus_diagnose.argtypes = [vp, vp, ctypes.POINTER(ArgusDiagOut), vp]
+    lib.argus_pack_planes.restype = i32
+    lib.argus_pack_planes.argtypes = [vp, vp, ctypes.c_uint32, ctypes.c_uint32, vp, vp, ctypes.c_uint32,
+                                      ctypes.c_uint32, vp]
+    lib.argus_diagnose_planes.restype = i32
+    lib.argus_diagnose_planes.argtypes = [vp, ctypes.POINTER(ArgusPlanes), ctypes.POINTER(ArgusDiagOut), vp]
     lib.argus_stats.restype = i32
     lib.argus_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_launch_count.restype = i32
@@ -231,6 +243,19 @@ class Argus:
                                                        "span_flags", "rank_score", "step_anomalous")])
         self._check(self.lib.argus_diagnose(self._h, _ptr(d_records), ctypes.byref(o),
                                             _stream(stream)))
+
+    def pack_planes(self, d_records, sig_lo: int, sig_hi: int, d_sig_plane, d_span_plane,
+                    rank_stride: int, rank_offset: int, stream=None) -> None:
+        self._check(self.lib.argus_pack_planes(self._h, _ptr(d_records), sig_lo, sig_hi, _ptr(d_sig_plane),
+                                               _ptr(d_span_plane), rank_stride, rank_offset, _stream(stream)))
+
+    def diagnose_planes(self, d_sig_plane, d_span_plane, n_ranks: int, rank_stride: int, n_sigs: int,
+                        outs: dict, stream=None) -> None:
+        pl = ArgusPlanes(_ptr(d_sig_plane), _ptr(d_span_plane), n_ranks, rank_stride, n_sigs, 0)
+        o = ArgusDiagOut(*[_ptr(outs.get(k)) for k in ("sig_stats", "sig_flags", "span_stats",
+                                                       "span_flags", "rank_score", "step_anomalous")])
+        self._check(self.lib.argus_diagnose_planes(self._h, ctypes.byref(pl), ctypes.byref(o),
+                                                   _stream(stream)))
 
     def stats(self):
         a, b = ctypes.c_uint64(), ctypes.c_uint64()

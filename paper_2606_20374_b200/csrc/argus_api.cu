@@ -337,6 +337,42 @@ extern "C" int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus
   return ARGUS_OK;
 }
 
+static bool aligned8(const void* p) { return ((uintptr_t)p & 7u) == 0; }
+
+extern "C" int argus_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t sig_lo, uint32_t sig_hi,
+                                 uint64_t* d_sig_plane, uint64_t* d_span_plane, uint32_t rank_stride,
+                                 uint32_t rank_offset, void* stream) {
+  if (!ctx || !d_records) return ARGUS_EINVAL;
+  if (d_records != ctx->d_records || !ctx->finalized) return ARGUS_ESTATE;   // the sum plane mirrors OUR table
+  if (sig_lo > sig_hi || sig_hi > ctx->dims.S) return ARGUS_EINVAL;
+  if (!aligned8(d_sig_plane) || !aligned8(d_span_plane)) return ARGUS_EINVAL;
+  if ((uint64_t)rank_offset + ctx->dims.R > rank_stride) return ARGUS_EINVAL;
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(ctx, cudaSetDevice(ctx->cfg.device));
+  int rc = note_stream(ctx, s);
+  if (rc != ARGUS_OK) return rc;
+  CU(ctx, argus_launch_pack_planes(ctx, d_records, sig_lo, sig_hi, d_sig_plane, d_span_plane, rank_stride,
+                                   rank_offset, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_diagnose_planes(argus_ctx* ctx, const argus_planes* pl, const argus_diag_out* outs,
+                                     void* stream) {
+  if (!ctx || !pl || !outs) return ARGUS_EINVAL;
+  if (pl->n_ranks == 0 || pl->n_ranks > ARGUS_MAX_RANKS || pl->rank_stride < pl->n_ranks) return ARGUS_EINVAL;
+  if (pl->n_sigs > ctx->dims.S || (pl->n_sigs != 0) != (pl->sig_sums != nullptr)) return ARGUS_EINVAL;
+  if (!aligned8(pl->sig_sums) || !aligned8(pl->span_ns)) return ARGUS_EINVAL;
+  if ((outs->sig_stats && !aligned16(outs->sig_stats)) || (outs->span_stats && !aligned16(outs->span_stats)))
+    return ARGUS_EINVAL;
+  if (((uintptr_t)outs->rank_score & 3u) || ((uintptr_t)outs->step_anomalous & 3u)) return ARGUS_EINVAL;
+  cudaStream_t s = (cudaStream_t)stream;
+  CU(ctx, cudaSetDevice(ctx->cfg.device));
+  int rc = note_stream(ctx, s);
+  if (rc != ARGUS_OK) return rc;
+  CU(ctx, argus_launch_diagnose_planes(ctx, pl, outs, s));
+  return ARGUS_OK;
+}
+
 extern "C" int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid) {
   if (!ctx) return ARGUS_EINVAL;
   CU(ctx, cudaSetDevice(ctx->cfg.device));

@@ -80,6 +80,11 @@ cudaError_t argus_launch_finalize(argus_ctx* ctx, void* d_records, argus_span* d
                                   cudaStream_t s);
 cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
                                   bool use_sums, cudaStream_t s);
+cudaError_t argus_launch_diagnose_planes(argus_ctx* ctx, const argus_planes* pl, const argus_diag_out* o,
+                                         cudaStream_t s);
+cudaError_t argus_launch_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t s0, uint32_t s1,
+                                     uint64_t* dst_sig, uint64_t* dst_span, uint32_t stride, uint32_t off,
+                                     cudaStream_t s);
 bool argus_seg_supported(const argus_ctx* ctx);
 void argus_partition_plan(const argus_config* cfg, int sm_count, int max_smem_optin, uint32_t* n_cta,
                           bool* smem);

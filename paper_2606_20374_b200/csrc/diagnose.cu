@@ -159,10 +159,22 @@ __device__ K block_median(const K (&v)[EPT], uint32_t R, SelSmem& sm) {
 // sums of one kernel differ by far less than 4.29 s) is selected on exact 32-bit offsets from its
 // minimum — half the registers, twice the resident CTAs; |x - med| fits 32 bits too.  A wider series is
 // only marked in todo[].  K = unsigned long long: the second pass, which does the marked series.
+// Where the series come from: the record table (and, for the sig series of the ctx's own table, its sum
+// plane), or rank-contiguous planes handed in by the caller (argus_diagnose_planes: the exchanged
+// planes of a rank-sharded job).
+struct DiagSrc {
+  const uint8_t* records;
+  const unsigned long long* sig_plane;    // [T][S][rank_stride] or null
+  const unsigned long long* span_plane;   // [T][P+1][rank_stride] or null
+  uint32_t rank_stride;
+  bool use_sums;
+};
+
 template <int NT, typename K>
 __global__ void __launch_bounds__(NT, (sizeof(K) == 4 && NT <= 256) ? 1024 / NT : 1)
-diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_out out, bool use_sums,
-                uint8_t* __restrict__ todo) {
+diagnose_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restrict__ todo) {
+  const uint8_t* __restrict__ records = src.records;
+  const bool use_sums = src.use_sums;
   __shared__ SelSmem sm;
   if (sizeof(K) == 8 && !todo[blockIdx.x]) return;
   const int tid = threadIdx.x;
@@ -173,6 +185,8 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
   if (is_sig ? (out.sig_stats == nullptr && out.sig_flags == nullptr && out.rank_score == nullptr)
              : (out.span_stats == nullptr && out.span_flags == nullptr && out.step_anomalous == nullptr))
     return;
+  const unsigned long long* plane = is_sig ? src.sig_plane : src.span_plane;
+  if (records == nullptr && plane == nullptr) return;      // planes mode without this family
 
   // ---- gather x[r] over ranks (a6) ----------------------------------------------------------
   unsigned long long x[EPT];
@@ -183,7 +197,10 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
     const uint32_t r = (uint32_t)(j * NT + tid);
     x[j] = 0ull;
     if (r < R) {
-      if (is_sig && use_sums) {
+      if (plane) {
+        // rank-contiguous plane: one coalesced read per warp
+        x[j] = __ldg(plane + ((size_t)t * (is_sig ? D.S : D.P + 1u) + (is_sig ? f : f - D.S)) * src.rank_stride + r);
+      } else if (is_sig && use_sums) {
         // the sum plane: 8 bytes per rank, neighbouring sigs (other CTAs) share the sector
         x[j] = __ldg(D.sums + ((size_t)r * D.T + t) * D.S + f);
       } else {
@@ -248,29 +265,104 @@ diagnose_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_diag_ou
 
 }  // namespace
 
-cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
-                                  bool use_sums, cudaStream_t s) {
-  const argus_dims& D = ctx->dims;
+static cudaError_t launch_select(argus_ctx* ctx, const DiagSrc& src, const argus_dims& D, const argus_diag_out* o,
+                                 cudaStream_t s) {
   if (o->rank_score) {
     cudaError_t e = cudaMemsetAsync(o->rank_score, 0, (size_t)D.T * D.R * sizeof(uint32_t), s);
     if (e != cudaSuccess) return e;
     ctx->n_memsets += 1;
   }
-  const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);
-  if (blocks > 0x7FFFFFFFull) return cudaErrorInvalidValue;
-  const uint8_t* rec = static_cast<const uint8_t*>(d_records);
+  const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);     // <= the ctx's own series count (checked by callers)
   uint8_t* todo = ctx->d_diag_todo;        // one mark byte per series (workspace)
   const unsigned nb = (unsigned)blocks;
   if (D.R <= 64u * EPT) {
-    diagnose_kernel<64, uint32_t><<<nb, 64, 0, s>>>(rec, D, *o, use_sums, todo);
-    diagnose_kernel<64, unsigned long long><<<nb, 64, 0, s>>>(rec, D, *o, use_sums, todo);
+    diagnose_kernel<64, uint32_t><<<nb, 64, 0, s>>>(src, D, *o, todo);
+    diagnose_kernel<64, unsigned long long><<<nb, 64, 0, s>>>(src, D, *o, todo);
   } else if (D.R <= 256u * EPT) {
-    diagnose_kernel<256, uint32_t><<<nb, 256, 0, s>>>(rec, D, *o, use_sums, todo);
-    diagnose_kernel<256, unsigned long long><<<nb, 256, 0, s>>>(rec, D, *o, use_sums, todo);
+    diagnose_kernel<256, uint32_t><<<nb, 256, 0, s>>>(src, D, *o, todo);
+    diagnose_kernel<256, unsigned long long><<<nb, 256, 0, s>>>(src, D, *o, todo);
   } else {
-    diagnose_kernel<1024, uint32_t><<<nb, 1024, 0, s>>>(rec, D, *o, use_sums, todo);
-    diagnose_kernel<1024, unsigned long long><<<nb, 1024, 0, s>>>(rec, D, *o, use_sums, todo);
+    diagnose_kernel<1024, uint32_t><<<nb, 1024, 0, s>>>(src, D, *o, todo);
+    diagnose_kernel<1024, unsigned long long><<<nb, 1024, 0, s>>>(src, D, *o, todo);
   }
   ctx->n_kernels += 2;
+  return cudaGetLastError();
+}
+
+cudaError_t argus_launch_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* o,
+                                  bool use_sums, cudaStream_t s) {
+  DiagSrc src;
+  src.records = static_cast<const uint8_t*>(d_records);
+  src.sig_plane = nullptr; src.span_plane = nullptr; src.rank_stride = 0; src.use_sums = use_sums;
+  return launch_select(ctx, src, ctx->dims, o, s);
+}
+
+// Series handed in as rank-contiguous planes (a slice of the sigs of a job of pl->n_ranks ranks).
+cudaError_t argus_launch_diagnose_planes(argus_ctx* ctx, const argus_planes* pl, const argus_diag_out* o,
+                                         cudaStream_t s) {
+  DiagSrc src;
+  src.records = nullptr;
+  src.sig_plane = reinterpret_cast<const unsigned long long*>(pl->sig_sums);
+  src.span_plane = reinterpret_cast<const unsigned long long*>(pl->span_ns);
+  src.rank_stride = pl->rank_stride; src.use_sums = false;
+  argus_dims D = ctx->dims;
+  D.R = pl->n_ranks; D.S = pl->n_sigs; D.sums = nullptr;
+  return launch_select(ctx, src, D, o, s);
+}
+
+// ---- plane export of a rank shard (the ONE exchange of a rank-sharded job) ---------------
+namespace {
+
+// dst[((t*ns + (s - s0)) * stride + off + r] = sums[(r*T + t)*S + s]: tiled transpose through shared memory,
+// reads coalesced over sigs, writes coalesced over ranks (rows of R_local u64 — whole lines for a peer).
+__global__ void __launch_bounds__(256)
+pack_sig_plane_kernel(const unsigned long long* __restrict__ sums, argus_dims D, uint32_t s0, uint32_t ns,
+                      unsigned long long* __restrict__ dst, uint32_t stride, uint32_t off) {
+  __shared__ unsigned long long tile[32][33];
+  const uint32_t t = blockIdx.z;
+  const uint32_t sb = blockIdx.x * 32u, rb = blockIdx.y * 32u;
+  const uint32_t tx = threadIdx.x & 31u, ty = threadIdx.x >> 5;      // 32 x 8
+  for (uint32_t i = ty; i < 32u; i += 8u) {
+    const uint32_t r = rb + i, sg = sb + tx;
+    tile[i][tx] = (r < D.R && sg < ns) ? __ldg(sums + ((size_t)r * D.T + t) * D.S + s0 + sg) : 0ull;
+  }
+  __syncthreads();
+  for (uint32_t i = ty; i < 32u; i += 8u) {
+    const uint32_t sg = sb + i, r = rb + tx;
+    if (sg < ns && r < D.R) dst[((size_t)t * ns + sg) * stride + off + r] = tile[tx][i];
+  }
+}
+
+// dst[((t*(P+1) + k) * stride + off + r] = span[r][t][k].span_ns of the finalised records
+__global__ void __launch_bounds__(256)
+pack_span_plane_kernel(const uint8_t* __restrict__ records, argus_dims D, unsigned long long* __restrict__ dst,
+                       uint32_t stride, uint32_t off) {
+  const uint32_t n = D.T * (D.P + 1u) * D.R;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const uint32_t r = i % D.R, tk = i / D.R, k = tk % (D.P + 1u), t = tk / (D.P + 1u);
+    const argus_span* sp = reinterpret_cast<const argus_span*>(records + ((size_t)r * D.T + t) * D.rec_bytes + D.span_off) + k;
+    dst[(size_t)tk * stride + off + r] = sp->span_ns;
+  }
+}
+
+}  // namespace
+
+cudaError_t argus_launch_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t s0, uint32_t s1,
+                                     uint64_t* dst_sig, uint64_t* dst_span, uint32_t stride, uint32_t off,
+                                     cudaStream_t s) {
+  const argus_dims& D = ctx->dims;
+  if (dst_sig && s1 > s0) {
+    const uint32_t ns = s1 - s0;
+    dim3 grid((ns + 31u) / 32u, (D.R + 31u) / 32u, D.T);
+    pack_sig_plane_kernel<<<grid, 256, 0, s>>>(D.sums, D, s0, ns, reinterpret_cast<unsigned long long*>(dst_sig),
+                                               stride, off);
+    ctx->n_kernels += 1;
+  }
+  if (dst_span) {
+    const uint32_t n = D.T * (D.P + 1u) * D.R;
+    pack_span_plane_kernel<<<(n + 255u) / 256u, 256, 0, s>>>(static_cast<const uint8_t*>(d_records), D,
+                                                            reinterpret_cast<unsigned long long*>(dst_span), stride, off);
+    ctx->n_kernels += 1;
+  }
   return cudaGetLastError();
 }

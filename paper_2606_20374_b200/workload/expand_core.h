@@ -58,6 +58,9 @@ typedef struct wl_desc {
   const uint32_t* pareto_q16;  /* [65536] Pareto(alpha) ratio quantiles, Q16 (dur_mode 1)        */
   const wl_fault* faults;      /* [n_faults] sorted by rank                                      */
   const uint32_t* fault_off;   /* [R+1] faults of rank r are faults[fault_off[r]..fault_off[r+1]) */
+  const uint32_t* mode2_q16;   /* [S] 0 = unimodal sig; else the multiplier (Q16) of the sig's SECOND duration
+                                  mode, taken by half of its events (same-name kernels "differ in
+                                  duration by several multiples" across positions) */
 } wl_desc;
 
 WL_HD uint64_t wl_mix(uint64_t x) {            /* splitmix64 finaliser */
@@ -142,6 +145,7 @@ WL_HD void wl_expand_rank(const wl_desc* d, uint32_t rank, wl_event* out, uint64
       uint64_t dur;
       if (d->dur_mode == 0) {
         dur = (d->base_ns[sig] * (uint64_t)d->jit_q16[h & 4095u]) >> 16;
+        if (d->mode2_q16[sig] != 0u && ((h >> 47) & 1u)) dur = (dur * (uint64_t)d->mode2_q16[sig]) >> 16;
       } else {
         uint32_t i1 = (uint32_t)(h >> 24) & 65535u;
         dur = (d->xmin_ns * (uint64_t)d->pareto_q16[i1]) >> 16;

@@ -71,6 +71,8 @@ class Spec:
     seed: int = 0
     step_base: int = 0
     fault_plan: str = ""   # which injected-fault recipe to use
+    bimodal_frac: float = 0.0      # stress knob: this share of the sigs has a second duration mode ...
+    bimodal_ratio: tuple = (8.0, 64.0)   # ... log-uniform in this range times the first, hit by half the events
 
     @property
     def total_events(self) -> int:
@@ -162,11 +164,11 @@ class DescC(ctypes.Structure):
                 ("stream_id", ctypes.c_void_p), ("base_ns", ctypes.c_void_p),
                 ("jit_q16", ctypes.c_void_p), ("gap_ns", ctypes.c_void_p),
                 ("pareto_q16", ctypes.c_void_p), ("faults", ctypes.c_void_p),
-                ("fault_off", ctypes.c_void_p)]
+                ("fault_off", ctypes.c_void_p), ("mode2_q16", ctypes.c_void_p)]
 
 
 _TABLE_NAMES = ["prog_sig", "prog_off", "stream_id", "base_ns", "jit_q16", "gap_ns", "pareto_q16",
-                "faults", "fault_off"]
+                "faults", "fault_off", "mode2_q16"]
 
 
 class Workload:
@@ -223,9 +225,20 @@ class Workload:
             fa[i] = (f.rank, f.step, f.sig, f.sig_class, f.phase, round(f.mult * 65536))
             foff[f.rank + 1:] += 1
 
+        # stress knob (bench.py --bimodal): a second duration mode for a share of the sigs, drawn from
+        # its own generator so that the named workloads keep their bytes
+        mode2 = np.zeros(S, dtype=np.uint32)
+        if spec.bimodal_frac > 0.0:
+            rng2 = np.random.Generator(np.random.PCG64(spec.seed ^ 0x5EED))
+            pick = rng2.random(S) < spec.bimodal_frac
+            lo, hi = spec.bimodal_ratio
+            ratio = np.exp(rng2.uniform(math.log(lo), math.log(hi), size=S))
+            mode2[pick] = np.rint(65536.0 * ratio[pick]).astype(np.uint32)
+        self.n_bimodal = int((mode2 != 0).sum())
+
         self.tables = dict(prog_sig=prog.reshape(-1), prog_off=off.reshape(-1), stream_id=stream_id,
                            base_ns=base, jit_q16=jit, gap_ns=gap, pareto_q16=par, faults=fa,
-                           fault_off=foff)
+                           fault_off=foff, mode2_q16=mode2)
         self._dev_tables = None
         self._host_lib = None
         self._dev_lib = None
