@@ -66,6 +66,7 @@ class ClockSampler(threading.Thread):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
         self._stop_evt = threading.Event()
+        self.ready = threading.Event()       # the first sample has been taken
         self.err = None
 
     def run(self):
@@ -83,9 +84,18 @@ class ClockSampler(threading.Thread):
                 for b, name in self.REASONS.items():
                     if bits & b:
                         self.reasons.add(name)
-                time.sleep(0.02)
+                self.ready.set()
+                time.sleep(0.002)
         except Exception as e:  # NVML missing: report it, do not fail the bench
             self.err = repr(e)
+            self.ready.set()
+
+    def begin(self):
+        """Start sampling; returns once the first sample is in (short timed regions still get clocks)."""
+        self.start()
+        self.ready.wait(timeout=5)
+        self.samples.clear()
+        return self
 
     def stop(self):
         self._stop_evt.set()
@@ -178,6 +188,9 @@ def run_ours(args, world):
     torch.cuda.set_device(world.local_rank)
     dev = world.local_rank
     wl0 = build_workload(args.workload)
+    if args.bimodal > 0.0:
+        wl0 = build_workload(dataclasses.replace(wl0.spec, bimodal_frac=args.bimodal,
+                                                 name=wl0.spec.name + f"+bimodal{args.bimodal:g}"))
     spec = dataclasses.replace(wl0.spec, seed=D.job_seed(wl0.spec.seed, world))
     wl = build_workload(spec) if world.rank else wl0
     s = wl.spec
@@ -207,8 +220,7 @@ def run_ours(args, world):
     torch.cuda.synchronize()
     D.barrier(world)
 
-    sampler = ClockSampler(dev)
-    sampler.start()
+    sampler = ClockSampler(dev).begin()
     mk = lambda: torch.cuda.Event(enable_timing=True)
     t_beg, t_end = mk(), mk()
     marks = [(mk(), mk(), mk()) for _ in range(args.steps)]
@@ -390,6 +402,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = one job of the named size per GPU; strong = ONE job sharded by trace rank")
+    ap.add_argument("--exchange", default="a2a", choices=["a2a", "p2p"],
+                    help="--scaling strong: all_to_all_single (NCCL) or peer stores through symmetric memory")
+    ap.add_argument("--bimodal", type=float, default=0.0,
+                    help="stress knob: share of the sigs with a second duration mode 8-64x the first (PAPER.md:166)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

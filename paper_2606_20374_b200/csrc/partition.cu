@@ -13,13 +13,8 @@
 //   offsets : per key, exclusive running sum over the CTAs (H[cta][key] becomes the CTA's offset
 //             inside the key's group) and the group size total[key]
 //   scan    : exclusive prefix sum of total in place (one CTA, running carry)
-//   scatter : CLUSTERS of 8 CTAs re-read the chunks their CTAs counted; the cluster shares ONE set of
-//             cursors, distributed over its CTAs' shared memory (key & 7 names the owner):
-//             pos = atom.shared::cluster.add(cursor[key], 1); grouped[pos] = event.  A cursor per
-//             CTA would leave #CTAs x #keys write streams open at once (1.2 M partially written
-//             128-byte lines at config 3: more than L2 holds, so lines went to HBM sector by sector
-//             and the scatter ran at a third of the copy bandwidth); per cluster there are 8 x
-//             fewer, which L2 assembles into whole lines.
+//   scatter : the same CTA re-reads its chunk with cursor[key] = total[key] + H[cta][key] in shared
+//             memory: pos = atomicAdd(&cursor[key], 1); grouped[pos] = event (one 256-bit store)
 // When R*T + 1 counters do not fit shared memory, count and scatter use L2 atomics on one global
 // counter array instead (same results, slower).  All buffers are areas of the ctx workspace.
 // Events whose key fields are out of range travel in the last bin, so that the segmented kernel
@@ -116,77 +111,34 @@ partition_count_smem_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t c
   for (uint32_t k = threadIdx.x; k < m; k += blockDim.x) row[k] = s_bins[k];
 }
 
-constexpr uint32_t CL = 8;     // CTAs per cluster of the scatter (the portable maximum)
-
-// B[g][k] := events of key k counted by the CTAs of clusters before g (g = c / CL);  total[k] := all.
-// (written over row g * CL of H: the first row of each cluster becomes the cluster's base offsets)
+// H[c][k] := sum over c' < c of H[c'][k];  total[k] := sum over all c
 __global__ void __launch_bounds__(256)
 partition_offsets_kernel(uint32_t* __restrict__ H, uint32_t n_cta, uint32_t m, uint32_t* __restrict__ total) {
   const uint32_t k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= m) return;
   uint32_t run = 0;
-  for (uint32_t c0 = 0; c0 < n_cta; c0 += CL) {
-    uint32_t v = 0;
-    for (uint32_t c = c0; c < c0 + CL && c < n_cta; ++c) v += H[(size_t)c * m + k];
-    H[(size_t)c0 * m + k] = run;
+  for (uint32_t c = 0; c < n_cta; ++c) {
+    const uint32_t v = H[(size_t)c * m + k];
+    H[(size_t)c * m + k] = run;
     run += v;
   }
   total[k] = run;
 }
 
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-// pos = old value of the cluster-shared cursor at shared-window offset `a` in CTA `owner` of the cluster
-__device__ __forceinline__ uint32_t cluster_cursor_take(uint32_t a, uint32_t owner) {
-  uint32_t ra, old;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(a), "r"(owner));
-  asm volatile("atom.shared::cluster.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(ra) : "memory");
-  return old;
-}
-
-// CTA j of cluster g re-reads chunk g * CL + j (the one count CTA g * CL + j counted); the cursors of
-// keys k with (k & 7) == j live in ITS shared memory: s_bins[k >> 3].
-__global__ void __cluster_dims__(CL, 1, 1) __launch_bounds__(1024)
-partition_scatter_cluster_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t chunk, argus_dims D,
-                                 uint32_t m, const uint32_t* __restrict__ H,
-                                 const uint32_t* __restrict__ start, uint4* __restrict__ grouped) {
-  const uint32_t j = cluster_ctarank();
-  const uint32_t* base = H + (size_t)(blockIdx.x - j) * m;      // row of the cluster's first CTA
-  for (uint32_t k = j + CL * threadIdx.x; k < m; k += CL * blockDim.x) s_bins[k >> 3] = start[k] + base[k];
-  cluster_sync_all();
-  const uint32_t a_bins = (uint32_t)__cvta_generic_to_shared(s_bins);
+__global__ void __launch_bounds__(1024)
+partition_scatter_smem_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t chunk, argus_dims D,
+                              uint32_t m, const uint32_t* __restrict__ H,
+                              const uint32_t* __restrict__ start, uint4* __restrict__ grouped) {
+  const uint32_t* row = H + (size_t)blockIdx.x * m;
+  for (uint32_t k = threadIdx.x; k < m; k += blockDim.x) s_bins[k] = start[k] + row[k];
+  __syncthreads();
   const uint64_t e0 = (uint64_t)blockIdx.x * chunk;
   const uint64_t e1 = e0 + chunk < n ? e0 + chunk : n;
-  constexpr int U = 4;                                         // events in flight per thread
-  uint64_t i = e0 + threadIdx.x;
-  for (; i + (uint64_t)(U - 1) * blockDim.x < e1; i += (uint64_t)U * blockDim.x) {
-    uint4 lo[U], hi[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      lo[u] = __ldcs(ev + 2 * (i + (uint64_t)u * blockDim.x));
-      hi[u] = __ldcs(ev + 2 * (i + (uint64_t)u * blockDim.x) + 1);
-    }
-    uint32_t pos[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-      const uint32_t key = group_key(D, lo[u].x, lo[u].y);
-      pos[u] = cluster_cursor_take(a_bins + (key >> 3) * 4u, key & 7u);
-    }
-#pragma unroll
-    for (int u = 0; u < U; ++u) store_event(grouped + 2 * (size_t)pos[u], lo[u], hi[u]);
-  }
-  for (; i < e1; i += blockDim.x) {
+  for (uint64_t i = e0 + threadIdx.x; i < e1; i += blockDim.x) {
     const uint4 lo = __ldcs(ev + 2 * i), hi = __ldcs(ev + 2 * i + 1);
-    const uint32_t key = group_key(D, lo.x, lo.y);
-    store_event(grouped + 2 * (size_t)cluster_cursor_take(a_bins + (key >> 3) * 4u, key & 7u), lo, hi);
+    const uint32_t pos = atomicAdd(&s_bins[group_key(D, lo.x, lo.y)], 1u);
+    store_event(grouped + 2 * (size_t)pos, lo, hi);
   }
-  cluster_sync_all();            // nobody leaves while a peer may still address its shared memory
 }
 
 }  // namespace
@@ -196,9 +148,7 @@ void argus_partition_plan(const argus_config* cfg, int sm_count, int max_smem_op
                           bool* smem) {
   const size_t bin_bytes = sizeof(uint32_t) * ((size_t)cfg->n_ranks * cfg->n_steps + 1u);
   *smem = bin_bytes <= 200u * 1024u && bin_bytes + 1024u <= (size_t)max_smem_optin;
-  // a multiple of the cluster size: 2 CTAs per SM when two histograms fit (296 = 37 clusters on B200)
-  const uint32_t want = (uint32_t)sm_count * (bin_bytes <= 100u * 1024u ? 2u : 1u);
-  *n_cta = *smem ? (want + CL - 1u) / CL * CL : 0u;
+  *n_cta = *smem ? (uint32_t)sm_count * (bin_bytes <= 100u * 1024u ? 2u : 1u) : 0u;
 }
 
 cudaError_t argus_configure_partition(argus_ctx* ctx) {
@@ -206,6 +156,9 @@ cudaError_t argus_configure_partition(argus_ctx* ctx) {
   const int bin_bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->dims.R * ctx->dims.T + 1u));
   cudaError_t e = cudaFuncSetAttribute(partition_count_smem_kernel,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize, bin_bytes);
+  if (e == cudaSuccess)
+    e = cudaFuncSetAttribute(partition_scatter_smem_kernel,
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, bin_bytes);
   return e;
 }
 
@@ -221,14 +174,12 @@ cudaError_t argus_launch_partition(argus_ctx* ctx, const argus_event* ev, uint64
     uint64_t chunk = (n + n_cta - 1) / n_cta;
     chunk = (chunk + 1023) / 1024 * 1024;
     n_cta = (uint32_t)((n + chunk - 1) / chunk);
-    const uint32_t n_cta_cl = (n_cta + CL - 1u) / CL * CL;    // whole clusters (CTAs past the data only sync)
     uint32_t* H = ctx->d_part;
     partition_count_smem_kernel<<<n_cta, 1024, bin_bytes, s>>>(src, n, chunk, D, m, H);
     partition_offsets_kernel<<<(m + 255u) / 256u, 256, 0, s>>>(H, n_cta, m, ctx->d_hist);
     partition_scan_kernel<<<1, 1024, 0, s>>>(ctx->d_hist, m);
-    const size_t cur_bytes = sizeof(uint32_t) * ((size_t)(m + CL - 1u) / CL);
-    partition_scatter_cluster_kernel<<<n_cta_cl, 1024, cur_bytes, s>>>(src, n, chunk, D, m, H, ctx->d_hist,
-                                                                       reinterpret_cast<uint4*>(ctx->d_group));
+    partition_scatter_smem_kernel<<<n_cta, 1024, bin_bytes, s>>>(src, n, chunk, D, m, H, ctx->d_hist,
+                                                                 reinterpret_cast<uint4*>(ctx->d_group));
     ctx->n_kernels += 4;
     return cudaGetLastError();
   }

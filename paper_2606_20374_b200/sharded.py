@@ -262,8 +262,7 @@ def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
         step()
     torch.cuda.synchronize()
     D.barrier(world)
-    sampler = ClockSampler(dev)
-    sampler.start()
+    sampler = ClockSampler(dev).begin()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record()
     for _ in range(args.steps):
