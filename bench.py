@@ -198,7 +198,8 @@ def run_ours(args, world):
 
     d_ev = wl.expand_device(device=f"cuda:{dev}")
     ctx = A.Argus(s.n_ranks, s.n_steps, s.n_sigs, s.n_phases, s.step_base, sorted_hint=not s.shuffle,
-                  device=dev, max_ungrouped_events=n if s.shuffle else 0)
+                  device=dev, max_ungrouped_events=n if s.shuffle else 0,
+                  max_spill_events=min(n // 4, 2**32 - 1) if args.spill < 0 else args.spill)
     rec = ctx.alloc_records()
     outs = ctx.alloc_diag()
     torch.cuda.synchronize()
@@ -241,6 +242,7 @@ def run_ours(args, world):
     # per-step durations (reset of step i+1 is two tiny memsets: attributed to the step they precede)
     step_list = [marks[i][0].elapsed_time(marks[i][2]) for i in range(args.steps)]
     n_valid, n_invalid = ctx.stats()
+    n_requeued, n_overflow = ctx.refused_count()
     total_events = D.sum_over_ranks(world, float(n))
     value = total_events / (ms_step * 1e-3)
     resident = {k: v.clone() for k, v in outs.items()}
@@ -351,8 +353,14 @@ def run_ours(args, world):
                      "algorithmic_bytes": alg_bytes, "share_of_step": agg_ms / ms_step},
         "clocks": clocks, "e2e": e2e,
         "gpu_launches": k1 - k0, "gpu_memsets": m1 - m0,     # counted by the library (argus_launch_count)
-        "counters": {"n_valid": n_valid, "n_invalid": n_invalid},
+        # events a compact shared-memory cell refused (range wider than four log2 buckets, >= 2^32 ns), per step:
+        # re-queued through the spill area and a second launch / taken one by one by L2 reductions
+        "counters": {"n_valid": n_valid, "n_invalid": n_invalid, "n_requeued": n_requeued,
+                     "n_overflow": n_overflow, "requeued_frac": n_requeued / max(1, n_valid),
+                     "overflow_frac": n_overflow / max(1, n_valid)},
     }
+    if args.bimodal > 0.0:
+        out["config"]["bimodal_sigs"] = wl.n_bimodal
     if world.size == 1 and not args.no_cpu_baseline:
         k = args.cpu_baseline_ranks if args.cpu_baseline_ranks > 0 else s.n_ranks
         if args.cpu_baseline_ranks < 0:      # default: a bounded sample, about 15 s of oracle time
@@ -406,6 +414,8 @@ def main():
                     help="--scaling strong: all_to_all_single (NCCL) or peer stores through symmetric memory")
     ap.add_argument("--bimodal", type=float, default=0.0,
                     help="stress knob: share of the sigs with a second duration mode 8-64x the first (PAPER.md:166)")
+    ap.add_argument("--spill", type=int, default=-1,
+                    help="argus_config.max_spill_events: -1 = a quarter of the events (default), 0 = no spill area")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")

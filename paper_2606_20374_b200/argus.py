@@ -33,7 +33,7 @@ HEADER_DTYPE = np.dtype([("magic", "<u4"), ("version", "<u2"), ("n_phases", "<u2
 EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes",
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
            "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
-           "argus_diagnose_planes", "argus_stats",
+           "argus_diagnose_planes", "argus_stats", "argus_refused_count",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
 
@@ -42,7 +42,8 @@ class ArgusConfig(ctypes.Structure):
     _fields_ = [("n_ranks", ctypes.c_uint32), ("n_steps", ctypes.c_uint32),
                 ("n_sigs", ctypes.c_uint32), ("n_phases", ctypes.c_uint32),
                 ("step_base", ctypes.c_uint32), ("flags", ctypes.c_uint32),
-                ("device", ctypes.c_int32), ("max_ungrouped_events", ctypes.c_uint32)]
+                ("device", ctypes.c_int32), ("max_ungrouped_events", ctypes.c_uint32),
+                ("max_spill_events", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
 
 
 class ArgusDiagOut(ctypes.Structure):
@@ -103,6 +104,8 @@ def load() -> ctypes.CDLL:
     lib.argus_diagnose_planes.argtypes = [vp, ctypes.POINTER(ArgusPlanes), ctypes.POINTER(ArgusDiagOut), vp]
     lib.argus_stats.restype = i32
     lib.argus_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    lib.argus_refused_count.restype = i32
+    lib.argus_refused_count.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_launch_count.restype = i32
     lib.argus_launch_count.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_tune.restype = i32
@@ -144,12 +147,13 @@ class Argus:
 
     def __init__(self, n_ranks: int, n_steps: int, n_sigs: int, n_phases: int, step_base: int = 0,
                  sorted_hint: bool = True, device: int = 0, max_ungrouped_events: int = 0,
-                 workspace="torch"):
+                 max_spill_events: int = 0, workspace="torch"):
         """workspace: "torch" = a caller-owned torch uint8 tensor of argus_workspace_bytes (kept in
         self.workspace); None = the library allocates it itself in argus_create; or a tensor."""
         self.lib = load()
         self.cfg = ArgusConfig(n_ranks, n_steps, n_sigs, n_phases, step_base,
-                               FLAG_SORTED if sorted_hint else 0, device, max_ungrouped_events)
+                               FLAG_SORTED if sorted_hint else 0, device, max_ungrouped_events,
+                               max_spill_events, 0)
         self.R, self.T, self.S, self.P = n_ranks, n_steps, n_sigs, n_phases
         self.device = device
         self.workspace = None
@@ -260,6 +264,12 @@ class Argus:
     def stats(self):
         a, b = ctypes.c_uint64(), ctypes.c_uint64()
         self._check(self.lib.argus_stats(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return int(a.value), int(b.value)
+
+    def refused_count(self):
+        """(re-queued through the spill area, taken by the overflow list / L2 atomics)"""
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self.lib.argus_refused_count(self._h, ctypes.byref(a), ctypes.byref(b)))
         return int(a.value), int(b.value)
 
     def launch_count(self):

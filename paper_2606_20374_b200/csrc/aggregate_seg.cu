@@ -19,9 +19,14 @@
 // invariant; an event that would extend the range goes through a 64-bit CAS that refuses the
 // extension when the invariant would break.  Only native 32-bit shared atomics are used on the
 // hot path (64-bit shared atomic adds are CAS loops on sm_100a).
-// An event the compact cell cannot take (duration >= 2^32 ns, or a range wider than four buckets)
-// is parked in the CTA's overflow list (global memory, workspace) and applied to the record with L2
-// reductions at the flush; when the record is already live it goes there at once.  When the
+// An event the compact cell cannot take (a range wider than four buckets: the second mode of a kernel
+// whose durations "differ by several multiples" between positions) is RE-QUEUED: the lane
+// appends the raw event to its CTA's region of a spill buffer (workspace) and goes on; a second launch
+// of this same kernel (REQUEUE: cells only, spans and counters were taken the first time) folds every
+// CTA's region, where the sig's remaining events now find the cell empty and open a window of their
+// own.  What that launch still refuses, events of 2^32 ns or more, and everything when the spill area
+// is absent or full, is parked in the CTA's overflow list (global memory, workspace) and applied to the
+// record with L2 reductions at the flush; when the record is already live it goes there at once.  When the
 // (rank, step) key changes the table is flushed: the first CTA to reach a record claims it and
 // writes the whole 160-byte cells with coalesced 128-bit stores (no read-modify-write, no separate
 // identity fill); any later contribution to the same record merges with L2 reductions.  Correct
@@ -55,6 +60,8 @@ struct Hdr {
   uint32_t mode;                      // claim on the current key's record: LAZY = ours to write, LIVE, BUSY = another CTA's
   uint32_t n_finished;                // consumer warps that ran out of events
   uint32_t ovf_n;                     // events parked in this CTA's overflow list since the last flush
+  uint32_t spill_n;                   // events this CTA re-queued into its spill region
+  uint32_t n_refused;                 // events that took the overflow list or L2 atomics
 };
 constexpr uint32_t OVF_CAP = ARGUS_OVF_CAP;   // entries of a CTA's overflow list (16 bytes each, workspace)
 constexpr unsigned long long NEXT_NONE = ~0ull;
@@ -457,11 +464,14 @@ __host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes
 
 // CW consumer warps + 1 producer warp; a stage = WPSTG warps' worth of events (WPSTG KB); the table
 // layout is compiled for SCAP sigs (S <= SCAP), so every table address is base + sig * c + constant.
-template <int CW, int WPSTG, uint32_t SCAP, int MINB>
+// REQUEUE = the second launch: CTA i folds the spill_cnt[i] events the first launch's CTA i re-queued into
+// region i of the spill buffer (ev), cells only.
+template <int CW, int WPSTG, uint32_t SCAP, int MINB, bool REQUEUE>
 __global__ void __launch_bounds__((CW + 1) * 32, MINB)
 aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __restrict__ ev, uint64_t n,
                      uint64_t per_cta, uint8_t* records, uint32_t* state, unsigned long long* counters,
-                     uint4* ovf, argus_dims D) {
+                     uint4* ovf, argus_dims D, uint4* __restrict__ spill, uint32_t* __restrict__ spill_cnt,
+                     uint32_t spill_cap) {
   constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG, MINB);
   static_assert(K >= 2 * (CW / WPSTG), "ring too shallow for this geometry");
   constexpr int NC = CW * 32;            // consumer threads
@@ -479,7 +489,8 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   const uint64_t e0 = (uint64_t)blockIdx.x * per_cta;
   if (e0 >= n) return;
   const uint64_t e1 = (e0 + per_cta < n) ? e0 + per_cta : n;
-  const uint32_t n_ev = (uint32_t)(e1 - e0);
+  const uint32_t n_ev = REQUEUE ? spill_cnt[blockIdx.x] : (uint32_t)(e1 - e0);
+  if (REQUEUE && n_ev == 0u) return;
   const uint32_t n_sub = (n_ev + SUBE - 1) / SUBE;
   const uint32_t n_iter = (n_ev + NC - 1) / NC;
 
@@ -488,7 +499,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       mbar_init(smem_u32(&H->full[k]), 1u);
       mbar_init(smem_u32(&H->empty[k]), (uint32_t)WPSTG);
     }
-    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u; H->ovf_n = 0u;
+    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u; H->ovf_n = 0u; H->spill_n = 0u; H->n_refused = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   {
@@ -592,6 +603,22 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     }                                                                                    \
   } while (0)
 
+  // A refused event of the current key (d < 2^32) is appended, as a raw 32-byte record rebuilt from the
+  // decoded fields (the stream id is not part of the method and is dropped), to this CTA's spill region.
+  uint4* const my_spill = spill + 2 * (size_t)blockIdx.x * spill_cap;
+#define ARGUS_SPILL(okv)                                                                              \
+  do {                                                                                               \
+    if (!REQUEUE && spill_cap != 0u) {                                                               \
+      const uint32_t sp_ = atomicAdd(&H->spill_n, 1u);                                               \
+      if (sp_ < spill_cap) {                                                                         \
+        my_spill[2 * (size_t)sp_] = make_uint4(cur_rank, cur_step, sig, phase << 16);                \
+        my_spill[2 * (size_t)sp_ + 1] = make_uint4((uint32_t)start, (uint32_t)((unsigned long long)start >> 32), \
+                                                   (uint32_t)end, (uint32_t)((unsigned long long)end >> 32));   \
+        okv = true;                                                                                  \
+      }                                                                                              \
+    }                                                                                                \
+  } while (0)
+
   const uint32_t n_full = n_ev / (uint32_t)NC;   // iterations in which every lane of every warp has an event
   // One iteration of a consumer warp.  TAIL = the ragged last iteration (stage or lanes may be missing).
   auto body = [&](auto tail_c) {
@@ -654,7 +681,10 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     if (all_fast) {
       // ---- hot path: the whole warp folds into the current table -------------------------------------
       ARGUS_COMPACT_ADD(ok);
-      if (__all_sync(FULL, ok && phase == ws.phase)) {
+      if (!ok) ARGUS_SPILL(ok);
+      if (REQUEUE) {
+        if (__all_sync(FULL, ok)) return;  // cells only
+      } else if (__all_sync(FULL, ok && phase == ws.phase)) {
         ws.mn = start < ws.mn ? start : ws.mn;
         ws.mx = end > ws.mx ? end : ws.mx;
         ws.n += 32u;                       // warp-uniform count
@@ -664,7 +694,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     } else {
       // full validity (R2, R3) of the lanes that failed the fast test
       pending = mine && argus_event_key(D, lo.x, lo.y, sig, phase, start, end, key);
-      n_invalid += (mine && !pending) ? 1u : 0u;
+      n_invalid += (!REQUEUE && mine && !pending) ? 1u : 0u;
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
 
@@ -673,7 +703,10 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       // ---- cells -----------------------------------------------------------------------------------
       if (!tried) {
         ok = false;
-        if (fast) ARGUS_COMPACT_ADD(ok);
+        if (fast) {
+          ARGUS_COMPACT_ADD(ok);
+          if (!ok) ARGUS_SPILL(ok);
+        }
       }
       tried = false;
       if (!ok && pending && key == cur_key) {
@@ -681,11 +714,13 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
         // overflow list (applied at the flush); a full list asks for a live record at the rendezvous
         if (live) {
           global_cell_add(records, D, cur_key, sig, d);
+          atomicAdd(&H->n_refused, 1u);
           ok = true;
         } else {
           const uint32_t oi = atomicAdd(&H->ovf_n, 1u);
           if (oi < OVF_CAP) {
             gl.ovf[oi] = make_uint4(sig, 0u, d32, (uint32_t)(d >> 32));
+            atomicAdd(&H->n_refused, 1u);
             ok = true;
           }
         }
@@ -694,7 +729,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       // registers; a warp with mixed phases (ungrouped or boundary input) updates the shared
       // accumulators lane by lane: test min/max with a plain load first (they rarely improve after
       // the first few events), count with a 32-bit add (a CTA's span holds < 2^26 events: no carry).
-      {
+      if (!REQUEUE) {
         const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
         if (__all_sync(FULL, ok && phase == ph0)) {
           if (ph0 != ws.phase) { ws.flush(lane); ws.phase = ph0; }
@@ -720,6 +755,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   for (uint32_t it = 0; it < n_full; ++it) body(std::false_type{});
   if (n_iter > n_full) { s = grp + n_full * (uint32_t)SPI; body(std::true_type{}); }
 #undef ARGUS_COMPACT_ADD
+#undef ARGUS_SPILL
   // ---- out of events: keep joining the rendezvous until every warp is done ---------------------------
   ws.flush(lane);
   if (lane == 0) atomicAdd(&H->n_finished, 1u);
@@ -732,7 +768,20 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
 
   n_invalid = __reduce_add_sync(FULL, n_invalid);
   if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
-  if (tid == 0) atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
+  if (tid == 0) {
+    // H->* are final: every warp has passed the last rendezvous
+    if (!REQUEUE) {
+      atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
+      if (spill_cap != 0u) {
+        uint32_t ns = *reinterpret_cast<volatile uint32_t*>(&H->spill_n);
+        ns = ns < spill_cap ? ns : spill_cap;
+        spill_cnt[blockIdx.x] = ns;
+        if (ns) atomicAdd(&counters[3], (unsigned long long)ns);
+      }
+    }
+    const uint32_t nr = *reinterpret_cast<volatile uint32_t*>(&H->n_refused);
+    if (nr) atomicAdd(&counters[2], (unsigned long long)nr);
+  }
 }
 
 // shared-memory bytes of one geometry
@@ -745,9 +794,34 @@ constexpr size_t geom_smem() {
 template <int CW, int WPSTG, uint32_t SCAP, int MINB>
 cudaError_t configure_cap() {
   static_assert(geom_smem<CW, WPSTG, SCAP, MINB>() <= smem_budget(MINB), "shared memory");
-  return cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB>,
+  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, false>,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)geom_smem<CW, WPSTG, SCAP, MINB>());
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, true>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize,
                               (int)geom_smem<CW, WPSTG, SCAP, MINB>());
+}
+
+// the events at `base` as a 2-D tensor of whole 128-byte rows (4 events), loaded a stage (box_rows rows) at a
+// time with the 128-byte shared-memory swizzle
+static cudaError_t encode_events(argus_ctx* ctx, const void* base, uint64_t rows, uint32_t box_rows, CUtensorMap* tmap) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
+                                CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                CUtensorMapFloatOOBfill);
+  const encode_fn encode = reinterpret_cast<encode_fn>(ctx->fn_tmap_encode);
+  if (!encode) return cudaErrorNotSupported;
+  const cuuint64_t dims[2] = {32u, rows ? rows : 1u};          // u32 elements per row, rows
+  const cuuint64_t strides[1] = {128u};                        // bytes between rows
+  const cuuint32_t box[2] = {32u, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1u, 1u};
+  // rows == 0: the map is never used (the producer only arrives), but it must still encode; point
+  // it at the buffer with a single row that is never fetched
+  const CUresult r = encode(tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2u, const_cast<void*>(base), dims,
+                            strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
 template <int CW, int WPSTG, uint32_t SCAP, int MINB>
@@ -762,32 +836,28 @@ cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* 
   if (per_cta > cap) per_cta = cap;
   per_cta = (per_cta + tile - 1) / tile * tile;
   const uint64_t ctas = (n + per_cta - 1) / per_cta;     // <= max(grid, 2^32 / 2^26 + 1) <= ARGUS_MAX_SEG_CTAS
-  // the events as a 2-D tensor of whole 128-byte rows (4 events), loaded a stage (WPSTG * 8 rows) at a
-  // time with the 128-byte shared-memory swizzle; the last n % 4 events are read by the consumers
+  // the last n % 4 events are not part of the tensor: the consumers read them directly
   CUtensorMap tmap;
-  {
-    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-    const encode_fn encode = reinterpret_cast<encode_fn>(ctx->fn_tmap_encode);
-    if (!encode) return cudaErrorNotSupported;
-    const uint64_t rows = n >> 2;
-    const cuuint64_t dims[2] = {32u, rows ? rows : 1u};          // u32 elements per row, rows
-    const cuuint64_t strides[1] = {128u};                        // bytes between rows
-    const cuuint32_t box[2] = {32u, (cuuint32_t)(WPSTG * 8)};
-    const cuuint32_t estr[2] = {1u, 1u};
-    // rows == 0: the map is never used (the producer only arrives), but it must still encode; point
-    // it at the buffer with a single row that is never fetched
-    const CUresult r = encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2u, const_cast<argus_event*>(ev), dims,
-                              strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) return cudaErrorInvalidValue;
-  }
-  aggregate_seg_kernel<CW, WPSTG, SCAP, MINB><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
+  cudaError_t e = encode_events(ctx, ev, n >> 2, (uint32_t)(WPSTG * 8), &tmap);
+  if (e != cudaSuccess) return e;
+  // spill regions: one per CTA, whole 128-byte rows (0: refused events go to the overflow lists)
+  uint64_t scap = ctx->d_spill ? ((uint64_t)ctx->cfg.max_spill_events / ctas) & ~3ull : 0u;
+  if (scap > per_cta) scap = per_cta;
+  uint4* spill = reinterpret_cast<uint4*>(ctx->d_spill);
+  aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, false><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       tmap, reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
-      ctx->d_counters, ctx->d_ovf, ctx->dims);
+      ctx->d_counters, ctx->d_ovf, ctx->dims, spill, ctx->d_spill_cnt, (uint32_t)scap);
   ctx->n_kernels += 1;
+  if (scap != 0u) {
+    // second launch: every CTA folds what its twin re-queued (most CTAs find nothing and leave at once)
+    CUtensorMap tmap2;
+    e = encode_events(ctx, spill, (ctas * scap) >> 2, (uint32_t)(WPSTG * 8), &tmap2);
+    if (e != cudaSuccess) return e;
+    aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, true><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
+        tmap2, spill, ctas * scap, scap, static_cast<uint8_t*>(d_records), ctx->d_state, ctx->d_counters,
+        ctx->d_ovf, ctx->dims, nullptr, ctx->d_spill_cnt, 0u);
+    ctx->n_kernels += 1;
+  }
   return cudaGetLastError();
 }
 

@@ -48,7 +48,7 @@ void argus_ws_plan(const argus_config* c, int sm_count, int max_smem_optin, argu
   const size_t RT = (size_t)c->n_ranks * c->n_steps;
   size_t o = 0;
   L->state = o;     o += up256(sizeof(uint32_t) * RT);
-  L->counters = o;  o += up256(2 * sizeof(unsigned long long));
+  L->counters = o;  o += up256(4 * sizeof(unsigned long long));
   L->hist = o;      o += up256(sizeof(uint32_t) * (RT + 1u));
   L->sums = o;      o += up256(sizeof(unsigned long long) * RT * c->n_sigs);
   L->ovf = o;       o += up256((size_t)ARGUS_MAX_SEG_CTAS * ARGUS_OVF_CAP * sizeof(uint4));
@@ -59,6 +59,12 @@ void argus_ws_plan(const argus_config* c, int sm_count, int max_smem_optin, argu
     if (L->part_smem) o += up256(sizeof(uint32_t) * (size_t)L->part_ctas * (RT + 1u));
     L->group = o;
     o += up256((size_t)c->max_ungrouped_events * sizeof(argus_event));
+  }
+  L->spill_cnt = o; L->spill = o;
+  if (c->max_spill_events) {
+    o += up256(sizeof(uint32_t) * ARGUS_MAX_SEG_CTAS);
+    L->spill = o;
+    o += up256((size_t)c->max_spill_events * sizeof(argus_event));
   }
   L->total = o;
 }
@@ -117,6 +123,10 @@ extern "C" int argus_create(const argus_config* cfg, void* d_workspace, size_t w
     D.sums = reinterpret_cast<unsigned long long*>(ctx->d_ws + L.sums);
     ctx->d_ovf = reinterpret_cast<uint4*>(ctx->d_ws + L.ovf);
     ctx->d_diag_todo = ctx->d_ws + L.diag_todo;
+    if (cfg->max_spill_events) {
+      ctx->d_spill_cnt = reinterpret_cast<uint32_t*>(ctx->d_ws + L.spill_cnt);
+      ctx->d_spill = ctx->d_ws + L.spill;
+    }
     if (cfg->max_ungrouped_events) {
       ctx->d_part = L.part_smem ? reinterpret_cast<uint32_t*>(ctx->d_ws + L.part) : nullptr;
       ctx->d_group = reinterpret_cast<argus_event*>(ctx->d_ws + L.group);
@@ -182,9 +192,9 @@ extern "C" int argus_reset(argus_ctx* ctx, void* d_records, void* stream) {
   CU(ctx, cudaSetDevice(ctx->cfg.device));
   int rc = note_stream(ctx, s);
   if (rc != ARGUS_OK) return rc;
-  CU(ctx, cudaMemsetAsync(ctx->d_state, 0, sizeof(uint32_t) * (size_t)ctx->dims.R * ctx->dims.T, s));
-  CU(ctx, cudaMemsetAsync(ctx->d_counters, 0, 2 * sizeof(unsigned long long), s));
-  ctx->n_memsets += 2;
+  // state words and counters are neighbours in the workspace: one memset
+  CU(ctx, cudaMemsetAsync(ctx->d_state, 0, ctx->ws.hist - ctx->ws.state, s));
+  ctx->n_memsets += 1;
   ctx->d_records = d_records;
   ctx->finalized = false;
   return ARGUS_OK;
@@ -383,6 +393,17 @@ extern "C" int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invali
   h[0] -= h[1];  // kernels count events seen and events rejected
   if (n_valid) *n_valid = h[0];
   if (n_invalid) *n_invalid = h[1];
+  return ARGUS_OK;
+}
+
+extern "C" int argus_refused_count(argus_ctx* ctx, uint64_t* n_requeued, uint64_t* n_overflow) {
+  if (!ctx) return ARGUS_EINVAL;
+  int rc = argus_stats(ctx, nullptr, nullptr);      // synchronises the streams
+  if (rc != ARGUS_OK) return rc;
+  unsigned long long h[2] = {0, 0};
+  CU(ctx, cudaMemcpy(h, ctx->d_counters + 2, sizeof h, cudaMemcpyDeviceToHost));
+  if (n_overflow) *n_overflow = h[0];
+  if (n_requeued) *n_requeued = h[1];
   return ARGUS_OK;
 }
 

@@ -30,7 +30,7 @@ struct argus_dims {
 #define ARGUS_MAX_SEG_CTAS 1024u      // CTAs of one segmented launch (bounds the overflow-list area)
 #define ARGUS_OVF_CAP 4096u           // entries (16 B) of one CTA's overflow list
 struct argus_ws_layout {
-  size_t state, counters, hist, sums, ovf, diag_todo, part, group, total;
+  size_t state, counters, hist, sums, ovf, diag_todo, part, group, spill_cnt, spill, total;
   uint32_t part_ctas;                 // CTAs of the grouping pass (0: no grouping area)
   bool part_smem;                     // its key histograms fit shared memory
 };
@@ -45,12 +45,14 @@ struct argus_ctx {
   uint8_t* d_ws;              // the workspace (caller's, or ours when ws_owned)
   bool ws_owned;
   uint32_t* d_state;          // [R*T]
-  unsigned long long* d_counters;  // [2] events seen, events rejected
+  unsigned long long* d_counters;  // [4] events seen, rejected, taken by the overflow list / L2 atomics, re-queued
   uint32_t* d_hist;           // [R*T + 1] group sizes / cursors of the grouping pass
   argus_event* d_group;       // grouping area [cfg.max_ungrouped_events] (null when 0)
   void* fn_tmap_encode;       // cuTensorMapEncodeTiled, resolved through the runtime (no libcuda link)
   uint32_t* d_part;           // per-CTA key histograms of the grouping pass [part_ctas][R*T + 1]
   uint8_t* d_diag_todo;       // argus_diagnose: one byte per series, set by the 32-bit pass for the 64-bit pass
+  uint8_t* d_spill;           // spill regions of the segmented kernel [cfg.max_spill_events] raw events (null when 0)
+  uint32_t* d_spill_cnt;      // events re-queued by each CTA of the last segmented launch [ARGUS_MAX_SEG_CTAS]
   uint4* d_ovf;               // per-CTA overflow lists of the segmented kernel [ARGUS_MAX_SEG_CTAS][ARGUS_OVF_CAP]
   void* d_records;            // table given to the last argus_reset
   cudaEvent_t ingest_event;   // recorded after every argus_ingest copy

@@ -171,15 +171,13 @@ struct DiagSrc {
 };
 
 template <int NT, typename K>
-__global__ void __launch_bounds__(NT, (sizeof(K) == 4 && NT <= 256) ? 1024 / NT : 1)
-diagnose_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restrict__ todo) {
+__device__ __forceinline__ void diagnose_series(const DiagSrc& src, const argus_dims& D, const argus_diag_out& out,
+                                                uint8_t* __restrict__ todo, uint32_t series_id, SelSmem& sm) {
   const uint8_t* __restrict__ records = src.records;
   const bool use_sums = src.use_sums;
-  __shared__ SelSmem sm;
-  if (sizeof(K) == 8 && !todo[blockIdx.x]) return;
   const int tid = threadIdx.x;
   const uint32_t F = D.S + D.P + 1u;
-  const uint32_t t = blockIdx.x / F, f = blockIdx.x % F;
+  const uint32_t t = series_id / F, f = series_id % F;
   const bool is_sig = f < D.S;
   const uint32_t R = D.R;
   if (is_sig ? (out.sig_stats == nullptr && out.sig_flags == nullptr && out.rank_score == nullptr)
@@ -221,7 +219,7 @@ diagnose_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restri
       if ((uint32_t)(j * NT + tid) < R) { xmn = x[j] < xmn ? x[j] : xmn; xmx = x[j] > xmx ? x[j] : xmx; }
     block_minmax<NT, unsigned long long>(xmn, xmx, sm, xmn, xmx);
     const bool wide = xmx - xmn > 0xFFFFFFFFull;
-    if (tid == 0) todo[blockIdx.x] = wide ? 1 : 0;
+    if (tid == 0) todo[series_id] = wide ? 1 : 0;
     if (wide) return;
     base = xmn;
   }
@@ -263,6 +261,198 @@ diagnose_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restri
   }
 }
 
+template <int NT, typename K>
+__global__ void __launch_bounds__(NT, (sizeof(K) == 4 && NT <= 256) ? 1024 / NT : 1)
+diagnose_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restrict__ todo, uint32_t n_series) {
+  __shared__ SelSmem sm;
+  // K = 32 bit: one CTA per series.  K = 64 bit: a few CTAs walk the (few) marked series.
+  for (uint32_t b = blockIdx.x; b < n_series; b += gridDim.x) {
+    if (sizeof(K) == 8 && !todo[b]) continue;
+    __syncthreads();                       // the previous series is done with sm
+    diagnose_series<NT, K>(src, D, out, todo, b, sm);
+  }
+}
+
+
+// ---- R <= 1024: one WARP per series ----------------------------------------------------------------
+// The block kernel above spends its time in block barriers (about ten radix passes of three barriers
+// per selection, two selections per series) while a series of a few hundred ranks is 8 values per
+// lane: here each warp owns a series, its digit histogram sits in 1 KB of shared memory of its own,
+// and the only synchronisation is __syncwarp.  Series whose values span 2^32 or more are marked for the
+// 64-bit pass (as in the block kernel).
+template <int VPL>
+__device__ __forceinline__ uint32_t warp_select(const uint32_t (&v)[VPL], uint32_t R, uint32_t k, uint32_t* hist) {
+  const int lane = threadIdx.x & 31;
+  uint32_t mn = 0xFFFFFFFFu, mx = 0u;
+#pragma unroll
+  for (int j = 0; j < VPL; ++j)
+    if ((uint32_t)(j * 32 + lane) < R) { mn = v[j] < mn ? v[j] : mn; mx = v[j] > mx ? v[j] : mx; }
+  mn = __reduce_min_sync(FULL, mn);
+  mx = __reduce_max_sync(FULL, mx);
+  if (mn == mx) return mn;
+  const int top = 31 - __clz((int)(mn ^ mx));
+  uint32_t prefix = top == 31 ? 0u : ((mn >> (top + 1)) << (top + 1));
+  uint32_t pmask = top == 31 ? 0u : (0xFFFFFFFFu << (top + 1));
+  int hi_bit = top;
+  for (;;) {
+    const int shift = hi_bit >= 7 ? hi_bit - 7 : 0;
+    const uint32_t dmask = (1u << (hi_bit - shift + 1)) - 1u;
+    __syncwarp();
+#pragma unroll
+    for (int i = 0; i < 8; ++i) hist[lane * 8 + i] = 0u;
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < VPL; ++j)
+      if ((uint32_t)(j * 32 + lane) < R && (v[j] & pmask) == prefix) atomicAdd(&hist[(v[j] >> shift) & dmask], 1u);
+    __syncwarp();
+    uint32_t c[8], sum = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { c[i] = hist[lane * 8 + i]; sum += c[i]; }
+    uint32_t inc = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(FULL, inc, o);
+      if (lane >= o) inc += t;
+    }
+    uint32_t before = inc - sum;
+    const bool here = k >= before && k < inc;          // exactly one lane
+    uint32_t digit = 0, dbefore = 0, dcount = 0;
+    if (here) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        if (k >= before && k < before + c[i]) { digit = (uint32_t)(lane * 8 + i); dbefore = before; dcount = c[i]; }
+        before += c[i];
+      }
+    }
+    const int src = __ffs((int)__ballot_sync(FULL, here)) - 1;
+    digit = __shfl_sync(FULL, digit, src);
+    dbefore = __shfl_sync(FULL, dbefore, src);
+    dcount = __shfl_sync(FULL, dcount, src);
+    k -= dbefore;
+    prefix |= digit << shift;
+    pmask |= dmask << shift;
+    if (shift == 0) return prefix;
+    if (dcount == 1u) {
+      uint32_t val = 0;
+      bool mine = false;
+#pragma unroll
+      for (int j = 0; j < VPL; ++j)
+        if ((uint32_t)(j * 32 + lane) < R && (v[j] & pmask) == prefix) { val = v[j]; mine = true; }
+      return __shfl_sync(FULL, val, __ffs((int)__ballot_sync(FULL, mine)) - 1);
+    }
+    hi_bit = shift - 1;
+  }
+}
+
+template <int VPL>
+__device__ __forceinline__ uint32_t warp_median(const uint32_t (&v)[VPL], uint32_t R, uint32_t* hist) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t k = (R - 1) / 2;
+  const uint32_t lo = warp_select<VPL>(v, R, k, hist);
+  if (R & 1u) return lo;
+  uint32_t le = 0, gt_min = 0xFFFFFFFFu;
+#pragma unroll
+  for (int j = 0; j < VPL; ++j)
+    if ((uint32_t)(j * 32 + lane) < R) {
+      if (v[j] <= lo) ++le;
+      else gt_min = v[j] < gt_min ? v[j] : gt_min;
+    }
+  le = __reduce_add_sync(FULL, le);
+  gt_min = __reduce_min_sync(FULL, gt_min);
+  const uint32_t hi = le >= k + 2u ? lo : gt_min;     // R10: hi = v[R/2]
+  return lo + (hi - lo) / 2u;
+}
+
+template <int VPL>
+__global__ void __launch_bounds__(256)
+diagnose_warp_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restrict__ todo, uint32_t n_series) {
+  __shared__ uint32_t s_hist[8][256];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t series_id = blockIdx.x * 8u + (uint32_t)w;
+  if (series_id >= n_series) return;
+  uint32_t* hist = s_hist[w];
+  const uint32_t F = D.S + D.P + 1u;
+  const uint32_t t = series_id / F, f = series_id % F;
+  const bool is_sig = f < D.S;
+  const uint32_t R = D.R;
+  if (lane == 0) todo[series_id] = 0;
+  if (is_sig ? (out.sig_stats == nullptr && out.sig_flags == nullptr && out.rank_score == nullptr)
+             : (out.span_stats == nullptr && out.span_flags == nullptr && out.step_anomalous == nullptr))
+    return;
+  const unsigned long long* plane = is_sig ? src.sig_plane : src.span_plane;
+  if (src.records == nullptr && plane == nullptr) return;
+  // ---- gather (a6) ------------------------------------------------------------------------------------
+  unsigned long long x[VPL];
+  const size_t off = is_sig ? (size_t)D.cell_off + (size_t)f * sizeof(argus_cell)
+                            : (size_t)D.span_off + (size_t)(f - D.S) * sizeof(argus_span) + 16u;
+  unsigned long long xmn = ~0ull, xmx = 0ull;
+#pragma unroll
+  for (int j = 0; j < VPL; ++j) {
+    const uint32_t r = (uint32_t)(j * 32 + lane);
+    x[j] = 0ull;
+    if (r < R) {
+      if (plane) {
+        x[j] = __ldg(plane + ((size_t)t * (is_sig ? D.S : D.P + 1u) + (is_sig ? f : f - D.S)) * src.rank_stride + r);
+      } else if (is_sig && src.use_sums) {
+        x[j] = __ldg(D.sums + ((size_t)r * D.T + t) * D.S + f);
+      } else {
+        const ulonglong2 q = __ldg(reinterpret_cast<const ulonglong2*>(
+            src.records + ((size_t)r * D.T + t) * D.rec_bytes + off));
+        x[j] = is_sig ? (q.x ? q.y : 0ull) : q.x;
+      }
+      xmn = x[j] < xmn ? x[j] : xmn;
+      xmx = x[j] > xmx ? x[j] : xmx;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long a = __shfl_xor_sync(FULL, xmn, o), b = __shfl_xor_sync(FULL, xmx, o);
+    xmn = a < xmn ? a : xmn;
+    xmx = b > xmx ? b : xmx;
+  }
+  if (xmx - xmn > 0xFFFFFFFFull) {           // the 64-bit pass takes this series
+    if (lane == 0) todo[series_id] = 1;
+    return;
+  }
+  // ---- a7 median, a8 MAD on exact 32-bit offsets from the minimum ------------------------------------------
+  uint32_t v[VPL], dev[VPL];
+#pragma unroll
+  for (int j = 0; j < VPL; ++j) v[j] = (uint32_t)(j * 32 + lane) < R ? (uint32_t)(x[j] - xmn) : 0u;
+  const uint32_t med_k = warp_median<VPL>(v, R, hist);
+#pragma unroll
+  for (int j = 0; j < VPL; ++j) dev[j] = v[j] >= med_k ? v[j] - med_k : med_k - v[j];
+  const uint32_t mad_k = warp_median<VPL>(dev, R, hist);
+  const unsigned long long med = xmn + med_k, mad = mad_k;
+  const unsigned long long thr = 3ull * mad;                         // mad < 2^32: no saturation (R12)
+  // ---- flags + roll-ups ------------------------------------------------------------------------------------
+  uint8_t* fl = is_sig ? out.sig_flags : out.span_flags;
+  const size_t series = is_sig ? (size_t)t * D.S + f : (size_t)t * (D.P + 1u) + (f - D.S);
+  uint32_t nh = 0, nl = 0;
+#pragma unroll
+  for (int j = 0; j < VPL; ++j) {
+    const uint32_t r = (uint32_t)(j * 32 + lane);
+    if (r < R) {
+      uint8_t g = ARGUS_FLAG_NONE;
+      if ((unsigned long long)dev[j] > thr) g = v[j] > med_k ? ARGUS_FLAG_HIGH : ARGUS_FLAG_LOW;   // R13, R14
+      nh += g == ARGUS_FLAG_HIGH;
+      nl += g == ARGUS_FLAG_LOW;
+      if (fl) fl[series * R + r] = g;
+      if (is_sig && out.rank_score && g == ARGUS_FLAG_HIGH) atomicAdd(&out.rank_score[(size_t)t * R + r], 1u);
+    }
+  }
+  nh = __reduce_add_sync(FULL, nh);
+  nl = __reduce_add_sync(FULL, nl);
+  if (lane == 0) {
+    argus_series_stat st;
+    st.median = med; st.mad = mad; st.n_high = nh; st.n_low = nl; st.reserved = 0;
+    if (is_sig) { if (out.sig_stats) out.sig_stats[series] = st; }
+    else {
+      if (out.span_stats) out.span_stats[series] = st;
+      if (f - D.S == D.P && out.step_anomalous) out.step_anomalous[t] = nh;
+    }
+  }
+}
+
 }  // namespace
 
 static cudaError_t launch_select(argus_ctx* ctx, const DiagSrc& src, const argus_dims& D, const argus_diag_out* o,
@@ -275,15 +465,21 @@ static cudaError_t launch_select(argus_ctx* ctx, const DiagSrc& src, const argus
   const uint64_t blocks = (uint64_t)D.T * (D.S + D.P + 1u);     // <= the ctx's own series count (checked by callers)
   uint8_t* todo = ctx->d_diag_todo;        // one mark byte per series (workspace)
   const unsigned nb = (unsigned)blocks;
-  if (D.R <= 64u * EPT) {
-    diagnose_kernel<64, uint32_t><<<nb, 64, 0, s>>>(src, D, *o, todo);
-    diagnose_kernel<64, unsigned long long><<<nb, 64, 0, s>>>(src, D, *o, todo);
+  // 32-bit pass: one warp per series up to 1024 ranks, one CTA per series beyond; then the few series
+  // that span 2^32 or more (marked in todo) in 64 bits, by a handful of CTAs that walk the marks
+  const unsigned wide_grid = nb < (unsigned)ctx->sm_count * 2u ? nb : (unsigned)ctx->sm_count * 2u;
+  if (D.R <= 256u) {
+    diagnose_warp_kernel<8><<<(nb + 7u) / 8u, 256, 0, s>>>(src, D, *o, todo, nb);
+    diagnose_kernel<64, unsigned long long><<<wide_grid, 64, 0, s>>>(src, D, *o, todo, nb);
+  } else if (D.R <= 1024u) {
+    diagnose_warp_kernel<32><<<(nb + 7u) / 8u, 256, 0, s>>>(src, D, *o, todo, nb);
+    diagnose_kernel<64, unsigned long long><<<wide_grid, 64, 0, s>>>(src, D, *o, todo, nb);
   } else if (D.R <= 256u * EPT) {
-    diagnose_kernel<256, uint32_t><<<nb, 256, 0, s>>>(src, D, *o, todo);
-    diagnose_kernel<256, unsigned long long><<<nb, 256, 0, s>>>(src, D, *o, todo);
+    diagnose_kernel<256, uint32_t><<<nb, 256, 0, s>>>(src, D, *o, todo, nb);
+    diagnose_kernel<256, unsigned long long><<<wide_grid, 256, 0, s>>>(src, D, *o, todo, nb);
   } else {
-    diagnose_kernel<1024, uint32_t><<<nb, 1024, 0, s>>>(src, D, *o, todo);
-    diagnose_kernel<1024, unsigned long long><<<nb, 1024, 0, s>>>(src, D, *o, todo);
+    diagnose_kernel<1024, uint32_t><<<nb, 1024, 0, s>>>(src, D, *o, todo, nb);
+    diagnose_kernel<1024, unsigned long long><<<wide_grid, 1024, 0, s>>>(src, D, *o, todo, nb);
   }
   ctx->n_kernels += 2;
   return cudaGetLastError();

@@ -5,7 +5,7 @@ import numpy as np
 from oracle import Oracle
 
 
-def run_gpu(events, R, T, S, P, step_base, sorted_hint=True, cuts=None, path=None, grid=None):
+def run_gpu(events, R, T, S, P, step_base, sorted_hint=True, cuts=None, path=None, grid=None, spill=0):
     """events: EVENT_DTYPE array (host).  Returns (records uint8 [R*T, rb], diag dict, (nv, ni), spans_out)."""
     import torch
     from paper_2606_20374_b200 import argus as A
@@ -13,7 +13,7 @@ def run_gpu(events, R, T, S, P, step_base, sorted_hint=True, cuts=None, path=Non
     biggest = n_all if cuts is None else max([b - a for a, b in zip(cuts[:-1], cuts[1:])] + [0])
     grouped = path == 3 or (path is None and not sorted_hint)
     ctx = A.Argus(R, T, S, P, step_base, sorted_hint=sorted_hint,
-                  max_ungrouped_events=biggest if grouped else 0)
+                  max_ungrouped_events=biggest if grouped else 0, max_spill_events=spill)
     if path is not None:
         ctx.tune(A.TUNE_FORCE_PATH, path)
     if grid is not None:

@@ -33,7 +33,7 @@ def test_sizes_and_pure_host_calls():
     assert lib.argus_record_bytes(None) == 0
     assert lib.argus_strerror(0) == b"ok" and b"invalid" in lib.argus_strerror(-1)
     assert b"sm_100a" in lib.argus_version()
-    assert ctypes.sizeof(A.ArgusConfig) == 32 and ctypes.sizeof(A.ArgusDiagOut) == 48
+    assert ctypes.sizeof(A.ArgusConfig) == 40 and ctypes.sizeof(A.ArgusDiagOut) == 48
     for dt, n in ((A.EVENT_DTYPE, 32), (A.CELL_DTYPE, 160), (A.SPAN_DTYPE, 32), (A.STAT_DTYPE, 32),
                   (A.HEADER_DTYPE, 64)):
         assert dt.itemsize == n

@@ -229,12 +229,49 @@ def test_launch_count_is_counted_not_assumed():
     outs = ctx.alloc_diag()
     assert ctx.launch_count() == (0, 0)
     ctx.reset(rec)
-    assert ctx.launch_count() == (0, 2)
+    assert ctx.launch_count() == (0, 1)
     ctx.aggregate(_dev(ev), ev.size, rec)
     k1 = ctx.launch_count()[0]
     assert k1 >= 1
     ctx.phase_times(rec)
     ctx.diagnose(rec, outs)
     k2, m2 = ctx.launch_count()
-    assert k2 > k1 + 1 and m2 == 3                   # finalize + selection kernels; rank_score clear
+    assert k2 > k1 + 1 and m2 == 2                   # finalize + selection kernels; rank_score clear
     ctx.close()
+
+
+def test_refused_count_diagnostic():
+    """Events the compact shared-memory cell cannot hold are re-queued through the spill area (range wider
+    than four buckets) or take the overflow list (>= 2^32 ns; everything when there is no spill area); both
+    are counted, and the results are exact either way (compare_with_oracle)."""
+    from paper_2606_20374_b200 import argus as A
+    n = 20000
+    # sig 0: one mode (no refusals); sig 1: two modes 2^10 and 2^20 (one of them is refused);
+    # sig 2: durations >= 2^32 ns (no 32-bit cell can hold them)
+    rows = []
+    for i in range(n):
+        rows.append((0, 0, 0, 0, 0, i, i + 1000 + i % 50))
+        rows.append((0, 0, 1, 0, 0, i, i + ((1 << 10) + i % 7 if i % 2 else (1 << 20) + i % 5)))
+        if i % 10 == 0:
+            rows.append((0, 0, 2, 0, 0, i, i + (1 << 33) + i))
+    ev = make_events(rows)
+    for spill in (0, ev.size, 3000):
+        ctx = A.Argus(1, 1, 3, 1, max_spill_events=spill)
+        rec = ctx.alloc_records()
+        outs = ctx.alloc_diag()
+        ctx.reset(rec)
+        ctx.aggregate(_dev(ev), ev.size, rec)
+        ctx.phase_times(rec)
+        ctx.diagnose(rec, outs)
+        requeued, overflow = ctx.refused_count()
+        if spill == 0:
+            assert requeued == 0 and 0.45 * n + n // 10 <= overflow <= n + n // 10, (requeued, overflow)   # every CTA refuses one of the modes
+        elif spill == ev.size:
+            assert 0.45 * n <= requeued <= n and overflow == n // 10, (requeued, overflow)   # one mode of sig 1; all of sig 2
+        else:
+            assert 0 < requeued <= 3000 and overflow >= 0.45 * n + n // 10 - requeued, (requeued, overflow)   # the area ran out
+        compare_with_oracle(ctx.records_to_host(rec), ctx.diag_to_host(outs), ctx.stats(), None, ev, 1, 1, 3, 1, 0)
+        ctx.reset(rec)
+        ctx.aggregate(_dev(ev[ev["sig"] == 0]), n, rec)
+        assert ctx.refused_count() == (0, 0)
+        ctx.close()

@@ -144,6 +144,7 @@ def test_bucket_window_invariant_cells():
     ev = make_events(rows)
     for grid in (None, 5):
         assert_parity(ev, R, T, n_sig, 2, 0, path=PATH_SEG, grid=grid)
+        assert_parity(ev, R, T, n_sig, 2, 0, path=PATH_SEG, grid=grid, spill=ev.size)
 
 
 @pytest.mark.parametrize("path", [PATH_SEG, PATH_GLOBAL])
@@ -174,6 +175,27 @@ def test_unsorted_scaled():
         assert_parity(ev2, *_dims(wl2.spec), sorted_hint=False)
     # the shuffled events in uneven chunks: every call groups its own chunk
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False, cuts=[0, 7, 100_000, 100_001, 900_000, ev.size])
+
+
+def test_multimodal_sigs_requeued():
+    # same-name kernels "differ in duration by several multiples" between positions.  A share of
+    # the sigs gets a second mode 8-4096x the first: the compact cell refuses it, the event is re-queued into
+    # the CTA's spill region and folded by the second launch; a third mode (or an exhausted region) falls
+    # back to the overflow list.
+    import dataclasses
+    for name, kw, frac in (("mid", dict(n_ranks=24, n_steps=2), 0.5),
+                           ("production", dict(n_ranks=8, n_events=150_001), 0.3),
+                           ("unsorted", dict(n_ranks=16, n_events=20_000, shuffle=False), 0.0)):   # Pareto tails
+        spec = dataclasses.replace(scaled(name, **kw), bimodal_frac=frac, bimodal_ratio=(8.0, 4096.0))
+        wl = build_workload(spec)
+        ev = wl.expand_host()
+        for grid, spill in ((None, ev.size), (7, ev.size // 16), (None, 0), (3, 1000)):
+            assert_parity(ev, *_dims(wl.spec), path=PATH_SEG, grid=grid, spill=spill)
+    # the invariant sweep of test_bucket_window_invariant_cells (five spread buckets in one sig: a chain of
+    # refusals in the second launch) with a spill area, chunked
+    wl = build_workload(dataclasses.replace(scaled("unsorted", n_ranks=32, n_events=6000), bimodal_frac=0.0))
+    ev = wl.expand_host()
+    assert_parity(ev, *_dims(wl.spec), sorted_hint=False, spill=ev.size, cuts=[0, 50_001, ev.size])
 
 
 def test_odd_rank_counts_select():
