@@ -265,14 +265,29 @@ template <int NT, typename K>
 __global__ void __launch_bounds__(NT, (sizeof(K) == 4 && NT <= 256) ? 1024 / NT : 1)
 diagnose_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restrict__ todo, uint32_t n_series) {
   __shared__ SelSmem sm;
-  // K = 32 bit: one CTA per series.  K = 64 bit: a few CTAs walk the (few) marked series.
-  for (uint32_t b = blockIdx.x; b < n_series; b += gridDim.x) {
-    if (sizeof(K) == 8 && !todo[b]) continue;
-    __syncthreads();                       // the previous series is done with sm
-    diagnose_series<NT, K>(src, D, out, todo, b, sm);
+  if (sizeof(K) == 4) {                    // one CTA per series
+    if (blockIdx.x < n_series) diagnose_series<NT, K>(src, D, out, todo, blockIdx.x, sm);
+    return;
+  }
+  // K = 64 bit: a few CTAs, each scanning its share of the marks NT at a time (coalesced byte loads, so that
+  // the usual case — no series spans 2^32 — costs one pass over the marks) and selecting the marked series
+  __shared__ uint32_t s_list[NT];
+  __shared__ uint32_t s_n;
+  const uint32_t chunk = (n_series + gridDim.x - 1u) / gridDim.x;
+  const uint32_t b0 = blockIdx.x * chunk, b1 = b0 + chunk < n_series ? b0 + chunk : n_series;
+  for (uint32_t base = b0; base < b1; base += NT) {
+    if (threadIdx.x == 0) s_n = 0u;
+    __syncthreads();
+    const uint32_t b = base + threadIdx.x;
+    if (b < b1 && todo[b]) s_list[atomicAdd(&s_n, 1u)] = b;
+    __syncthreads();
+    const uint32_t cnt = s_n;
+    for (uint32_t i = 0; i < cnt; ++i) {
+      diagnose_series<NT, K>(src, D, out, todo, s_list[i], sm);
+      __syncthreads();                     // the next series reuses sm
+    }
   }
 }
-
 
 // ---- R <= 1024: one WARP per series ----------------------------------------------------------------
 // The block kernel above spends its time in block barriers (about ten radix passes of three barriers
