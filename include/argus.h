@@ -258,6 +258,92 @@ int argus_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t sig_lo, ui
  * step_anomalous [T]; T and P are the ctx's, R = planes->n_ranks.  [host] planes, [host] outs. */
 int argus_diagnose_planes(argus_ctx* ctx, const argus_planes* planes, const argus_diag_out* outs, void* stream);
 
+/* ==== the paper's own float algorithms (SURVEY 8(f) NEXT-1..3), fp64; every constant the paper leaves open
+ * is a parameter whose default is a reading of DESIGN.md 3 (R23-R36) ================================== */
+
+/* ---- NEXT-1: online statistical compression (eq. 1) ---------------------------------
+ * "applies a logarithmic transformation to the raw durations, then computes the KDE density function on an
+ * equally-spaced grid" with Scott's bandwidth, "local minima (valleys) as cluster boundaries", two filters,
+ * then "(count, p50, p99)" per cluster.  The grid is a histogram of log-durations with per_octave bins per
+ * factor of two: the 32-bucket histogram of the records (per_octave = 1), or the fine histogram of
+ * argus_fine_hist (per_octave = 8, 256 bins: bin(d) = floor(8 log2 d), 0 for d <= 1, 255 for d >= 2^32). */
+typedef struct argus_cluster {
+  uint32_t count;      /* 0 = unused slot */
+  uint16_t p50_bin;    /* grid bin where the cluster's cumulative count first reaches ceil(0.5 count) */
+  uint16_t p99_bin;    /* ... ceil(0.99 count); a bin stands for 2^((bin + 0.5) / per_octave) ns */
+} argus_cluster;       /* 8 B */
+typedef struct argus_kde_params {
+  uint32_t per_octave;    /* grid steps per factor of two: 1 or 8 */
+  uint32_t n_bins;        /* 32 or 256 (<= 256) */
+  uint32_t min_count;     /* cluster-level filter: both sides of a kept valley hold >= max(min_count, min_frac n) samples (8) */
+  uint32_t min_gap_bins;  /* spacing filter: kept boundaries are >= this many grid steps apart (half an octave) */
+  uint32_t max_clusters;  /* output slots per cell (the last one takes the rest), 1..16 */
+  uint32_t reserved;
+  double   min_frac;      /* 0.02 */
+} argus_kde_params;
+/* Fine histogram of the valid events' durations per (rank, step, sig): [device] d_hist [R][T][S][256] u32,
+ * accumulated into (the caller zeroes it).  L2 atomics: meant for the sizes a [R][T][S][256] table fits. */
+int argus_fine_hist(argus_ctx* ctx, const argus_event* d_events, uint64_t n, uint32_t* d_hist, void* stream);
+/* n_cells histograms of p->n_bins counters -> [device] d_clusters [n_cells][max_clusters], d_n_clusters
+ * [n_cells]; d_density [n_cells][n_bins] f64 receives the density of eq. (1) (with 1/h) or may be NULL. */
+int argus_kde_clusters(argus_ctx* ctx, const uint32_t* d_hist, uint64_t n_cells, const argus_kde_params* p,
+                       argus_cluster* d_clusters, uint8_t* d_n_clusters, double* d_density, void* stream);
+/* The same on the 32-bucket histograms of this ctx's finalised record table (p->per_octave = 1, n_bins = 32):
+ * d_clusters [R][T][S][max_clusters], d_n_clusters [R][T][S].  No pass over the events. */
+int argus_kde_clusters_records(argus_ctx* ctx, const void* d_records, const argus_kde_params* p,
+                               argus_cluster* d_clusters, uint8_t* d_n_clusters, void* stream);
+
+/* ---- NEXT-2: L3 kernel-statistics anomaly detection (eq. 2-4) -------------------------
+ * Per key (kernel): every rank's clusters (count, p50, p99) -> log-normal mixture CDF (mu = ln p50,
+ * sigma = (ln p99 - ln p50)/2.326) on a log-uniform grid of n_grid points from 0.5 min p50 to 2 max p99 ->
+ * W1 by the trapezoid rule -> score = mean W1 to the other ranks -> flag when score > Q3 + alpha (Q3 - Q1). */
+typedef struct argus_l3_in {
+  const uint32_t* count;   /* [device] [n_keys][n_ranks][max_clusters] (0 = no cluster) */
+  const double*   p50;     /* [device] same shape, ns */
+  const double*   p99;
+  uint32_t n_keys, n_ranks /* <= 4096 */, max_clusters, reserved;
+} argus_l3_in;
+typedef struct argus_l3_params { uint32_t n_grid /* >= 2 (256) */; uint32_t reserved; double alpha /* 1.5 */; } argus_l3_params;
+typedef struct argus_l3_stat { double q1, q3, fence, x_lo, x_hi; } argus_l3_stat;
+/* [device] d_score [n_keys][n_ranks] f64, d_stat [n_keys], d_flags [n_keys][n_ranks] u8. */
+int argus_l3_detect(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* p, double* d_score,
+                    argus_l3_stat* d_stat, uint8_t* d_flags, void* stream);
+
+/* ---- NEXT-3: L2 phase-level attribution (eq. 5, Table 3) ---------------------
+ * For every phase span k (index P = whole iteration) of this ctx's finalised table: x_r = mean over the T
+ * steps of span_ns; the ranks are compared inside the parallelism group the event is routed to:
+ * d_route [P+1] u8 names the dimension of event k, d_group_id [n_dims][R] u32 the group (an id < R; >= R =
+ * none) of every rank in each dimension.  Per group: n, mu, sigma (|G| - 1), CV = sigma/mu and its class
+ * (0 balanced < 0.02 <= 1 mild < 0.05 <= 2 severe); per rank z = (x - mu)/sigma, flag = z > z_threshold. */
+typedef struct argus_l2_group { uint32_t n, cls; double mu, sigma, cv; } argus_l2_group;   /* 32 B */
+/* [device] d_groups [P+1][R] (indexed by group id; n = 0: no such group), d_z [P+1][R] f64, d_flags [P+1][R]
+ * u8, d_xbar [P+1][R] f64 (the x_r; also scratch). */
+int argus_l2_groups(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
+                    double z_threshold, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
+                    void* stream);
+
+/* ---- NEXT-3: L1 iteration-level detection ----------------------------------------------
+ * n_series time series of n_steps u64 values (iteration times in ns), value (s, t) at
+ * d_base + s*series_stride + t*step_stride bytes (e.g. the span_ns of index P in argus_phase_times'
+ * d_spans_out).  Jitter: windows of `window` points whose max/min exceeds theta are candidates, adjacent or
+ * overlapping ones merge; per merged interval the baseline is the median of the points outside it and the
+ * effective width the longest run inside it above beta x baseline.  Change point: the split (both sides >=
+ * min_seg points) with the largest mu_R/mu_L among those with mu_R/mu_L > ratio_min and sigma/mu < rsd_max on
+ * both sides.  cls: 0 stable, 1 jitter, 2 regression, 3 both.  n_steps <= 2048. */
+#define ARGUS_L1_MAX_INTERVALS 8
+typedef struct argus_l1_params {
+  uint32_t window /* 8 */, min_seg /* 4 */;
+  double theta /* 1.5 */, beta /* 1.25 */, ratio_min /* 1.1 */, rsd_max /* 0.05 */;
+} argus_l1_params;
+typedef struct argus_l1_interval { uint32_t first, last, width, reserved; double baseline; } argus_l1_interval;  /* 24 B */
+typedef struct argus_l1_out {
+  uint32_t cls, n_intervals /* may exceed ARGUS_L1_MAX_INTERVALS: only the first are stored */, cp_found, cp_step;
+  double cp_ratio;
+  argus_l1_interval interval[ARGUS_L1_MAX_INTERVALS];
+} argus_l1_out;
+int argus_l1_detect(argus_ctx* ctx, const void* d_base, uint64_t series_stride, uint64_t step_stride,
+                    uint32_t n_series, uint32_t n_steps, const argus_l1_params* p, argus_l1_out* d_out, void* stream);
+
 /* Synchronises the internal copy stream and every stream passed to this ctx since argus_create (the ctx
  * remembers up to 8 distinct ones; the oldest is synchronised when a ninth appears) and returns the event
  * counters since argus_reset.  Asynchronous kernel faults surface here as ARGUS_ECUDA.  [host] outputs,

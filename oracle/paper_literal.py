@@ -58,7 +58,7 @@ def grid_points(n_bins: int, per_octave: int) -> np.ndarray:
 
 
 def kde_clusters(hist: Sequence[int], per_octave: int = FINE_PER_OCTAVE, min_count: int = 8,
-                 min_frac: float = 0.02, min_gap: float = 0.5 * math.log(2.0)):
+                 min_frac: float = 0.02, min_gap_bins: int = FINE_PER_OCTAVE // 2, max_clusters: int = 8):
     """One (kernel, rank, window) histogram on the equally spaced log grid -> clusters.
     Returns (density f[n_bins], h, boundaries (bin indices), clusters [(count, p50_bin, p99_bin)]).
 
@@ -67,15 +67,19 @@ def kde_clusters(hist: Sequence[int], per_octave: int = FINE_PER_OCTAVE, min_cou
     binned KDE), the grid is the same bin centres.
     eq. (1) with the 1/h factor restored (R22): f(x) = 1/(n h) * sum_b c_b K((x - x_b)/h), K = N(0, 1) pdf.
     PAPER.md:182 Scott's rule h = 1.06 sigma n^(-1/5); sigma = sample standard deviation (n - 1) of the
-    weighted samples (R25); n < 2 or sigma = 0 -> no density, one cluster (R26).
+    weighted samples (R25); n < 2 or every sample in ONE grid bin (sigma = 0) -> no density, one cluster
+    (R26; tested on the occupied range, an integer comparison, not on a rounded sigma).
     PAPER.md:182 "All local minima on the density curve are identified as candidate cluster boundaries":
     bin j strictly inside the occupied range with f[j] < f[j-1] and f[j] <= f[j+1] (R27).
     "cluster-level filtering requires that both sides of each valley contain sufficient samples" (R28): left
     to right, a candidate is kept when the samples since the previous kept boundary and the samples to its
     right both number >= max(min_count, min_frac * n); the boundary belongs to the right-hand cluster.
     "spacing filtering requires that the duration difference between adjacent retained boundaries is
-    sufficiently significant" (R29): a kept boundary must lie >= min_gap (half an octave) in log-duration
-    after the previous kept one.
+    sufficiently significant" (R29): a kept boundary must lie >= min_gap_bins grid steps (half an octave, a
+    factor 1.41 in duration) after the previous kept one — counted in grid steps so that the decision is an
+    integer comparison.
+    At most max_clusters clusters (a fixed-size output slot): once max_clusters - 1 boundaries are kept, the
+    last cluster takes the rest.
     PAPER.md:182-194 per cluster: count, p50, p99 — the bins where the cluster's cumulative count first
     reaches ceil(0.5 count) and ceil(0.99 count) (R30: bin-quantised percentiles)."""
     c = np.asarray(hist, dtype=np.float64)
@@ -93,7 +97,7 @@ def kde_clusters(hist: Sequence[int], per_octave: int = FINE_PER_OCTAVE, min_cou
         mean = float((c * x).sum() / n)
         var = float((c * (x - mean) ** 2).sum() / (n - 1.0))
         sigma = math.sqrt(var)
-        if sigma > 0.0:
+        if hi > lo:
             h = SCOTT * sigma * n ** (-0.2)
             for j in range(nb):
                 u = (x[j] - x) / h
@@ -104,7 +108,8 @@ def kde_clusters(hist: Sequence[int], per_octave: int = FINE_PER_OCTAVE, min_cou
                 if f[j] < f[j - 1] and f[j] <= f[j + 1]:
                     left = float(c[prev:j].sum())
                     right = float(c[j:hi + 1].sum())
-                    if left >= need and right >= need and (not bounds or x[j] - x[bounds[-1]] >= min_gap):
+                    if left >= need and right >= need and (not bounds or j - bounds[-1] >= min_gap_bins) \
+                            and len(bounds) + 1 < max_clusters:
                         bounds.append(j)
                         prev = j
     clusters = []

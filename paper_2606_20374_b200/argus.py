@@ -30,10 +30,20 @@ HEADER_DTYPE = np.dtype([("magic", "<u4"), ("version", "<u2"), ("n_phases", "<u2
                          ("n_events", "<u8"), ("min_start", "<i8"), ("max_end", "<i8"),
                          ("iter_ns", "<u8"), ("reserved1", "<u8")])
 
+CLUSTER_DTYPE = np.dtype([("count", "<u4"), ("p50_bin", "<u2"), ("p99_bin", "<u2")])
+L3_STAT_DTYPE = np.dtype([("q1", "<f8"), ("q3", "<f8"), ("fence", "<f8"), ("x_lo", "<f8"), ("x_hi", "<f8")])
+L2_GROUP_DTYPE = np.dtype([("n", "<u4"), ("cls", "<u4"), ("mu", "<f8"), ("sigma", "<f8"), ("cv", "<f8")])
+L1_MAX_INTERVALS = 8
+L1_INTERVAL_DTYPE = np.dtype([("first", "<u4"), ("last", "<u4"), ("width", "<u4"), ("reserved", "<u4"),
+                              ("baseline", "<f8")])
+L1_OUT_DTYPE = np.dtype([("cls", "<u4"), ("n_intervals", "<u4"), ("cp_found", "<u4"), ("cp_step", "<u4"),
+                         ("cp_ratio", "<f8"), ("interval", L1_INTERVAL_DTYPE, (L1_MAX_INTERVALS,))])
+
 EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes",
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
            "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
-           "argus_diagnose_planes", "argus_stats", "argus_refused_count",
+           "argus_diagnose_planes", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
+           "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
 
@@ -56,6 +66,27 @@ class ArgusPlanes(ctypes.Structure):
     _fields_ = [("sig_sums", ctypes.c_void_p), ("span_ns", ctypes.c_void_p),
                 ("n_ranks", ctypes.c_uint32), ("rank_stride", ctypes.c_uint32),
                 ("n_sigs", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
+
+
+class ArgusKdeParams(ctypes.Structure):
+    _fields_ = [("per_octave", ctypes.c_uint32), ("n_bins", ctypes.c_uint32), ("min_count", ctypes.c_uint32),
+                ("min_gap_bins", ctypes.c_uint32), ("max_clusters", ctypes.c_uint32), ("reserved", ctypes.c_uint32),
+                ("min_frac", ctypes.c_double)]
+
+
+class ArgusL3In(ctypes.Structure):
+    _fields_ = [("count", ctypes.c_void_p), ("p50", ctypes.c_void_p), ("p99", ctypes.c_void_p),
+                ("n_keys", ctypes.c_uint32), ("n_ranks", ctypes.c_uint32), ("max_clusters", ctypes.c_uint32),
+                ("reserved", ctypes.c_uint32)]
+
+
+class ArgusL3Params(ctypes.Structure):
+    _fields_ = [("n_grid", ctypes.c_uint32), ("reserved", ctypes.c_uint32), ("alpha", ctypes.c_double)]
+
+
+class ArgusL1Params(ctypes.Structure):
+    _fields_ = [("window", ctypes.c_uint32), ("min_seg", ctypes.c_uint32), ("theta", ctypes.c_double),
+                ("beta", ctypes.c_double), ("ratio_min", ctypes.c_double), ("rsd_max", ctypes.c_double)]
 
 
 class ArgusError(RuntimeError):
@@ -102,6 +133,19 @@ def load() -> ctypes.CDLL:
                                       ctypes.c_uint32, vp]
     lib.argus_diagnose_planes.restype = i32
     lib.argus_diagnose_planes.argtypes = [vp, ctypes.POINTER(ArgusPlanes), ctypes.POINTER(ArgusDiagOut), vp]
+    lib.argus_fine_hist.restype = i32
+    lib.argus_fine_hist.argtypes = [vp, vp, u64, vp, vp]
+    lib.argus_kde_clusters.restype = i32
+    lib.argus_kde_clusters.argtypes = [vp, vp, u64, ctypes.POINTER(ArgusKdeParams), vp, vp, vp, vp]
+    lib.argus_kde_clusters_records.restype = i32
+    lib.argus_kde_clusters_records.argtypes = [vp, vp, ctypes.POINTER(ArgusKdeParams), vp, vp, vp]
+    lib.argus_l3_detect.restype = i32
+    lib.argus_l3_detect.argtypes = [vp, ctypes.POINTER(ArgusL3In), ctypes.POINTER(ArgusL3Params), vp, vp, vp, vp]
+    lib.argus_l2_groups.restype = i32
+    lib.argus_l2_groups.argtypes = [vp, vp, vp, vp, ctypes.c_double, vp, vp, vp, vp, vp]
+    lib.argus_l1_detect.restype = i32
+    lib.argus_l1_detect.argtypes = [vp, vp, u64, u64, ctypes.c_uint32, ctypes.c_uint32,
+                                    ctypes.POINTER(ArgusL1Params), vp, vp]
     lib.argus_stats.restype = i32
     lib.argus_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_refused_count.restype = i32
@@ -260,6 +304,43 @@ class Argus:
                                                        "span_flags", "rank_score", "step_anomalous")])
         self._check(self.lib.argus_diagnose_planes(self._h, ctypes.byref(pl), ctypes.byref(o),
                                                    _stream(stream)))
+
+    # ---- the paper-literal float algorithms (NEXT-1..3): marshalling only ---------------------------------
+    def fine_hist(self, d_events, n: int, d_hist, stream=None) -> None:
+        self._check(self.lib.argus_fine_hist(self._h, _ptr(d_events), n, _ptr(d_hist), _stream(stream)))
+
+    @staticmethod
+    def kde_params(per_octave: int = 8, n_bins: int = 256, min_count: int = 8, min_gap_bins: Optional[int] = None,
+                   max_clusters: int = 8, min_frac: float = 0.02) -> "ArgusKdeParams":
+        gap = per_octave // 2 if min_gap_bins is None else min_gap_bins
+        return ArgusKdeParams(per_octave, n_bins, min_count, gap, max_clusters, 0, min_frac)
+
+    def kde_clusters(self, d_hist, n_cells: int, params, d_clusters, d_n_clusters, d_density=None, stream=None) -> None:
+        self._check(self.lib.argus_kde_clusters(self._h, _ptr(d_hist), n_cells, ctypes.byref(params), _ptr(d_clusters),
+                                                _ptr(d_n_clusters), _ptr(d_density), _stream(stream)))
+
+    def kde_clusters_records(self, d_records, params, d_clusters, d_n_clusters, stream=None) -> None:
+        self._check(self.lib.argus_kde_clusters_records(self._h, _ptr(d_records), ctypes.byref(params),
+                                                        _ptr(d_clusters), _ptr(d_n_clusters), _stream(stream)))
+
+    def l3_detect(self, d_count, d_p50, d_p99, n_keys: int, n_ranks: int, max_clusters: int, d_score, d_stat,
+                  d_flags, n_grid: int = 256, alpha: float = 1.5, stream=None) -> None:
+        i = ArgusL3In(_ptr(d_count), _ptr(d_p50), _ptr(d_p99), n_keys, n_ranks, max_clusters, 0)
+        q = ArgusL3Params(n_grid, 0, alpha)
+        self._check(self.lib.argus_l3_detect(self._h, ctypes.byref(i), ctypes.byref(q), _ptr(d_score), _ptr(d_stat),
+                                             _ptr(d_flags), _stream(stream)))
+
+    def l2_groups(self, d_records, d_route, d_group_id, z_threshold: float, d_groups, d_z, d_flags, d_xbar,
+                  stream=None) -> None:
+        self._check(self.lib.argus_l2_groups(self._h, _ptr(d_records), _ptr(d_route), _ptr(d_group_id), z_threshold,
+                                             _ptr(d_groups), _ptr(d_z), _ptr(d_flags), _ptr(d_xbar), _stream(stream)))
+
+    def l1_detect(self, d_base, series_stride: int, step_stride: int, n_series: int, n_steps: int, d_out,
+                  window: int = 8, min_seg: int = 4, theta: float = 1.5, beta: float = 1.25, ratio_min: float = 1.1,
+                  rsd_max: float = 0.05, stream=None) -> None:
+        q = ArgusL1Params(window, min_seg, theta, beta, ratio_min, rsd_max)
+        self._check(self.lib.argus_l1_detect(self._h, _ptr(d_base), series_stride, step_stride, n_series, n_steps,
+                                             ctypes.byref(q), _ptr(d_out), _stream(stream)))
 
     def stats(self):
         a, b = ctypes.c_uint64(), ctypes.c_uint64()

@@ -383,6 +383,85 @@ extern "C" int argus_diagnose_planes(argus_ctx* ctx, const argus_planes* pl, con
   return ARGUS_OK;
 }
 
+// ---- the paper-literal float algorithms (paper_literal.cu) ------------------------------------------------
+static bool kde_params_ok(const argus_kde_params* p) {
+  return p && (p->per_octave == 1u || p->per_octave == 8u) && p->n_bins >= 2u && p->n_bins <= 256u &&
+         p->max_clusters >= 1u && p->max_clusters <= 16u && p->min_frac >= 0.0;
+}
+
+#define ARGUS_ENTER(ctx, stream)                       \
+  cudaStream_t s = (cudaStream_t)(stream);             \
+  CU(ctx, cudaSetDevice((ctx)->cfg.device));           \
+  {                                                    \
+    int rc__ = note_stream(ctx, s);                    \
+    if (rc__ != ARGUS_OK) return rc__;                 \
+  }
+
+extern "C" int argus_fine_hist(argus_ctx* ctx, const argus_event* d_events, uint64_t n, uint32_t* d_hist, void* stream) {
+  if (!ctx || !d_hist || ((uintptr_t)d_hist & 3u)) return ARGUS_EINVAL;
+  if (n != 0 && (!d_events || !aligned16(d_events))) return ARGUS_EINVAL;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_fine_hist(ctx, d_events, n, d_hist, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_kde_clusters(argus_ctx* ctx, const uint32_t* d_hist, uint64_t n_cells, const argus_kde_params* p,
+                                  argus_cluster* d_clusters, uint8_t* d_n_clusters, double* d_density, void* stream) {
+  if (!ctx || !kde_params_ok(p) || !d_hist || !d_clusters || !d_n_clusters) return ARGUS_EINVAL;
+  if (((uintptr_t)d_hist & 3u) || !aligned8(d_clusters) || !aligned8(d_density)) return ARGUS_EINVAL;
+  if ((n_cells + 7) / 8 > 0x7FFFFFFFull) return ARGUS_ESIZE;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_kde_hist(ctx, d_hist, n_cells, p, d_clusters, d_n_clusters, d_density, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_kde_clusters_records(argus_ctx* ctx, const void* d_records, const argus_kde_params* p,
+                                          argus_cluster* d_clusters, uint8_t* d_n_clusters, void* stream) {
+  if (!ctx || !kde_params_ok(p) || p->n_bins != 32u || p->per_octave != 1u) return ARGUS_EINVAL;
+  if (!d_records || !d_clusters || !d_n_clusters || !aligned8(d_clusters)) return ARGUS_EINVAL;
+  if (d_records == ctx->d_records && !ctx->finalized) return ARGUS_ESTATE;
+  if (((uint64_t)ctx->dims.R * ctx->dims.T * ctx->dims.S + 7) / 8 > 0x7FFFFFFFull) return ARGUS_ESIZE;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_kde_records(ctx, d_records, p, d_clusters, d_n_clusters, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_l3_detect(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* p, double* d_score,
+                               argus_l3_stat* d_stat, uint8_t* d_flags, void* stream) {
+  if (!ctx || !in || !p || !d_score || !d_stat || !d_flags) return ARGUS_EINVAL;
+  if (in->n_keys != 0 && (!in->count || !in->p50 || !in->p99)) return ARGUS_EINVAL;
+  if (in->n_ranks == 0 || in->max_clusters == 0 || p->n_grid < 2u) return ARGUS_EINVAL;
+  if (in->n_ranks > 4096u || argus_l3_smem_bytes(in->n_ranks) > (size_t)ctx->max_smem_optin) return ARGUS_ESIZE;
+  if (!aligned8(d_score) || !aligned8(d_stat) || !aligned8(in->p50) || !aligned8(in->p99)) return ARGUS_EINVAL;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_l3(ctx, in, p, d_score, d_stat, d_flags, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_l2_groups(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
+                               double z_threshold, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags,
+                               double* d_xbar, void* stream) {
+  if (!ctx || !d_records || !d_route || !d_group_id || !d_groups || !d_z || !d_flags || !d_xbar) return ARGUS_EINVAL;
+  if (!aligned8(d_groups) || !aligned8(d_z) || !aligned8(d_xbar) || ((uintptr_t)d_group_id & 3u)) return ARGUS_EINVAL;
+  if (d_records == ctx->d_records && !ctx->finalized) return ARGUS_ESTATE;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_l2(ctx, d_records, d_route, d_group_id, z_threshold, d_groups, d_z, d_flags, d_xbar, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_l1_detect(argus_ctx* ctx, const void* d_base, uint64_t series_stride, uint64_t step_stride,
+                               uint32_t n_series, uint32_t n_steps, const argus_l1_params* p, argus_l1_out* d_out,
+                               void* stream) {
+  if (!ctx || !p || !d_out || !aligned8(d_out)) return ARGUS_EINVAL;
+  if (n_series != 0 && n_steps != 0 && (!d_base || !aligned8(d_base) || (series_stride & 7u) || (step_stride & 7u)))
+    return ARGUS_EINVAL;
+  if (p->window < 2u || p->min_seg < 2u) return ARGUS_EINVAL;
+  if (n_steps > 2048u) return ARGUS_ESIZE;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_l1(ctx, d_base, series_stride, step_stride, n_series, n_steps, p, d_out, s));
+  return ARGUS_OK;
+}
+
 extern "C" int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid) {
   if (!ctx) return ARGUS_EINVAL;
   CU(ctx, cudaSetDevice(ctx->cfg.device));

@@ -87,6 +87,19 @@ cudaError_t argus_launch_diagnose_planes(argus_ctx* ctx, const argus_planes* pl,
 cudaError_t argus_launch_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t s0, uint32_t s1,
                                      uint64_t* dst_sig, uint64_t* dst_span, uint32_t stride, uint32_t off,
                                      cudaStream_t s);
+cudaError_t argus_launch_fine_hist(argus_ctx* ctx, const argus_event* ev, uint64_t n, uint32_t* d_hist, cudaStream_t s);
+cudaError_t argus_launch_kde_hist(argus_ctx* ctx, const uint32_t* d_hist, uint64_t n_cells, const argus_kde_params* P,
+                                  argus_cluster* d_clusters, uint8_t* d_n, double* d_density, cudaStream_t s);
+cudaError_t argus_launch_kde_records(argus_ctx* ctx, const void* d_records, const argus_kde_params* P,
+                                     argus_cluster* d_clusters, uint8_t* d_n, cudaStream_t s);
+size_t argus_l3_smem_bytes(uint32_t R);
+cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,
+                            argus_l3_stat* d_stat, uint8_t* d_flags, cudaStream_t s);
+cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
+                            double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
+                            cudaStream_t s);
+cudaError_t argus_launch_l1(argus_ctx* ctx, const void* d_base, uint64_t sstride, uint64_t tstride, uint32_t n_series,
+                            uint32_t T, const argus_l1_params* P, argus_l1_out* d_out, cudaStream_t s);
 bool argus_seg_supported(const argus_ctx* ctx);
 void argus_partition_plan(const argus_config* cfg, int sm_count, int max_smem_optin, uint32_t* n_cta,
                           bool* smem);

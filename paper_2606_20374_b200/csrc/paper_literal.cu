@@ -1,0 +1,567 @@
+// paper_literal.cu — the paper's own float algorithms on top of the integer path (SURVEY §8(f) NEXT-1..3):
+//   NEXT-1  online statistical compression: log transform -> KDE on an equally spaced grid with Scott's
+//           bandwidth (eq. 1) -> valleys -> two filters -> per-cluster (count, p50, p99)
+//   NEXT-2  L3: log-normal mixture CDF (eq. 2) -> W1 by trapezoid on a log-uniform grid (eq. 3) -> mean-W1
+//           deviation score -> IQR upper fence (eq. 4)
+//   NEXT-3  L2: CV + z-score within a parallelism group (eq. 5, Table 3); L1: sliding-window ratio-gated
+//           jitter detection and full-scan change point
+// All in fp64 (the oracle's precision; where a float decides an integer — a valley, a flag — both sides
+// decide in fp64).  Constants the paper leaves open are parameters; their defaults are the readings
+// R23-R36 of DESIGN.md §3.  None of this is a contraction: no tensor cores.
+#include <math.h>
+
+#include "argus_internal.cuh"
+
+namespace {
+
+constexpr uint32_t FULL = 0xFFFFFFFFu;
+
+// ---- NEXT-1: fine histogram ---------------------------------------------------------------------------
+// R23: bin(d) = floor(8 log2 d) in [0, 255], decided in integers: b = floor(log2 d), m = d normalised to 32
+// bits, sub = #{j in 1..7 : m >= ceil(2^(31 + j/8))} — exact because m is an integer and 2^(31 + j/8) is not.
+__device__ __forceinline__ uint32_t fine_bin(unsigned long long d) {
+  if (d <= 1ull) return 0u;
+  if (d >> 32) return 255u;
+  const uint32_t d32 = (uint32_t)d;
+  const uint32_t b = 31u - (uint32_t)__clz((int)d32);
+  const uint32_t m = d32 << (31u - b);
+  const uint32_t sub = (m >= 0x8b95c1e4u) + (m >= 0x9837f052u) + (m >= 0xa5fed6aau) + (m >= 0xb504f334u) +
+                       (m >= 0xc5672a12u) + (m >= 0xd744fccbu) + (m >= 0xeac0c6e8u);
+  return 8u * b + sub;
+}
+
+__global__ void __launch_bounds__(256)
+fine_hist_kernel(const uint4* __restrict__ ev, uint64_t n, argus_dims D, uint32_t* __restrict__ hist) {
+  const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    const uint4 lo = __ldcs(ev + 2 * i), hi = __ldcs(ev + 2 * i + 1);
+    const long long start = (long long)(((unsigned long long)hi.y << 32) | hi.x);
+    const long long end = (long long)(((unsigned long long)hi.w << 32) | hi.z);
+    uint32_t key;
+    if (!argus_event_key(D, lo.x, lo.y, lo.z, lo.w >> 16, start, end, key)) continue;
+    atomicAdd(&hist[((size_t)key * D.S + lo.z) * 256u + fine_bin((unsigned long long)(end - start))], 1u);
+  }
+}
+
+// ---- NEXT-1: KDE -> valleys -> filters -> triples, one warp per histogram ---------------------------------
+constexpr int KDE_MAX_BINS = 256;
+struct KdeSmem {
+  double f[KDE_MAX_BINS];
+  uint32_t c[KDE_MAX_BINS];
+};
+
+// hist: n_bins counters of this cell (global, stride 1).  Lanes share the grid points; lane 0 walks the valleys.
+__device__ void kde_cell(const uint32_t* __restrict__ hist, const argus_kde_params& P, KdeSmem& sm,
+                         argus_cluster* __restrict__ out, uint8_t* __restrict__ out_n, double* __restrict__ dens) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t nb = P.n_bins;
+  const double step = 0.6931471805599453 / (double)P.per_octave;     // ln 2 / bins per octave
+  // counts, occupied range, n, mean
+  double n = 0.0, sx = 0.0;
+  uint32_t lo = nb, hi = 0;
+  for (uint32_t b = lane; b < nb; b += 32) {
+    const uint32_t c = hist[b];
+    sm.c[b] = c;
+    sm.f[b] = 0.0;
+    if (c) {
+      n += (double)c;
+      sx += (double)c * (((double)b + 0.5) * step);
+      lo = b < lo ? b : lo;
+      hi = b > hi ? b : hi;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    n += __shfl_xor_sync(FULL, n, o);
+    sx += __shfl_xor_sync(FULL, sx, o);
+  }
+  lo = __reduce_min_sync(FULL, lo);
+  hi = __reduce_max_sync(FULL, hi);
+  __syncwarp();
+  for (uint32_t k = lane; k < P.max_clusters; k += 32) { out[k].count = 0u; out[k].p50_bin = 0; out[k].p99_bin = 0; }
+  if (n == 0.0) {
+    if (lane == 0) *out_n = 0;
+    if (dens) for (uint32_t b = lane; b < nb; b += 32) dens[b] = 0.0;
+    return;
+  }
+  double h = 0.0;
+  if (n >= 2.0 && hi > lo) {            // R26: a single occupied bin (sigma = 0) has no density
+    const double mean = sx / n;
+    double ss = 0.0;
+    for (uint32_t b = lo + lane; b <= hi; b += 32) {
+      const double dx = ((double)b + 0.5) * step - mean;
+      ss += (double)sm.c[b] * dx * dx;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(FULL, ss, o);
+    const double sigma = sqrt(ss / (n - 1.0));                        // R25: sample standard deviation (> 0: two bins)
+    {
+      h = 1.06 * sigma * pow(n, -0.2);                                // Scott's rule
+      const double norm = 1.0 / (n * h * 2.5066282746310002);         // 1 / (n h sqrt(2 pi)): eq. (1), R22
+      // the density is needed where valleys can lie: the occupied range (it is tabulated on the whole grid
+      // only when the caller asks for it)
+      const uint32_t j0 = dens ? 0u : lo, j1 = dens ? nb - 1u : hi;
+      for (uint32_t j = j0 + lane; j <= j1; j += 32) {
+        const double xj = ((double)j + 0.5) * step;
+        double acc = 0.0;
+        for (uint32_t b = lo; b <= hi; ++b) {
+          const uint32_t c = sm.c[b];
+          if (c) {
+            const double u = (xj - ((double)b + 0.5) * step) / h;
+            acc += (double)c * exp(-0.5 * u * u);
+          }
+        }
+        sm.f[j] = acc * norm;
+      }
+    }
+  }
+  __syncwarp();
+  if (dens) for (uint32_t b = lane; b < nb; b += 32) dens[b] = sm.f[b];
+  if (lane == 0) {
+    // valleys (R27), cluster-level filter (R28), spacing filter (R29); then the triples (R30)
+    double need = P.min_frac * n;
+    if ((double)P.min_count > need) need = (double)P.min_count;
+    uint32_t n_out = 0;
+    uint32_t seg_lo = lo;                   // first bin of the current cluster
+    double since = 0.0, right = n;          // samples in [seg_lo, j), samples in [j, hi]
+    uint32_t last_bound = 0;
+    bool have_bound = false;
+    auto emit = [&](uint32_t a, uint32_t b) {          // cluster of the bins [a, b)
+      unsigned long long cnt = 0;
+      for (uint32_t q = a; q < b; ++q) cnt += sm.c[q];
+      if (cnt == 0ull || n_out >= P.max_clusters) return;
+      const unsigned long long t50 = (cnt + 1ull) / 2ull;                     // ceil(0.5 cnt)
+      const unsigned long long t99 = (unsigned long long)ceil(0.99 * (double)cnt);
+      unsigned long long cum = 0;
+      uint32_t p50 = b - 1u, p99 = b - 1u;
+      bool got50 = false, got99 = false;
+      for (uint32_t q = a; q < b; ++q) {
+        cum += sm.c[q];
+        if (!got50 && cum >= t50) { p50 = q; got50 = true; }
+        if (!got99 && cum >= t99) { p99 = q; got99 = true; }
+      }
+      out[n_out].count = (uint32_t)cnt; out[n_out].p50_bin = (uint16_t)p50; out[n_out].p99_bin = (uint16_t)p99;
+      ++n_out;
+    };
+    if (h > 0.0) {
+      for (uint32_t j = lo + 1u; j < hi; ++j) {
+        since += (double)sm.c[j - 1u];
+        right -= (double)sm.c[j - 1u];
+        if (sm.f[j] < sm.f[j - 1u] && sm.f[j] <= sm.f[j + 1u]) {
+          const bool spaced = !have_bound || j - last_bound >= P.min_gap_bins;
+          if (since >= need && right >= need && spaced && n_out + 1u < P.max_clusters) {   // the last slot takes the rest
+            emit(seg_lo, j);
+            seg_lo = j; since = 0.0; last_bound = j; have_bound = true;
+          }
+        }
+      }
+    }
+    emit(seg_lo, hi + 1u);
+    *out_n = (uint8_t)n_out;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+kde_hist_kernel(const uint32_t* __restrict__ hist, uint64_t n_cells, argus_kde_params P, argus_cluster* clusters,
+                uint8_t* n_clusters, double* density) {
+  __shared__ KdeSmem sm[8];
+  const uint64_t cell = (uint64_t)blockIdx.x * 8u + (threadIdx.x >> 5);
+  if (cell >= n_cells) return;
+  kde_cell(hist + cell * P.n_bins, P, sm[threadIdx.x >> 5], clusters + cell * P.max_clusters, n_clusters + cell,
+           density ? density + cell * P.n_bins : nullptr);
+}
+
+// the 32-bucket histograms of the finalised record table (per_octave = 1, n_bins = 32)
+__global__ void __launch_bounds__(256)
+kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_params P, argus_cluster* clusters,
+                   uint8_t* n_clusters) {
+  __shared__ KdeSmem sm[8];
+  const uint64_t cell = (uint64_t)blockIdx.x * 8u + (threadIdx.x >> 5);
+  if (cell >= (uint64_t)D.R * D.T * D.S) return;
+  const uint64_t rec = cell / D.S;
+  const uint32_t sig = (uint32_t)(cell % D.S);
+  const argus_cell* c = reinterpret_cast<const argus_cell*>(records + rec * D.rec_bytes + D.cell_off) + sig;
+  kde_cell(c->hist, P, sm[threadIdx.x >> 5], clusters + cell * P.max_clusters, n_clusters + cell, nullptr);
+}
+
+// ---- NEXT-2: L3 -------------------------------------------------------------------------------------------
+// One CTA per key.  Shared memory: R (value, rank) pairs for the sort, the R scores.
+__device__ __forceinline__ double normal_cdf(double z) { return 0.5 * erfc(-z * 0.7071067811865476); }
+
+extern __shared__ unsigned char l3_smem[];
+
+// bitonic sort of n (power of two) doubles with their payload, ascending; all threads of the CTA call
+__device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
+  for (uint32_t k = 2; k <= n; k <<= 1) {
+    for (uint32_t j = k >> 1; j > 0; j >>= 1) {
+      for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+        const uint32_t p = i ^ j;
+        if (p > i) {
+          const bool up = (i & k) == 0u;
+          const double a = v[i], b = v[p];
+          if ((a > b) == up && a != b) {
+            v[i] = b; v[p] = a;
+            const uint16_t t = id[i]; id[i] = id[p]; id[p] = t;
+          }
+        }
+      }
+      __syncthreads();
+    }
+  }
+}
+
+__global__ void __launch_bounds__(1024)
+l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, argus_l3_stat* __restrict__ stat_out,
+          uint8_t* __restrict__ flags_out) {
+  const uint32_t R = in.n_ranks, C = in.max_clusters, key = blockIdx.x, G = P.n_grid;
+  uint32_t n2 = 1;
+  while (n2 < R) n2 <<= 1;
+  double* val = reinterpret_cast<double*>(l3_smem);                 // [n2]
+  double* score = val + n2;                                         // [R]
+  double* pre = score + R;                                          // [n2] prefix sums of the sorted values
+  uint16_t* id = reinterpret_cast<uint16_t*>(pre + n2);             // [n2]
+  __shared__ double s_red[64];
+  __shared__ double s_lo, s_hi, s_fence;
+  const uint32_t* cnt = in.count + (size_t)key * R * C;
+  const double* p50 = in.p50 + (size_t)key * R * C;
+  const double* p99 = in.p99 + (size_t)key * R * C;
+  // grid bounds (R32): 0.5 * min p50 .. 2 * max p99 over the clusters with count > 0
+  double mn = INFINITY, mx = 0.0;
+  for (uint32_t i = threadIdx.x; i < R * C; i += blockDim.x)
+    if (cnt[i]) { mn = fmin(mn, p50[i]); mx = fmax(mx, p99[i]); }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { mn = fmin(mn, __shfl_xor_sync(FULL, mn, o)); mx = fmax(mx, __shfl_xor_sync(FULL, mx, o)); }
+  if ((threadIdx.x & 31) == 0) { s_red[threadIdx.x >> 5] = mn; s_red[32 + (threadIdx.x >> 5)] = mx; }
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) score[r] = 0.0;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = INFINITY, b = 0.0;
+    for (uint32_t w = 0; w < (blockDim.x + 31u) / 32u; ++w) { a = fmin(a, s_red[w]); b = fmax(b, s_red[32 + w]); }
+    s_lo = a; s_hi = b;
+  }
+  __syncthreads();
+  const bool empty = !(s_hi > 0.0);
+  if (!empty) {
+    const double llo = log(0.5 * s_lo), lhi = log(2.0 * s_hi);
+    for (uint32_t j = 0; j < G; ++j) {
+      const double lx = llo + (lhi - llo) * (double)j / (double)(G - 1u);
+      const double x = exp(lx);
+      // trapezoid weight of grid point j: half the two neighbouring intervals (eq. 3 on a log-uniform grid)
+      const double xm = j ? exp(llo + (lhi - llo) * (double)(j - 1u) / (double)(G - 1u)) : x;
+      const double xp = j + 1u < G ? exp(llo + (lhi - llo) * (double)(j + 1u) / (double)(G - 1u)) : x;
+      const double wj = 0.5 * (xp - xm);
+      // F_r(x_j), eq. (2); log(x) of the oracle is log(exp(lx)): take it the same way
+      const double lgx = log(x);
+      for (uint32_t r = threadIdx.x; r < n2; r += blockDim.x) {
+        double F = INFINITY;                       // padding sorts to the end
+        if (r < R) {
+          double tot = 0.0;
+          for (uint32_t c = 0; c < C; ++c) tot += (double)cnt[r * C + c];
+          F = 0.0;
+          if (tot > 0.0)
+            for (uint32_t c = 0; c < C; ++c) {
+              const uint32_t k = cnt[r * C + c];
+              if (!k) continue;
+              const double mu = log(p50[r * C + c]);
+              const double sg = (log(p99[r * C + c]) - mu) / 2.326;
+              F += (double)k / tot * (sg > 0.0 ? normal_cdf((lgx - mu) / sg) : (lgx >= mu ? 1.0 : 0.0));
+            }
+        }
+        val[r] = F;
+        id[r] = (uint16_t)r;
+      }
+      __syncthreads();
+      bitonic_sort(val, id, n2);
+      // exclusive prefix sums of the sorted values (one thread: R <= 4096 adds per grid point is small next
+      // to the sort) and the total
+      if (threadIdx.x == 0) {
+        double run = 0.0;
+        for (uint32_t i = 0; i < R; ++i) { pre[i] = run; run += val[i]; }
+        s_red[0] = run;
+      }
+      __syncthreads();
+      const double total = s_red[0];
+      // sum_b |F_r - F_b| for the value at sorted position i: F (2 i - R) + total - 2 pre[i]
+      for (uint32_t i = threadIdx.x; i < R; i += blockDim.x) {
+        const double F = val[i];
+        const double S = F * (2.0 * (double)i - (double)R) + total - 2.0 * pre[i];
+        score[id[i]] += wj * S;
+      }
+      __syncthreads();
+    }
+  }
+  // deviation score = mean W1 to the other ranks; quartiles by linear interpolation (R33)
+  const double inv = R > 1u ? 1.0 / (double)(R - 1u) : 1.0;
+  for (uint32_t r = threadIdx.x; r < n2; r += blockDim.x) {
+    if (r < R) {
+      score[r] *= inv;
+      score_out[(size_t)key * R + r] = score[r];
+      val[r] = score[r];
+    } else {
+      val[r] = INFINITY;
+    }
+    id[r] = (uint16_t)r;
+  }
+  __syncthreads();
+  bitonic_sort(val, id, n2);
+  if (threadIdx.x == 0) {
+    auto quant = [&](double q) {
+      const double pos = q * (double)(R - 1u);
+      const uint32_t i0 = (uint32_t)floor(pos);
+      const double fr = pos - (double)i0;
+      const uint32_t i1 = i0 + 1u < R ? i0 + 1u : i0;
+      return val[i0] + fr * (val[i1] - val[i0]);
+    };
+    const double q1 = quant(0.25), q3 = quant(0.75);
+    s_fence = q3 + P.alpha * (q3 - q1);                              // eq. (4)
+    argus_l3_stat st;
+    st.q1 = q1; st.q3 = q3; st.fence = s_fence;
+    st.x_lo = empty ? 1.0 : 0.5 * s_lo; st.x_hi = empty ? 1.0 : 2.0 * s_hi;
+    stat_out[key] = st;
+  }
+  __syncthreads();
+  const double fence = s_fence;
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) flags_out[(size_t)key * R + r] = score[r] > fence ? 1 : 0;
+}
+
+// ---- NEXT-3: L2 ---------------------------------------------------------------------------------------------
+// One CTA per routed event k (phase span, index P = whole iteration): x_r = mean over the T steps of span_ns.
+__global__ void __launch_bounds__(256)
+l2_kernel(const uint8_t* __restrict__ records, argus_dims D, const uint8_t* __restrict__ route,
+          const uint32_t* __restrict__ group_id, double z_thr, argus_l2_group* __restrict__ groups,
+          double* __restrict__ z_out, uint8_t* __restrict__ flag_out, double* __restrict__ xbar_ws) {
+  const uint32_t k = blockIdx.x, R = D.R;
+  const uint32_t* gid = group_id + (size_t)route[k] * R;
+  argus_l2_group* G = groups + (size_t)k * R;
+  double* xb = xbar_ws + (size_t)k * R;
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
+    double s = 0.0;
+    for (uint32_t t = 0; t < D.T; ++t) {
+      const argus_span* sp = reinterpret_cast<const argus_span*>(records + ((size_t)r * D.T + t) * D.rec_bytes + D.span_off) + k;
+      s += (double)sp->span_ns;
+    }
+    xb[r] = s / (double)D.T;
+    argus_l2_group g;
+    g.n = 0u; g.cls = 0u; g.mu = 0.0; g.sigma = 0.0; g.cv = 0.0;
+    G[r] = g;
+  }
+  __syncthreads();
+  // group sums (fp64 L2 atomics: a few thousand adds), then means, then squared deviations
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
+    if (gid[r] >= R) continue;              // not a member of any group of this dimension: z = 0
+    atomicAdd(&G[gid[r]].n, 1u);
+    atomicAdd(&G[gid[r]].mu, xb[r]);
+  }
+  __threadfence();
+  __syncthreads();
+  for (uint32_t g = threadIdx.x; g < R; g += blockDim.x)
+    if (G[g].n) G[g].mu = G[g].mu / (double)G[g].n;
+  __threadfence();
+  __syncthreads();
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
+    if (gid[r] >= R) continue;
+    const double d = xb[r] - G[gid[r]].mu;
+    atomicAdd(&G[gid[r]].sigma, d * d);
+  }
+  __threadfence();
+  __syncthreads();
+  for (uint32_t g = threadIdx.x; g < R; g += blockDim.x) {
+    argus_l2_group q = G[g];
+    if (!q.n) continue;
+    q.sigma = q.n > 1u ? sqrt(q.sigma / (double)(q.n - 1u)) : 0.0;             // eq. (5): |G| - 1
+    q.cv = (q.mu > 0.0 && q.sigma > 0.0) ? q.sigma / q.mu : 0.0;                // R34
+    q.cls = q.cv < 0.02 ? 0u : (q.cv < 0.05 ? 1u : 2u);
+    G[g] = q;
+  }
+  __threadfence();
+  __syncthreads();
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
+    double z = 0.0;
+    if (gid[r] < R) {
+      const argus_l2_group q = G[gid[r]];
+      if (q.sigma > 0.0) z = (xb[r] - q.mu) / q.sigma;
+    }
+    z_out[(size_t)k * R + r] = z;
+    flag_out[(size_t)k * R + r] = z > z_thr ? 1 : 0;
+  }
+}
+
+// ---- NEXT-3: L1, one warp per series -----------------------------------------------------------------------
+__device__ __forceinline__ double series_at(const uint8_t* base, uint64_t sstride, uint64_t tstride, uint32_t s, uint32_t t) {
+  return (double)*reinterpret_cast<const unsigned long long*>(base + (size_t)s * sstride + (size_t)t * tstride);
+}
+
+// median (mean of the two middle values for an even count) of the points of x outside [a, b], by rank counting
+__device__ double median_outside(const double* x, uint32_t T, uint32_t a, uint32_t b) {
+  const int lane = threadIdx.x & 31;
+  const uint32_t n = T - (b - a + 1u);
+  if (n == 0u) return 0.0;
+  const uint32_t k_hi = n / 2u, k_lo = (n & 1u) ? k_hi : k_hi - 1u;
+  double v_lo = 0.0, v_hi = 0.0;
+  for (uint32_t i = lane; i < ((T + 31u) & ~31u); i += 32) {
+    bool f_lo = false, f_hi = false;
+    double v = 0.0;
+    if (i < T && (i < a || i > b)) {
+      v = x[i];
+      uint32_t less = 0, eq = 0;
+      for (uint32_t q = 0; q < T; ++q)
+        if (q < a || q > b) { less += x[q] < v; eq += x[q] == v; }
+      f_lo = less <= k_lo && k_lo < less + eq;
+      f_hi = less <= k_hi && k_hi < less + eq;
+    }
+    const uint32_t m_lo = __ballot_sync(FULL, f_lo), m_hi = __ballot_sync(FULL, f_hi);
+    if (m_lo) v_lo = __shfl_sync(FULL, v, __ffs((int)m_lo) - 1);
+    if (m_hi) v_hi = __shfl_sync(FULL, v, __ffs((int)m_hi) - 1);
+  }
+  return (n & 1u) ? v_hi : 0.5 * (v_lo + v_hi);
+}
+
+extern __shared__ double l1_smem[];
+
+__global__ void __launch_bounds__(128)
+l1_kernel(const uint8_t* __restrict__ base, uint64_t sstride, uint64_t tstride, uint32_t n_series, uint32_t T,
+          argus_l1_params P, argus_l1_out* __restrict__ out) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t s = blockIdx.x * 4u + (uint32_t)w;
+  if (s >= n_series) return;
+  double* x = l1_smem + (size_t)w * (2u * T);               // T values, then T candidate marks (as doubles: 0 / 1)
+  double* mark = x + T;
+  for (uint32_t t = lane; t < T; t += 32) { x[t] = series_at(base, sstride, tstride, s, t); mark[t] = 0.0; }
+  __syncwarp();
+  argus_l1_out o;
+  memset(&o, 0, sizeof o);
+  // ---- jitter, phase 1: windows whose max/min exceeds theta mark their points
+  const uint32_t W = P.window;
+  if (T >= W) {
+    for (uint32_t i = lane; i + W <= T; i += 32) {
+      double mn = x[i], mx = x[i];
+      for (uint32_t q = 1; q < W; ++q) { mn = fmin(mn, x[i + q]); mx = fmax(mx, x[i + q]); }
+      if (mx > P.theta * mn)
+        for (uint32_t q = 0; q < W; ++q) mark[i + q] = 1.0;      // benign race: everybody writes 1
+    }
+  }
+  __syncwarp();
+  // adjacent or overlapping candidate windows merge = maximal runs of marked points; phase 2 per run
+  uint32_t n_int = 0, t0 = 0;
+  bool any_width = false;
+  while (t0 < T) {
+    if (mark[t0] == 0.0) { ++t0; continue; }
+    uint32_t t1 = t0;
+    while (t1 + 1u < T && mark[t1 + 1u] != 0.0) ++t1;
+    const double basel = median_outside(x, T, t0, t1);
+    uint32_t best = 0, run = 0;
+    for (uint32_t t = t0; t <= t1; ++t) {            // every lane walks the run (it is short): uniform result
+      run = x[t] > P.beta * basel ? run + 1u : 0u;
+      best = run > best ? run : best;
+    }
+    if (n_int < ARGUS_L1_MAX_INTERVALS) {
+      o.interval[n_int].first = t0; o.interval[n_int].last = t1; o.interval[n_int].width = best;
+      o.interval[n_int].baseline = basel;
+    }
+    ++n_int;
+    any_width |= best > 0u;
+    t0 = t1 + 1u;
+  }
+  o.n_intervals = n_int;
+  // ---- change point: lanes share the splits, two passes per side as the oracle
+  double best_ratio = 0.0;
+  uint32_t best_t = 0;
+  const uint32_t m = P.min_seg;
+  if (T >= 2u * m) {
+    for (uint32_t t = m + lane; t + m <= T; t += 32) {
+      double sL = 0.0, sR = 0.0;
+      for (uint32_t q = 0; q < t; ++q) sL += x[q];
+      for (uint32_t q = t; q < T; ++q) sR += x[q];
+      const double muL = sL / (double)t, muR = sR / (double)(T - t);
+      if (!(muL > 0.0) || !(muR > 0.0)) continue;
+      double vL = 0.0, vR = 0.0;
+      for (uint32_t q = 0; q < t; ++q) vL += (x[q] - muL) * (x[q] - muL);
+      for (uint32_t q = t; q < T; ++q) vR += (x[q] - muR) * (x[q] - muR);
+      const double sdL = sqrt(vL / (double)(t - 1u)), sdR = sqrt(vR / (double)(T - t - 1u));
+      const double ratio = muR / muL;
+      if (ratio > P.ratio_min && sdL / muL < P.rsd_max && sdR / muR < P.rsd_max && ratio > best_ratio) {
+        best_ratio = ratio; best_t = t;
+      }
+    }
+  }
+  // the largest ratio wins, the earliest split among equals
+#pragma unroll
+  for (int ofs = 16; ofs > 0; ofs >>= 1) {
+    const double r2 = __shfl_xor_sync(FULL, best_ratio, ofs);
+    const uint32_t t2 = __shfl_xor_sync(FULL, best_t, ofs);
+    if (r2 > best_ratio || (r2 == best_ratio && r2 > 0.0 && t2 < best_t)) { best_ratio = r2; best_t = t2; }
+  }
+  o.cp_found = best_ratio > 0.0 ? 1u : 0u;
+  o.cp_step = best_t;
+  o.cp_ratio = best_ratio;
+  o.cls = (any_width ? 1u : 0u) | (o.cp_found ? 2u : 0u);     // stable / jitter / regression / both
+  if (lane == 0) out[s] = o;
+}
+
+}  // namespace
+
+// ---- launchers ---------------------------------------------------------------------------------------------
+cudaError_t argus_launch_fine_hist(argus_ctx* ctx, const argus_event* ev, uint64_t n, uint32_t* d_hist, cudaStream_t s) {
+  if (n == 0) return cudaSuccess;
+  uint64_t blocks = (n + 255) / 256;
+  const uint64_t cap = (uint64_t)ctx->sm_count * 16;
+  if (blocks > cap) blocks = cap;
+  fine_hist_kernel<<<(unsigned)blocks, 256, 0, s>>>(reinterpret_cast<const uint4*>(ev), n, ctx->dims, d_hist);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t argus_launch_kde_hist(argus_ctx* ctx, const uint32_t* d_hist, uint64_t n_cells, const argus_kde_params* P,
+                                  argus_cluster* d_clusters, uint8_t* d_n, double* d_density, cudaStream_t s) {
+  if (n_cells == 0) return cudaSuccess;
+  kde_hist_kernel<<<(unsigned)((n_cells + 7) / 8), 256, 0, s>>>(d_hist, n_cells, *P, d_clusters, d_n, d_density);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t argus_launch_kde_records(argus_ctx* ctx, const void* d_records, const argus_kde_params* P,
+                                     argus_cluster* d_clusters, uint8_t* d_n, cudaStream_t s) {
+  const uint64_t n_cells = (uint64_t)ctx->dims.R * ctx->dims.T * ctx->dims.S;
+  kde_records_kernel<<<(unsigned)((n_cells + 7) / 8), 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, *P,
+                                                                   d_clusters, d_n);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}
+
+size_t argus_l3_smem_bytes(uint32_t R) {
+  uint32_t n2 = 1;
+  while (n2 < R) n2 <<= 1;
+  return sizeof(double) * ((size_t)2 * n2 + R) + sizeof(uint16_t) * n2;
+}
+
+cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,
+                            argus_l3_stat* d_stat, uint8_t* d_flags, cudaStream_t s) {
+  if (in->n_keys == 0) return cudaSuccess;
+  const size_t smem = argus_l3_smem_bytes(in->n_ranks);
+  cudaError_t e = cudaFuncSetAttribute(l3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  l3_kernel<<<in->n_keys, 1024, smem, s>>>(*in, *P, d_score, d_stat, d_flags);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
+                            double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
+                            cudaStream_t s) {
+  l2_kernel<<<ctx->dims.P + 1u, 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, d_route, d_group_id, z_thr,
+                                             d_groups, d_z, d_flags, d_xbar);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t argus_launch_l1(argus_ctx* ctx, const void* d_base, uint64_t sstride, uint64_t tstride, uint32_t n_series,
+                            uint32_t T, const argus_l1_params* P, argus_l1_out* d_out, cudaStream_t s) {
+  if (n_series == 0 || T == 0) return cudaSuccess;
+  const size_t smem = sizeof(double) * 2u * T * 4u;
+  cudaError_t e = cudaFuncSetAttribute(l1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return e;
+  l1_kernel<<<(n_series + 3u) / 4u, 128, smem, s>>>(static_cast<const uint8_t*>(d_base), sstride, tstride, n_series, T, *P,
+                                                   d_out);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}

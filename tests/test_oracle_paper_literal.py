@@ -103,7 +103,7 @@ def test_filters_reject_noise_valleys():
     h2[100], h2[102], h2[104] = 1000, 1000, 1000
     f, bw, bounds, cl = PL.kde_clusters(h2)
     assert bounds == [101] and [c[0] for c in cl] == [1000, 2000]
-    assert PL.kde_clusters(h2, min_gap=0.0)[2] == [101, 103]
+    assert PL.kde_clusters(h2, min_gap_bins=0)[2] == [101, 103]
     # three well separated modes: two boundaries, counts add up, boundaries ascending
     h3 = np.zeros(256, dtype=np.int64)
     h3[80:83] = [300, 500, 300]
