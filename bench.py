@@ -182,7 +182,7 @@ def run_ours(args, world):
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
-    if args.scaling == "strong" and world.size > 1:
+    if args.scaling == "strong":
         from paper_2606_20374_b200 import sharded
         return sharded.bench_strong(args, world, METRIC, measured_peak_gbs, ClockSampler)
     torch.cuda.set_device(world.local_rank)

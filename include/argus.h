@@ -305,6 +305,11 @@ typedef struct argus_l3_in {
 } argus_l3_in;
 typedef struct argus_l3_params { uint32_t n_grid /* >= 2 (256) */; uint32_t reserved; double alpha /* 1.5 */; } argus_l3_params;
 typedef struct argus_l3_stat { double q1, q3, fence, x_lo, x_hi; } argus_l3_stat;
+/* The clusters of argus_kde_clusters(_records) over this ctx's table, [R][T][S][max_clusters], regrouped as
+ * the L3 input of key (t, s): [device] d_count / d_p50 / d_p99 [T*S][R][max_clusters]; a bin becomes the
+ * duration it stands for, 2^((bin + 0.5) / per_octave) ns (R30). */
+int argus_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_clusters, uint32_t max_clusters, uint32_t per_octave,
+                         uint32_t* d_count, double* d_p50, double* d_p99, void* stream);
 /* [device] d_score [n_keys][n_ranks] f64, d_stat [n_keys], d_flags [n_keys][n_ranks] u8. */
 int argus_l3_detect(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* p, double* d_score,
                     argus_l3_stat* d_stat, uint8_t* d_flags, void* stream);

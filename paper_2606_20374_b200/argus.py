@@ -43,7 +43,7 @@ EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_b
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
            "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
            "argus_diagnose_planes", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
-           "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
+           "argus_clusters_to_l3", "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
 
@@ -139,6 +139,8 @@ def load() -> ctypes.CDLL:
     lib.argus_kde_clusters.argtypes = [vp, vp, u64, ctypes.POINTER(ArgusKdeParams), vp, vp, vp, vp]
     lib.argus_kde_clusters_records.restype = i32
     lib.argus_kde_clusters_records.argtypes = [vp, vp, ctypes.POINTER(ArgusKdeParams), vp, vp, vp]
+    lib.argus_clusters_to_l3.restype = i32
+    lib.argus_clusters_to_l3.argtypes = [vp, vp, ctypes.c_uint32, ctypes.c_uint32, vp, vp, vp, vp]
     lib.argus_l3_detect.restype = i32
     lib.argus_l3_detect.argtypes = [vp, ctypes.POINTER(ArgusL3In), ctypes.POINTER(ArgusL3Params), vp, vp, vp, vp]
     lib.argus_l2_groups.restype = i32
@@ -322,6 +324,10 @@ class Argus:
     def kde_clusters_records(self, d_records, params, d_clusters, d_n_clusters, stream=None) -> None:
         self._check(self.lib.argus_kde_clusters_records(self._h, _ptr(d_records), ctypes.byref(params),
                                                         _ptr(d_clusters), _ptr(d_n_clusters), _stream(stream)))
+
+    def clusters_to_l3(self, d_clusters, max_clusters: int, per_octave: int, d_count, d_p50, d_p99, stream=None) -> None:
+        self._check(self.lib.argus_clusters_to_l3(self._h, _ptr(d_clusters), max_clusters, per_octave, _ptr(d_count),
+                                                  _ptr(d_p50), _ptr(d_p99), _stream(stream)))
 
     def l3_detect(self, d_count, d_p50, d_p99, n_keys: int, n_ranks: int, max_clusters: int, d_score, d_stat,
                   d_flags, n_grid: int = 256, alpha: float = 1.5, stream=None) -> None:

@@ -426,6 +426,15 @@ extern "C" int argus_kde_clusters_records(argus_ctx* ctx, const void* d_records,
   return ARGUS_OK;
 }
 
+extern "C" int argus_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_clusters, uint32_t max_clusters,
+                                    uint32_t per_octave, uint32_t* d_count, double* d_p50, double* d_p99, void* stream) {
+  if (!ctx || !d_clusters || !d_count || !d_p50 || !d_p99 || max_clusters == 0 || per_octave == 0) return ARGUS_EINVAL;
+  if (!aligned8(d_clusters) || !aligned8(d_p50) || !aligned8(d_p99) || ((uintptr_t)d_count & 3u)) return ARGUS_EINVAL;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_clusters_to_l3(ctx, d_clusters, max_clusters, per_octave, d_count, d_p50, d_p99, s));
+  return ARGUS_OK;
+}
+
 extern "C" int argus_l3_detect(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* p, double* d_score,
                                argus_l3_stat* d_stat, uint8_t* d_flags, void* stream) {
   if (!ctx || !in || !p || !d_score || !d_stat || !d_flags) return ARGUS_EINVAL;

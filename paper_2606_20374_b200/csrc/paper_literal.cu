@@ -184,6 +184,25 @@ kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_
   kde_cell(c->hist, P, sm[threadIdx.x >> 5], clusters + cell * P.max_clusters, n_clusters + cell, nullptr);
 }
 
+// clusters [R][T][S][mc] (rank-major, as argus_kde_clusters_records writes them) -> the L3 input
+// [key = t*S + s][R][mc]: count, p50, p99 in ns (a bin stands for its geometric centre, R30)
+__global__ void __launch_bounds__(256)
+clusters_to_l3_kernel(const argus_cluster* __restrict__ cl, argus_dims D, uint32_t mc, uint32_t per_octave,
+                      uint32_t* __restrict__ count, double* __restrict__ p50, double* __restrict__ p99) {
+  const uint64_t n = (uint64_t)D.R * D.T * D.S * mc;
+  for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (uint64_t)gridDim.x * blockDim.x) {
+    // o walks the OUTPUT (coalesced writes): o = ((key * R) + r) * mc + c
+    const uint32_t c = (uint32_t)(o % mc);
+    const uint64_t kr = o / mc;
+    const uint32_t r = (uint32_t)(kr % D.R);
+    const uint64_t key = kr / D.R;
+    const argus_cluster q = cl[(((uint64_t)r * D.T * D.S) + key) * mc + c];
+    count[o] = q.count;
+    p50[o] = q.count ? exp2(((double)q.p50_bin + 0.5) / (double)per_octave) : 1.0;
+    p99[o] = q.count ? exp2(((double)q.p99_bin + 0.5) / (double)per_octave) : 1.0;
+  }
+}
+
 // ---- NEXT-2: L3 -------------------------------------------------------------------------------------------
 // One CTA per key.  Shared memory: R (value, rank) pairs for the sort, the R scores.
 __device__ __forceinline__ double normal_cdf(double z) { return 0.5 * erfc(-z * 0.7071067811865476); }
@@ -524,6 +543,14 @@ cudaError_t argus_launch_kde_records(argus_ctx* ctx, const void* d_records, cons
   const uint64_t n_cells = (uint64_t)ctx->dims.R * ctx->dims.T * ctx->dims.S;
   kde_records_kernel<<<(unsigned)((n_cells + 7) / 8), 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, *P,
                                                                    d_clusters, d_n);
+  ctx->n_kernels += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t argus_launch_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_clusters, uint32_t mc, uint32_t per_octave,
+                                        uint32_t* d_count, double* d_p50, double* d_p99, cudaStream_t s) {
+  clusters_to_l3_kernel<<<(unsigned)ctx->sm_count * 8u, 256, 0, s>>>(d_clusters, ctx->dims, mc, per_octave, d_count, d_p50,
+                                                                    d_p99);
   ctx->n_kernels += 1;
   return cudaGetLastError();
 }

@@ -237,7 +237,14 @@ def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
     d_ev.view(torch.int32).view(-1, 8)[:, 0] -= sh.r0
     mode = args.exchange
     peer = None
-    if mode == "p2p":
+    local = None
+    if G == 1:
+        # a world of one: the "exchange" is the pack kernel writing this GPU's own planes (the p2p path with
+        # the local pointers) — runs the whole sharded step on a single-GPU box
+        mode = "local"
+        local = (torch.empty(lay.T * lay.S * lay.R, dtype=torch.int64, device=f"cuda:{dev}"),
+                 torch.empty(lay.T * (lay.P + 1) * lay.R, dtype=torch.int64, device=f"cuda:{dev}"))
+    elif mode == "p2p":
         try:
             peer = PeerPlanes(lay, g, dev)
         except Exception as e:                      # no peer access / symmetric memory on this box
@@ -247,6 +254,10 @@ def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
 
     def step():
         sh.aggregate(d_ev, n)
+        if local is not None:
+            sh.pack_into_planes([local[0].data_ptr()], [local[1].data_ptr()])
+            sh.diagnose(local[0], local[1])
+            return
         if peer is not None:
             peer.barrier()                          # nobody still reads last step's planes
             sh.pack_into_planes(peer.sig_ptrs, peer.span_ptrs)

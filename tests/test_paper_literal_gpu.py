@@ -202,6 +202,65 @@ def test_l3_scores_and_fence(R, C, K, G):
     ctx.close()
 
 
+def test_events_to_l3_end_to_end():
+    """The paper's whole L3 route on one table (PAPER.md:176-198 then 234-251): events -> fine histograms ->
+    clusters (argus_kde_clusters) -> regrouped triples in ns (argus_clusters_to_l3) -> scores, fence, flags
+    (argus_l3_detect), against the oracle chained the same way on the oracle's own histograms.  tiny's
+    injected fault (rank 5 x1.5 on sig 17) must carry the top score of its key in every step."""
+    import torch
+    from paper_2606_20374_b200 import argus as A
+    wl = build_workload(scaled("tiny", n_events=6000))
+    ev = wl.expand_host()
+    R, T, S, P, base = _dims(wl.spec)
+    MC, G = 4, 64
+    ctx = A.Argus(R, T, S, P, base)
+    n_cells = R * T * S
+    hist = torch.zeros(n_cells * 256, dtype=torch.int32, device="cuda")
+    ctx.fine_hist(_cuda(ev.view(np.uint8).reshape(-1)), ev.size, hist)
+    d_c = torch.zeros(n_cells * MC * 8, dtype=torch.uint8, device="cuda")
+    d_n = torch.zeros(n_cells, dtype=torch.uint8, device="cuda")
+    ctx.kde_clusters(hist, n_cells, ctx.kde_params(max_clusters=MC), d_c, d_n)
+    K = T * S
+    d_cnt = torch.full((K * R * MC,), 9, dtype=torch.int32, device="cuda")
+    d_p50 = torch.zeros(K * R * MC, dtype=torch.float64, device="cuda")
+    d_p99 = torch.zeros(K * R * MC, dtype=torch.float64, device="cuda")
+    ctx.clusters_to_l3(d_c, MC, 8, d_cnt, d_p50, d_p99)
+    d_score = torch.zeros(K * R, dtype=torch.float64, device="cuda")
+    d_stat = torch.zeros(K * 5, dtype=torch.float64, device="cuda")
+    d_flags = torch.zeros(K * R, dtype=torch.uint8, device="cuda")
+    ctx.l3_detect(d_cnt, d_p50, d_p99, K, R, MC, d_score, d_stat, d_flags, n_grid=G, alpha=1.5)
+    cnt = d_cnt.cpu().numpy().view(np.uint32).reshape(K, R, MC)
+    p50 = d_p50.cpu().numpy().reshape(K, R, MC)
+    p99 = d_p99.cpu().numpy().reshape(K, R, MC)
+    score = d_score.cpu().numpy().reshape(K, R)
+    flags = d_flags.cpu().numpy().reshape(K, R)
+    stat = d_stat.cpu().numpy().view(A.L3_STAT_DTYPE).reshape(K)
+    H = PL.fine_histograms(ev, R, T, S, P, base)
+    for t in range(T):
+        for s in range(S):
+            k = t * S + s
+            tr = []
+            for r in range(R):
+                cl = PL.kde_clusters(H[r, t, s], max_clusters=MC)[3]
+                tr.append([(c, PL.bin_value_ns(b50), PL.bin_value_ns(b99)) for c, b50, b99 in cl])
+                for j in range(MC):                       # the regrouped triples themselves
+                    if j < len(cl):
+                        assert int(cnt[k, r, j]) == cl[j][0]
+                        assert p50[k, r, j] == pytest.approx(tr[r][j][1], rel=1e-14)
+                        assert p99[k, r, j] == pytest.approx(tr[r][j][2], rel=1e-14)
+                    else:
+                        assert int(cnt[k, r, j]) == 0
+            xs, F, W, want, q1, q3, fence, wflags = PL.l3_scores(tr, n_grid=G, alpha=1.5)
+            scale = max(1e-300, float(np.abs(want).max()))
+            assert np.allclose(score[k], want, rtol=1e-8, atol=1e-9 * scale), k
+            assert stat[k]["fence"] == pytest.approx(fence, rel=1e-8, abs=1e-9 * scale)
+            clear = np.abs(want - fence) > 1e-7 * scale
+            assert (flags[k][clear] == wflags[clear]).all(), k
+    for t in range(T):
+        assert int(np.argmax(score[t * S + 17])) == 5 and flags[t * S + 17, 5] == 1
+    ctx.close()
+
+
 # ---- NEXT-3 -------------------------------------------------------------------------------------------
 def test_l2_groups_on_a_table():
     import torch
