@@ -176,3 +176,68 @@ def check_handworked(g, cells_arr, spans_arr, n_valid, n_invalid, diag):
         assert list(diag["span_flags"][0, k]) == fl
     assert list(diag["rank_score"][0]) == g["rs"]
     assert list(diag["step_anomalous"]) == g["sa"]
+
+
+# ---- compact encodings (R37 sparse, R38 triple) -----------------------------------------------------
+def parse_compact_golden():
+    """tests/golden/compact_handworked.txt -> dict(sparse={rank: bytes}, triple={rank: bytes},
+    clusters={(rank, sig): [(count, p50, p99)...]})."""
+    import struct
+    out = dict(sparse={}, triple={}, clusters={})
+    cur = None
+    with open(os.path.join(GOLDEN, "compact_handworked.txt")) as f:
+        for line in f:
+            p = line.split()
+            if not p or p[0].startswith("#"):
+                continue
+            if p[0] in ("SPARSE", "TRIPLE"):
+                cur = out[p[0].lower()].setdefault(int(p[1]), bytearray())
+            elif p[0] == "CLUSTERS":
+                v = [int(x) for x in p[3:]]
+                out["clusters"][(int(p[1]), int(p[2]))] = [tuple(v[i:i + 3]) for i in range(0, len(v), 3)]
+            else:
+                cur += struct.pack("<" + p[0], *[int(x, 0) for x in p[1:]])
+    return out
+
+
+def sparse_to_dense(stream: bytes, offsets, S: int, P: int) -> np.ndarray:
+    """An independent READER of the R37 sparse stream (walks it with an explicit cursor and rebuilds the dense
+    R17 table, identities of R7 for what the stream leaves out) — used to pin the oracle's writer."""
+    import struct
+    rb = 64 + 32 * (P + 1) + 160 * S
+    table = np.zeros((len(offsets) - 1, rb), dtype=np.uint8)
+    for k in range(len(offsets) - 1):
+        pos, end = offsets[k], offsets[k + 1]
+        magic, ver, n_ph, n_sg, rank, step, n_cells, n_ev, mn, mx, it, length = struct.unpack_from("<IHHIIIIQqqQQ", stream, pos)
+        assert (magic, ver, n_ph, n_sg, length) == (0x53475241, 2, P, S, end - pos)
+        rec = bytearray(rb)
+        struct.pack_into("<IHHIIIIQqqQQ", rec, 0, magic, 1, n_ph, n_sg, rank, step, 0, n_ev, mn, mx, it, 0)
+        for j in range(P):
+            struct.pack_into("<qqQQ", rec, 64 + 32 * j, I64_MAX, I64_MIN, 0, 0)
+        struct.pack_into("<qqQQ", rec, 64 + 32 * P, mn, mx, it, n_ev)
+        for s in range(S):
+            struct.pack_into("<QQQQ", rec, 64 + 32 * (P + 1) + 160 * s, 0, 0, U64_MAX, 0)
+        pos += 64
+        mask, = struct.unpack_from("<Q", stream, pos)
+        pos += 8
+        for j in range(P):
+            if mask >> j & 1:
+                rec[64 + 32 * j: 96 + 32 * j] = stream[pos:pos + 32]
+                pos += 32
+        assert mask >> P == 0
+        last = -1
+        for _ in range(n_cells):
+            s, b0, nb, z = struct.unpack_from("<IBBH", stream, pos)
+            assert s > last and z == 0 and 1 <= nb and b0 + nb <= 32
+            last = s
+            c0 = 64 + 32 * (P + 1) + 160 * s
+            rec[c0:c0 + 32] = stream[pos + 8: pos + 40]
+            hist = struct.unpack_from("<%dI" % nb, stream, pos + 40)
+            struct.pack_into("<%dI" % nb, rec, c0 + 32 + 4 * b0, *hist)
+            pos += 40 + 4 * nb
+            if nb & 1:
+                assert struct.unpack_from("<I", stream, pos)[0] == 0
+                pos += 4
+        assert pos == end, (k, pos, end)
+        table[k] = np.frombuffer(bytes(rec), dtype=np.uint8)
+    return table
