@@ -258,6 +258,30 @@ int argus_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t sig_lo, ui
  * step_anomalous [T]; T and P are the ctx's, R = planes->n_ranks.  [host] planes, [host] outs. */
 int argus_diagnose_planes(argus_ctx* ctx, const argus_planes* planes, const argus_diag_out* outs, void* stream);
 
+/* ---- compact record encodings (second half: "sparse/bit-packed record encoding (non-empty
+ * bins only) to raise the compression ratio"; the paper's per-rank record of "approximately 200 triples ... about
+ * 2.7 KB").  Both turn this ctx's FINALISED table (argus_phase_times ran; ARGUS_ESTATE otherwise)
+ * into one byte stream of variable-length records in (rank, step) order; every field little-endian, every part
+ * 8-byte aligned.  Record k occupies [d_offsets[k], d_offsets[k+1]) of d_out; d_offsets[R*T] = total length.
+ *   SPARSE (R37, lossless):
+ *     argus_record_header   version = 2, reserved0 = number of non-empty cells, reserved1 = byte length of the record
+ *     u64 phase_mask        bit k: phase span k (k < P) has n_events != 0 (the whole-iteration span is in the header)
+ *     argus_span            one per set bit, ascending k
+ *     per non-empty cell (count != 0), ascending sig:
+ *       u32 sig | u8 b0 | u8 nb | u16 0         b0 = bucket(min_ns), nb = bucket(max_ns) - b0 + 1
+ *       u64 count | u64 sum_ns | u64 min_ns | u64 max_ns
+ *       u32 hist[b0 .. b0 + nb) | u32 0 when nb is odd
+ *   TRIPLE (R38, the paper's (count, p50, p99) record; lossy: what NEXT-1 keeps of a cell):
+ *     argus_record_header   version = 3, reserved0 = number of cells with >= 1 cluster, reserved1 = byte length
+ *     u64 phase_mask + spans as above
+ *     per cell with n_clusters > 0, ascending sig:  u32 sig | u32 n_clusters | n_clusters x argus_cluster
+ * [device] d_out (8-byte aligned, out_capacity bytes), [device] d_offsets [R*T + 1] u64.  A record that would end
+ * beyond out_capacity is not written (d_offsets is still complete: compare d_offsets[R*T] with out_capacity);
+ * argus_sparse_bound / argus_triple_bound give a capacity that always suffices.  Asynchronous on `stream`. */
+size_t argus_sparse_bound(const argus_config* cfg);
+int argus_sparse_encode(argus_ctx* ctx, const void* d_records, uint8_t* d_out, uint64_t out_capacity,
+                        uint64_t* d_offsets, void* stream);
+
 /* ==== the paper's own float algorithms (SURVEY 8(f) NEXT-1..3), fp64; every constant the paper leaves open
  * is a parameter whose default is a reading of DESIGN.md 3 (R23-R36) ================================== */
 
@@ -292,6 +316,13 @@ int argus_kde_clusters(argus_ctx* ctx, const uint32_t* d_hist, uint64_t n_cells,
  * d_clusters [R][T][S][max_clusters], d_n_clusters [R][T][S].  No pass over the events. */
 int argus_kde_clusters_records(argus_ctx* ctx, const void* d_records, const argus_kde_params* p,
                                argus_cluster* d_clusters, uint8_t* d_n_clusters, void* stream);
+
+/* The TRIPLE record stream (layout above) from the clusters of argus_kde_clusters(_records) over this ctx's
+ * table: [device] d_clusters [R][T][S][max_clusters], d_n_clusters [R][T][S]. */
+size_t argus_triple_bound(const argus_config* cfg, uint32_t max_clusters);
+int argus_triple_encode(argus_ctx* ctx, const void* d_records, const argus_cluster* d_clusters,
+                        const uint8_t* d_n_clusters, uint32_t max_clusters, uint8_t* d_out, uint64_t out_capacity,
+                        uint64_t* d_offsets, void* stream);
 
 /* ---- NEXT-2: L3 kernel-statistics anomaly detection (eq. 2-4) -------------------------
  * Per key (kernel): every rank's clusters (count, p50, p99) -> log-normal mixture CDF (mu = ln p50,

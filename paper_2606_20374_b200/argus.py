@@ -43,6 +43,7 @@ EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_b
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
            "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
            "argus_diagnose_planes", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
+           "argus_sparse_bound", "argus_sparse_encode", "argus_triple_bound", "argus_triple_encode",
            "argus_clusters_to_l3", "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
@@ -139,6 +140,14 @@ def load() -> ctypes.CDLL:
     lib.argus_kde_clusters.argtypes = [vp, vp, u64, ctypes.POINTER(ArgusKdeParams), vp, vp, vp, vp]
     lib.argus_kde_clusters_records.restype = i32
     lib.argus_kde_clusters_records.argtypes = [vp, vp, ctypes.POINTER(ArgusKdeParams), vp, vp, vp]
+    lib.argus_sparse_bound.restype = ctypes.c_size_t
+    lib.argus_sparse_bound.argtypes = [ctypes.POINTER(ArgusConfig)]
+    lib.argus_triple_bound.restype = ctypes.c_size_t
+    lib.argus_triple_bound.argtypes = [ctypes.POINTER(ArgusConfig), ctypes.c_uint32]
+    lib.argus_sparse_encode.restype = i32
+    lib.argus_sparse_encode.argtypes = [vp, vp, vp, u64, vp, vp]
+    lib.argus_triple_encode.restype = i32
+    lib.argus_triple_encode.argtypes = [vp, vp, vp, vp, ctypes.c_uint32, vp, u64, vp, vp]
     lib.argus_clusters_to_l3.restype = i32
     lib.argus_clusters_to_l3.argtypes = [vp, vp, ctypes.c_uint32, ctypes.c_uint32, vp, vp, vp, vp]
     lib.argus_l3_detect.restype = i32
@@ -324,6 +333,21 @@ class Argus:
     def kde_clusters_records(self, d_records, params, d_clusters, d_n_clusters, stream=None) -> None:
         self._check(self.lib.argus_kde_clusters_records(self._h, _ptr(d_records), ctypes.byref(params),
                                                         _ptr(d_clusters), _ptr(d_n_clusters), _stream(stream)))
+
+    def sparse_bound(self) -> int:
+        return int(self.lib.argus_sparse_bound(ctypes.byref(self.cfg)))
+
+    def triple_bound(self, max_clusters: int) -> int:
+        return int(self.lib.argus_triple_bound(ctypes.byref(self.cfg), max_clusters))
+
+    def sparse_encode(self, d_records, d_out, d_offsets, stream=None) -> None:
+        self._check(self.lib.argus_sparse_encode(self._h, _ptr(d_records), _ptr(d_out), d_out.numel() * d_out.element_size(),
+                                                 _ptr(d_offsets), _stream(stream)))
+
+    def triple_encode(self, d_records, d_clusters, d_n_clusters, max_clusters: int, d_out, d_offsets, stream=None) -> None:
+        self._check(self.lib.argus_triple_encode(self._h, _ptr(d_records), _ptr(d_clusters), _ptr(d_n_clusters), max_clusters,
+                                                 _ptr(d_out), d_out.numel() * d_out.element_size(), _ptr(d_offsets),
+                                                 _stream(stream)))
 
     def clusters_to_l3(self, d_clusters, max_clusters: int, per_octave: int, d_count, d_p50, d_p99, stream=None) -> None:
         self._check(self.lib.argus_clusters_to_l3(self._h, _ptr(d_clusters), max_clusters, per_octave, _ptr(d_count),

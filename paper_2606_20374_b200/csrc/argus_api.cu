@@ -426,6 +426,36 @@ extern "C" int argus_kde_clusters_records(argus_ctx* ctx, const void* d_records,
   return ARGUS_OK;
 }
 
+extern "C" size_t argus_sparse_bound(const argus_config* c) {
+  if (!cfg_ok(c)) return 0;
+  return (size_t)c->n_ranks * c->n_steps * (72u + 32u * (size_t)c->n_phases + 168u * (size_t)c->n_sigs);
+}
+
+extern "C" size_t argus_triple_bound(const argus_config* c, uint32_t max_clusters) {
+  if (!cfg_ok(c) || max_clusters == 0) return 0;
+  return (size_t)c->n_ranks * c->n_steps * (72u + 32u * (size_t)c->n_phases + (8u + 8u * (size_t)max_clusters) * c->n_sigs);
+}
+
+extern "C" int argus_sparse_encode(argus_ctx* ctx, const void* d_records, uint8_t* d_out, uint64_t out_capacity,
+                                   uint64_t* d_offsets, void* stream) {
+  if (!ctx || !d_records || !d_out || !d_offsets || !aligned8(d_out) || !aligned8(d_offsets)) return ARGUS_EINVAL;
+  if (d_records == ctx->d_records && !ctx->finalized) return ARGUS_ESTATE;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_sparse_encode(ctx, d_records, d_out, out_capacity, d_offsets, s));
+  return ARGUS_OK;
+}
+
+extern "C" int argus_triple_encode(argus_ctx* ctx, const void* d_records, const argus_cluster* d_clusters,
+                                   const uint8_t* d_n_clusters, uint32_t max_clusters, uint8_t* d_out,
+                                   uint64_t out_capacity, uint64_t* d_offsets, void* stream) {
+  if (!ctx || !d_records || !d_clusters || !d_n_clusters || !d_out || !d_offsets || max_clusters == 0) return ARGUS_EINVAL;
+  if (!aligned8(d_clusters) || !aligned8(d_out) || !aligned8(d_offsets)) return ARGUS_EINVAL;
+  if (d_records == ctx->d_records && !ctx->finalized) return ARGUS_ESTATE;
+  ARGUS_ENTER(ctx, stream);
+  CU(ctx, argus_launch_triple_encode(ctx, d_records, d_clusters, d_n_clusters, max_clusters, d_out, out_capacity, d_offsets, s));
+  return ARGUS_OK;
+}
+
 extern "C" int argus_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_clusters, uint32_t max_clusters,
                                     uint32_t per_octave, uint32_t* d_count, double* d_p50, double* d_p99, void* stream) {
   if (!ctx || !d_clusters || !d_count || !d_p50 || !d_p99 || max_clusters == 0 || per_octave == 0) return ARGUS_EINVAL;

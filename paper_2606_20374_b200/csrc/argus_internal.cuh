@@ -94,6 +94,11 @@ cudaError_t argus_launch_kde_records(argus_ctx* ctx, const void* d_records, cons
                                      argus_cluster* d_clusters, uint8_t* d_n, cudaStream_t s);
 cudaError_t argus_launch_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_clusters, uint32_t mc, uint32_t per_octave,
                                         uint32_t* d_count, double* d_p50, double* d_p99, cudaStream_t s);
+cudaError_t argus_launch_sparse_encode(argus_ctx* ctx, const void* d_records, uint8_t* d_out, uint64_t capacity,
+                                       uint64_t* d_offsets, cudaStream_t s);
+cudaError_t argus_launch_triple_encode(argus_ctx* ctx, const void* d_records, const argus_cluster* d_clusters,
+                                       const uint8_t* d_n_clusters, uint32_t mc, uint8_t* d_out, uint64_t capacity,
+                                       uint64_t* d_offsets, cudaStream_t s);
 size_t argus_l3_smem_bytes(uint32_t R);
 cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,
                             argus_l3_stat* d_stat, uint8_t* d_flags, cudaStream_t s);
