@@ -53,10 +53,19 @@ void argus_ws_plan(const argus_config* c, int sm_count, int max_smem_optin, argu
   L->sums = o;      o += up256(sizeof(unsigned long long) * RT * c->n_sigs);
   L->ovf = o;       o += up256((size_t)ARGUS_MAX_SEG_CTAS * ARGUS_OVF_CAP * sizeof(uint4));
   L->diag_todo = o; o += up256((size_t)c->n_steps * ((size_t)c->n_sigs + c->n_phases + 1u));
-  L->part = o; L->group = o; L->part_ctas = 0; L->part_smem = false;
+  L->part = o; L->group = o; L->coarse = o; L->part_ctas = 0; L->part_smem = false;
+  L->part_two_level = false; L->part_shift = 0;
   if (c->max_ungrouped_events) {
-    argus_partition_plan(c, sm_count, max_smem_optin, &L->part_ctas, &L->part_smem);
-    if (L->part_smem) o += up256(sizeof(uint32_t) * (size_t)L->part_ctas * (RT + 1u));
+    size_t small = 0;
+    L->part_two_level = (size_t)max_smem_optin >= 100u * 1024u && argus_partition2_plan(c, &L->part_shift, &small);
+    if (L->part_two_level) {
+      o += up256(small);
+      L->coarse = o;
+      o += up256((size_t)c->max_ungrouped_events * 16u);
+    } else {
+      argus_partition_plan(c, sm_count, max_smem_optin, &L->part_ctas, &L->part_smem);
+      if (L->part_smem) o += up256(sizeof(uint32_t) * (size_t)L->part_ctas * (RT + 1u));
+    }
     L->group = o;
     o += up256((size_t)c->max_ungrouped_events * sizeof(argus_event));
   }
@@ -128,7 +137,8 @@ extern "C" int argus_create(const argus_config* cfg, void* d_workspace, size_t w
       ctx->d_spill = ctx->d_ws + L.spill;
     }
     if (cfg->max_ungrouped_events) {
-      ctx->d_part = L.part_smem ? reinterpret_cast<uint32_t*>(ctx->d_ws + L.part) : nullptr;
+      ctx->d_part = (L.part_smem || L.part_two_level) ? reinterpret_cast<uint32_t*>(ctx->d_ws + L.part) : nullptr;
+      ctx->d_coarse = L.part_two_level ? ctx->d_ws + L.coarse : nullptr;
       ctx->d_group = reinterpret_cast<argus_event*>(ctx->d_ws + L.group);
     }
     cudaDriverEntryPointQueryResult q;

@@ -31,8 +31,11 @@ struct argus_dims {
 #define ARGUS_OVF_CAP 4096u           // entries (16 B) of one CTA's overflow list
 struct argus_ws_layout {
   size_t state, counters, hist, sums, ovf, diag_todo, part, group, spill_cnt, spill, total;
+  size_t coarse;                      // two-level grouping: the packed events grouped by coarse bin (16 B per event)
   uint32_t part_ctas;                 // CTAs of the grouping pass (0: no grouping area)
   bool part_smem;                     // its key histograms fit shared memory
+  bool part_two_level;                // two-level grouping (partition.cu) instead of the single scatter
+  uint32_t part_shift;                // keys per coarse bin = 2^part_shift
 };
 void argus_ws_plan(const argus_config* cfg, int sm_count, int max_smem_optin, argus_ws_layout* out);
 
@@ -49,7 +52,9 @@ struct argus_ctx {
   uint32_t* d_hist;           // [R*T + 1] group sizes / cursors of the grouping pass
   argus_event* d_group;       // grouping area [cfg.max_ungrouped_events] (null when 0)
   void* fn_tmap_encode;       // cuTensorMapEncodeTiled, resolved through the runtime (no libcuda link)
-  uint32_t* d_part;           // per-CTA key histograms of the grouping pass [part_ctas][R*T + 1]
+  uint32_t* d_part;           // per-CTA key histograms of the grouping pass [part_ctas][R*T + 1], or the small
+                              // state of the two-level pass
+  uint8_t* d_coarse;          // two-level grouping: coarse area [cfg.max_ungrouped_events] x 16 B
   uint8_t* d_diag_todo;       // argus_diagnose: one byte per series, set by the 32-bit pass for the 64-bit pass
   uint8_t* d_spill;           // spill regions of the segmented kernel [cfg.max_spill_events] raw events (null when 0)
   uint32_t* d_spill_cnt;      // events re-queued by each CTA of the last segmented launch [ARGUS_MAX_SEG_CTAS]
@@ -110,6 +115,7 @@ cudaError_t argus_launch_l1(argus_ctx* ctx, const void* d_base, uint64_t sstride
 bool argus_seg_supported(const argus_ctx* ctx);
 void argus_partition_plan(const argus_config* cfg, int sm_count, int max_smem_optin, uint32_t* n_cta,
                           bool* smem);
+bool argus_partition2_plan(const argus_config* cfg, uint32_t* shift, size_t* small_bytes);
 // opt-in shared-memory sizes of the kernels this ctx will launch (argus_create, once)
 cudaError_t argus_configure_seg(argus_ctx* ctx);
 cudaError_t argus_configure_partition(argus_ctx* ctx);

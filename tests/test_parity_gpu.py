@@ -233,9 +233,56 @@ def test_device_expander_matches_host():
 
 def test_grouping_with_many_groups():
     # R*T + 1 = 65,537 group counters do not fit shared memory: the grouping pass falls back to one
-    # global counter array (L2 atomics); R*T = 3,000 uses the per-CTA shared-memory histograms
+    # global counter array (L2 atomics); R*T = 32,768 uses the single scatter with per-CTA shared-memory
+    # histograms; R*T = 3,000 the two-level grouping
     rnd = random.Random(5)
-    for R, T in ((8192, 8), (1000, 3)):
+    for R, T in ((8192, 8), (16384, 2), (1000, 3)):
         rows = [(rnd.randrange(R + 1), 3 + rnd.randrange(T + 1), rnd.randrange(4), 0, rnd.randrange(2),
                  rnd.randrange(10**6), 10**6 + rnd.randrange(10**5)) for _ in range(30000)]
         assert_parity(make_events(rows), R, T, 4, 2, 3, sorted_hint=False)
+
+
+def test_two_level_grouping_edges():
+    """Ungrouped input through the two-level grouping pass: durations of 2^32 ns and more (they bypass the packed
+    16-byte form), invalid events of every kind (dropped by the pass, re-appear as padding and must still be
+    counted), a call of a few events, one whose events are all invalid, one whose events all bypass, a key
+    count that is not a power of two, and several tiles per coarse bin."""
+    rnd = random.Random(11)
+    R, T, S, P, base = 37, 3, 50, 5, 1000
+    rows = []
+    for i in range(60_000):
+        r, t, sg, ph = rnd.randrange(R), base + rnd.randrange(T), rnd.randrange(S), rnd.randrange(P)
+        a = rnd.randrange(10**9)
+        d = rnd.randrange(1, 10**5)
+        k = rnd.random()
+        if k < 0.02:
+            d = (1 << 32) + rnd.randrange(1 << 33)              # bypasses the packed form
+        elif k < 0.03:
+            d = (1 << 32) - 1 - rnd.randrange(2)                # the largest packable durations
+        elif k < 0.04:
+            r = R + rnd.randrange(3)
+        elif k < 0.05:
+            t = base - 1 - rnd.randrange(2)
+        elif k < 0.06:
+            sg = S + rnd.randrange(100)
+        elif k < 0.07:
+            ph = P
+        elif k < 0.08:
+            a = -1 - rnd.randrange(100)
+        elif k < 0.09:
+            d = -1 - rnd.randrange(50)
+        rows.append((r, t, sg, rnd.randrange(9), ph, a, a + d))
+    ev = make_events(rows)
+    assert_parity(ev, R, T, S, P, base, sorted_hint=False)
+    assert_parity(ev, R, T, S, P, base, sorted_hint=False, cuts=[0, 3, 2051, 2052, 40_000, ev.size])
+    bad = ev.copy()
+    bad["sig"] = S + 1
+    assert_parity(bad[:5000], R, T, S, P, base, sorted_hint=False)
+    big = ev[(ev["end_ns"] - ev["start_ns"]) >= (1 << 32)]
+    assert big.size > 500
+    assert_parity(big, R, T, S, P, base, sorted_hint=False)
+    one = ev.copy()                                              # every event in ONE key: a single coarse bin, 30 tiles
+    one["rank"] = 7
+    one["step"] = base + 1
+    assert_parity(one, R, T, S, P, base, sorted_hint=False)
+    assert_parity(ev[:1], R, T, S, P, base, sorted_hint=False)
