@@ -229,6 +229,72 @@ __device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
   }
 }
 
+// Sum over b of |v_i - v_b| for every position i of the ascending array v[0..R) — the per-grid-point term of
+// the mean-W1 score — from the GAPS g_i = v[i+1] - v[i] >= 0:  D_0 = sum_i g_i (R - 1 - i),
+// D_{i+1} = D_i + g_i (2 i + 2 - R).  Every term is a gap times an integer, so ranks with identical CDF values
+// get exactly equal sums (0 when all are equal); the prefix form F (2 i - R) + total - 2 pre[i] cancels instead.
+// Block-wide: every thread owns PER consecutive positions; returns D of its positions in d[].
+template <int PER>
+__device__ __forceinline__ void abs_dev_sums(const double* v, uint32_t R, double* s_w, double* d) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const uint32_t i0 = threadIdx.x * PER;
+  double h[PER], hsum = 0.0, d0 = 0.0;
+#pragma unroll
+  for (int k = 0; k < PER; ++k) {
+    const uint32_t i = i0 + k;
+    double g = 0.0;
+    if (i + 1u < R) g = v[i + 1u] - v[i];
+    h[k] = g * (double)((long long)(2u * i + 2u) - (long long)R);
+    d0 += g * (double)(R - 1u - (i < R ? i : R - 1u));
+    hsum += h[k];
+  }
+  // inclusive warp scans of hsum, warp totals of both
+  double inc = hsum, tot0 = d0;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const double t = __shfl_up_sync(FULL, inc, o);
+    if (lane >= o) inc += t;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) tot0 += __shfl_xor_sync(FULL, tot0, o);
+  if (lane == 31) s_w[warp] = inc;
+  if (lane == 0) s_w[32 + warp] = tot0;
+  __syncthreads();
+  double before = 0.0, D0 = 0.0;
+  for (int w = 0; w < nw; ++w) {
+    if (w < warp) before += s_w[w];
+    D0 += s_w[32 + w];
+  }
+  double run = D0 + before + inc - hsum;          // D at this thread's first position
+#pragma unroll
+  for (int k = 0; k < PER; ++k) { d[k] = run; run += h[k]; }
+  __syncthreads();                                 // s_w is reused by the next grid point
+}
+
+// One CTA of 1024 threads per key; R <= 4096: every thread owns at most 4 ranks (CDF evaluation) and at most 4
+// sorted positions.  Per (rank, cluster) the log-normal parameters mu = ln p50, 1/sigma and the weight are
+// computed once per key and kept in registers when the key has at most L3_CACHE (rank, cluster) pairs per thread
+// (C = 1 at R = 4096, C <= 4 at R <= 1024), else recomputed per grid point.
+constexpr int L3_CACHE = 4;
+struct L3Par { double mu, isg, w; };               // isg = 1/sigma, 0 = a step at mu (R31)
+
+__device__ __forceinline__ L3Par l3_par(uint32_t k, double tot, double p50, double p99) {
+  L3Par q;
+  q.mu = log(p50);
+  const double sg = (log(p99) - q.mu) / 2.326;
+  q.isg = sg > 0.0 ? 1.0 / sg : 0.0;
+  q.w = (double)k / tot;
+  return q;
+}
+// w Phi((lgx - mu) / sigma); |z| > 8.3: Phi differs from 0 / 1 by < 6e-17 (below half an ulp of the sums it enters)
+__device__ __forceinline__ double l3_term(const L3Par& q, double lgx) {
+  if (q.isg == 0.0) return lgx >= q.mu ? q.w : 0.0;
+  const double z = (lgx - q.mu) * q.isg;
+  if (z < -8.3) return 0.0;
+  if (z > 8.3) return q.w;
+  return q.w * normal_cdf(z);
+}
+
 __global__ void __launch_bounds__(1024)
 l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, argus_l3_stat* __restrict__ stat_out,
           uint8_t* __restrict__ flags_out) {
@@ -237,8 +303,7 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
   while (n2 < R) n2 <<= 1;
   double* val = reinterpret_cast<double*>(l3_smem);                 // [n2]
   double* score = val + n2;                                         // [R]
-  double* pre = score + R;                                          // [n2] prefix sums of the sorted values
-  uint16_t* id = reinterpret_cast<uint16_t*>(pre + n2);             // [n2]
+  uint16_t* id = reinterpret_cast<uint16_t*>(score + R);            // [n2]
   __shared__ double s_red[64];
   __shared__ double s_lo, s_hi, s_fence;
   const uint32_t* cnt = in.count + (size_t)key * R * C;
@@ -261,6 +326,26 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
   __syncthreads();
   const bool empty = !(s_hi > 0.0);
   if (!empty) {
+    // per-thread totals and, when they fit, the cached parameters of this thread's (rank, cluster) pairs
+    const uint32_t per_thread = (n2 + blockDim.x - 1u) / blockDim.x;      // ranks per thread, <= 4
+    const bool cached = per_thread * C <= (uint32_t)L3_CACHE;
+    L3Par par[L3_CACHE];
+    double tot[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const uint32_t r = threadIdx.x + (uint32_t)a * blockDim.x;
+      if (r < R)
+        for (uint32_t c = 0; c < C; ++c) tot[a] += (double)cnt[r * C + c];
+    }
+    if (cached) {
+#pragma unroll
+      for (int q = 0; q < L3_CACHE; ++q) {
+        const uint32_t a = (uint32_t)q / C, c = (uint32_t)q % C;
+        const uint32_t r = threadIdx.x + a * blockDim.x;
+        par[q].mu = 0.0; par[q].isg = 0.0; par[q].w = 0.0;
+        if (a < per_thread && r < R && cnt[r * C + c]) par[q] = l3_par(cnt[r * C + c], tot[a], p50[r * C + c], p99[r * C + c]);
+      }
+    }
     const double llo = log(0.5 * s_lo), lhi = log(2.0 * s_hi);
     for (uint32_t j = 0; j < G; ++j) {
       const double lx = llo + (lhi - llo) * (double)j / (double)(G - 1u);
@@ -271,40 +356,42 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
       const double wj = 0.5 * (xp - xm);
       // F_r(x_j), eq. (2); log(x) of the oracle is log(exp(lx)): take it the same way
       const double lgx = log(x);
-      for (uint32_t r = threadIdx.x; r < n2; r += blockDim.x) {
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        const uint32_t r = threadIdx.x + (uint32_t)a * blockDim.x;
+        if (r >= n2) break;
         double F = INFINITY;                       // padding sorts to the end
         if (r < R) {
-          double tot = 0.0;
-          for (uint32_t c = 0; c < C; ++c) tot += (double)cnt[r * C + c];
           F = 0.0;
-          if (tot > 0.0)
-            for (uint32_t c = 0; c < C; ++c) {
-              const uint32_t k = cnt[r * C + c];
-              if (!k) continue;
-              const double mu = log(p50[r * C + c]);
-              const double sg = (log(p99[r * C + c]) - mu) / 2.326;
-              F += (double)k / tot * (sg > 0.0 ? normal_cdf((lgx - mu) / sg) : (lgx >= mu ? 1.0 : 0.0));
+          if (tot[a] > 0.0) {
+            if (cached) {
+#pragma unroll
+              for (int q = 0; q < L3_CACHE; ++q)
+                if ((uint32_t)q / C == (uint32_t)a && (uint32_t)q < per_thread * C) F += l3_term(par[q], lgx);
+            } else {
+              for (uint32_t c = 0; c < C; ++c) {
+                const uint32_t k = cnt[r * C + c];
+                if (k) F += l3_term(l3_par(k, tot[a], p50[r * C + c], p99[r * C + c]), lgx);
+              }
             }
+          }
         }
         val[r] = F;
         id[r] = (uint16_t)r;
       }
       __syncthreads();
       bitonic_sort(val, id, n2);
-      // exclusive prefix sums of the sorted values (one thread: R <= 4096 adds per grid point is small next
-      // to the sort) and the total
-      if (threadIdx.x == 0) {
-        double run = 0.0;
-        for (uint32_t i = 0; i < R; ++i) { pre[i] = run; run += val[i]; }
-        s_red[0] = run;
-      }
-      __syncthreads();
-      const double total = s_red[0];
-      // sum_b |F_r - F_b| for the value at sorted position i: F (2 i - R) + total - 2 pre[i]
-      for (uint32_t i = threadIdx.x; i < R; i += blockDim.x) {
-        const double F = val[i];
-        const double S = F * (2.0 * (double)i - (double)R) + total - 2.0 * pre[i];
-        score[id[i]] += wj * S;
+      // sum_b |F_r - F_b| at every sorted position, from the gaps
+      double d[4];
+      if (n2 >= 4096u) {
+        abs_dev_sums<4>(val, R, s_red, d);
+        for (int k = 0; k < 4; ++k) { const uint32_t i = threadIdx.x * 4u + k; if (i < R) score[id[i]] += wj * d[k]; }
+      } else if (n2 >= 2048u) {
+        abs_dev_sums<2>(val, R, s_red, d);
+        for (int k = 0; k < 2; ++k) { const uint32_t i = threadIdx.x * 2u + k; if (i < R) score[id[i]] += wj * d[k]; }
+      } else {
+        abs_dev_sums<1>(val, R, s_red, d);
+        if (threadIdx.x < R) score[id[threadIdx.x]] += wj * d[0];
       }
       __syncthreads();
     }
@@ -558,7 +645,7 @@ cudaError_t argus_launch_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_c
 size_t argus_l3_smem_bytes(uint32_t R) {
   uint32_t n2 = 1;
   while (n2 < R) n2 <<= 1;
-  return sizeof(double) * ((size_t)2 * n2 + R) + sizeof(uint16_t) * n2;
+  return sizeof(double) * ((size_t)n2 + R) + sizeof(uint16_t) * n2;
 }
 
 cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,
