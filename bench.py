@@ -173,6 +173,116 @@ def _ms(pairs):
     return [a.elapsed_time(b) for a, b in pairs]
 
 
+def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=512, fine_limit_bytes=6 << 30):
+    """The SURVEY 8(f) NEXT rows on the table the timed steps left behind (finalised), each call timed alone
+    with CUDA events (1 warm-up, median of `reps`); outside the step's timed region.  Bytes are the
+    algorithmic ones of DESIGN.md 6.6 / 6.7 (what the call must read and write), GB/s = bytes / median time.
+    Nothing here is compared with the oracle (tests/test_paper_literal_gpu.py, tests/test_compact_gpu.py do)."""
+    import torch
+    R, T, S, P = s.n_ranks, s.n_steps, s.n_sigs, s.n_phases
+    n, n_cells, K, MC = s.total_events, R * T * S, T * S, 8
+    dev = rec.device
+    mk = lambda: torch.cuda.Event(enable_timing=True)
+
+    def timed(fn, reset=None):
+        ts = []
+        for i in range(reps + 1):
+            if reset is not None:
+                reset()
+            a, b = mk(), mk()
+            a.record()
+            fn()
+            b.record()
+            torch.cuda.synchronize()
+            if i:
+                ts.append(a.elapsed_time(b))
+        return float(np.median(ts)), float(np.min(ts))
+
+    def line(ms, best, nbytes, bound, **kw):
+        d = {"ms": ms, "ms_best": best, "algorithmic_bytes": int(nbytes), "gbs": nbytes / (ms * 1e-3) / 1e9,
+             "hbm_frac": nbytes / (ms * 1e-3) / 1e9 / peak, "bound": bound}
+        d.update(kw)
+        return d
+
+    out = {}
+    u8 = lambda m: torch.zeros(m, dtype=torch.uint8, device=dev)
+    # NEXT-1 on the records' own 32-bucket histograms: read 128 B of histogram per cell, write MC triples + 1 B
+    d_c, d_n = u8(n_cells * MC * 8), u8(n_cells)
+    p32 = ctx.kde_params(per_octave=1, n_bins=32, max_clusters=MC)
+    ms, best = timed(lambda: ctx.kde_clusters_records(rec, p32, d_c, d_n))
+    ncl = d_n.to(torch.int64)
+    n_clusters = int(ncl.sum())
+    out["next1_kde_records"] = line(ms, best, n_cells * (128 + 8 * MC + 1), "alu (fp64 exp per occupied bin pair)",
+                                    cells=n_cells, cells_per_s=n_cells / (ms * 1e-3), clusters=n_clusters,
+                                    cells_with_2plus=int((ncl >= 2).sum()))
+    # NEXT-4b record encodings: read the table once, write the stream
+    tb = ctx.table_bytes
+    off = torch.zeros(R * T + 1, dtype=torch.int64, device=dev)
+    buf = u8(ctx.sparse_bound())
+    ms, best = timed(lambda: ctx.sparse_encode(rec, buf, off))
+    sparse_len = int(off[-1])
+    out["next4_sparse_encode"] = line(ms, best, tb + sparse_len, "hbm", stream_bytes=sparse_len,
+                                      raw_over_record=32 * n / sparse_len, dense_over_record=tb / sparse_len,
+                                      bytes_per_rank_step=sparse_len / (R * T))
+    del buf
+    buf = u8(ctx.triple_bound(MC))
+    ms, best = timed(lambda: ctx.triple_encode(rec, d_c, d_n, MC, buf, off))
+    triple_len = int(off[-1])
+    out["next4_triple_encode"] = line(ms, best, R * T * (64 + 32 * (P + 1)) + n_cells * (8 * MC + 1) + triple_len, "hbm",
+                                      stream_bytes=triple_len, raw_over_record=32 * n / triple_len,
+                                      bytes_per_rank_step=triple_len / (R * T), triples_per_rank_step=n_clusters / (R * T),
+                                      paper="~3,700x: ~10 MB -> ~2.7 KB, ~200 triples per rank per step (PAPER.md:196; "
+                                            "its key is (kernel, stream, rank) with a few hundred kernels, this workload "
+                                            "has S sigs per rank-step)")
+    del buf
+    # NEXT-1 on the fine grid (8 bins per octave): events -> [R][T][S][256] u32 with L2 atomics -> clusters
+    fine_bytes = n_cells * 1024
+    if d_ev is not None and fine_bytes <= fine_limit_bytes:
+        hist = torch.zeros(n_cells * 256, dtype=torch.int32, device=dev)
+        ms, best = timed(lambda: ctx.fine_hist(d_ev, n, hist), reset=lambda: hist.zero_())
+        out["next1_fine_hist"] = line(ms, best, 32 * n + fine_bytes, "hbm + L2 atomics", events_per_s=n / (ms * 1e-3))
+        d_c8, d_n8 = u8(n_cells * MC * 8), u8(n_cells)
+        p256 = ctx.kde_params(max_clusters=MC)
+        ms, best = timed(lambda: ctx.kde_clusters(hist, n_cells, p256, d_c8, d_n8))
+        out["next1_kde_fine"] = line(ms, best, n_cells * (1024 + 8 * MC + 1), "hbm (1 KB of counters per cell) / alu",
+                                     cells=n_cells, cells_per_s=n_cells / (ms * 1e-3), clusters=int(d_n8.sum()))
+        del hist, d_c8, d_n8
+    else:
+        out["next1_fine_hist"] = {"skipped": f"[R][T][S][256] u32 = {fine_bytes / 2**30:.1f} GiB: measured on mid / scale"}
+    # NEXT-2: regroup the triples per key, then score the first l3_keys keys over all R ranks
+    d_cnt = torch.zeros(K * R * MC, dtype=torch.int32, device=dev)
+    d_p50 = torch.zeros(K * R * MC, dtype=torch.float64, device=dev)
+    d_p99 = torch.zeros(K * R * MC, dtype=torch.float64, device=dev)
+    ms, best = timed(lambda: ctx.clusters_to_l3(d_c, MC, 1, d_cnt, d_p50, d_p99))
+    out["next2_clusters_to_l3"] = line(ms, best, n_cells * MC * (8 + 20), "hbm (transpose)")
+    kk = min(K, l3_keys)
+    G = 256
+    d_score = torch.zeros(kk * R, dtype=torch.float64, device=dev)
+    d_stat = torch.zeros(kk * 5, dtype=torch.float64, device=dev)
+    d_fl = u8(kk * R)
+    ms, best = timed(lambda: ctx.l3_detect(d_cnt, d_p50, d_p99, kk, R, MC, d_score, d_stat, d_fl, n_grid=G))
+    out["next2_l3_detect"] = line(ms, best, kk * R * (MC * 20 + 9), "alu / shared memory (a sort of R CDF values per grid point)",
+                                  keys=kk, ranks=R, n_grid=G, cdf_points_per_s=kk * R * G / (ms * 1e-3),
+                                  flagged=int(d_fl.sum()))
+    del d_cnt, d_p50, d_p99, d_c, d_n
+    # NEXT-3: L2 over every phase span (one group per 8 consecutive ranks), L1 over the R iteration-time series
+    route = u8(P + 1)
+    gid = (torch.arange(R, device=dev, dtype=torch.int32) // 8 * 8).contiguous()
+    d_groups = u8((P + 1) * R * 32)
+    d_z = torch.zeros((P + 1) * R, dtype=torch.float64, device=dev)
+    d_xb = torch.zeros((P + 1) * R, dtype=torch.float64, device=dev)
+    d_f2 = u8((P + 1) * R)
+    ms, best = timed(lambda: ctx.l2_groups(rec, route, gid, 3.0, d_groups, d_z, d_f2, d_xb))
+    out["next3_l2_groups"] = line(ms, best, R * T * (P + 1) * 32 + (P + 1) * R * (32 + 8 + 1), "latency (KBs of data)")
+    if 8 <= T <= 2048:
+        spans = torch.zeros(R * T * (P + 1) * 32, dtype=torch.uint8, device=dev)
+        ctx.phase_times(rec, spans)
+        d_l1 = u8(R * 216)
+        ms, best = timed(lambda: ctx.l1_detect(spans.data_ptr() + P * 32 + 16, T * (P + 1) * 32, (P + 1) * 32, R, T, d_l1))
+        out["next3_l1_detect"] = line(ms, best, R * T * 8 + R * 216, "latency (KBs of data)")
+    return out
+
+
 def run_ours(args, world):
     import torch
     from paper_2606_20374_b200 import argus as A
@@ -246,6 +356,15 @@ def run_ours(args, world):
     total_events = D.sum_over_ranks(world, float(n))
     value = total_events / (ms_step * 1e-3)
     resident = {k: v.clone() for k, v in outs.items()}
+
+    # ---- the NEXT rows of SURVEY 8(f) on the finalised table (outside the timed steps) --------------
+    nxt = None
+    if world.rank == 0 and not args.no_next:
+        try:
+            nxt = next_rows(ctx, rec, d_ev, s, measured_peak_gbs()[0])
+        except Exception as e:
+            nxt = {"error": repr(e)[:300]}
+        torch.cuda.synchronize()
 
     # ---- e2e: HOST buffers through argus_aggregate_host, copies inside the timed region ----------
     e2e = None
@@ -361,6 +480,8 @@ def run_ours(args, world):
     }
     if args.bimodal > 0.0:
         out["config"]["bimodal_sigs"] = wl.n_bimodal
+    if nxt is not None:
+        out["next_rows"] = nxt
     if world.size == 1 and not args.no_cpu_baseline:
         k = args.cpu_baseline_ranks if args.cpu_baseline_ranks > 0 else s.n_ranks
         if args.cpu_baseline_ranks < 0:      # default: a bounded sample, about 15 s of oracle time
@@ -419,6 +540,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true",
+                    help="skip the separately timed NEXT rows (KDE clusters, record encodings, L3 / L2 / L1)")
     ap.add_argument("--cpu-baseline-ranks", type=int, default=-1,
                     help="ranks of the workload the oracle is timed on: -1 = bounded sample (default), 0 = all")
     args = ap.parse_args()
