@@ -123,11 +123,12 @@ typedef struct argus_config {
   uint32_t max_ungrouped_events; /* largest n of one argus_aggregate call on input WITHOUT the SORTED hint that
                           is still grouped first (sizes the grouping area of the workspace: 32 B per event);
                           0 = no grouping area, ungrouped input goes through the global-table kernel */
-  uint32_t max_spill_events; /* events one argus_aggregate call may RE-QUEUE (sizes the spill area of the workspace,
-                          32 B per event): an event whose (rank, step, sig) cell cannot hold it in shared memory —
-                          the second mode of a kernel whose durations "differ by several multiples" between
-                          positions, PAPER.md:166 — is set aside and folded by a second launch; 0 or exhausted:
-                          such events take L2 reductions one by one (same results, far slower when they are many) */
+  uint32_t max_spill_events; /* RE-QUEUED events the segmented kernel may hold at one time (sizes the spill area of the
+                          workspace, 8 B per event, shared evenly by its persistent CTAs): an event whose (rank, step,
+                          sig) cell cannot hold it in shared memory — the second mode of a kernel whose durations
+                          "differ by several multiples" between positions, PAPER.md:166 — is set aside as {sig, duration}
+                          and folded when its rank-step is flushed; 0 or exhausted: such events take L2 reductions
+                          one by one (same results, far slower when they are many) */
   uint32_t reserved;   /* 0 */
 } argus_config;
 
@@ -161,7 +162,7 @@ typedef struct argus_ctx argus_ctx;  /* opaque */
  * gather of argus_diagnose reads whole sectors: 134 MB at R = S = 4096), the per-CTA overflow lists of the
  * segmented kernel (64 KB x 1024), one mark byte per diagnosed series, and — only when
  * cfg->max_ungrouped_events > 0 — the per-CTA key histograms of the grouping pass and the grouping area
- * itself (32 B per event), and — only when cfg->max_spill_events > 0 — the spill area (32 B per event).  Queries the device of cfg for its SM count.  0 if cfg is invalid. */
+ * itself (32 B per event), and — only when cfg->max_spill_events > 0 — the spill area (8 B per event).  Queries the device of cfg for its SM count.  0 if cfg is invalid. */
 size_t argus_workspace_bytes(const argus_config* cfg);
 
 /* Create a context for one table geometry.  [device] d_workspace: argus_workspace_bytes(cfg) bytes,
@@ -388,7 +389,7 @@ int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid);
 
 /* Events the shared-memory compact cells of the segmented kernel refused since argus_reset (duration >= 2^32
  * ns, or a (rank, step, sig) whose durations spread over more than four consecutive log2 buckets: heavy
- * tails, multimodal kernels): n_requeued went through the spill area and a second launch,
+ * tails, multimodal kernels): n_requeued went through the spill area and were folded at the flush of their rank-step,
  * n_overflow took the overflow list / L2 reductions.  A throughput diagnostic: results do not depend on
  * it.  Synchronises like argus_stats.  [host] outputs, may be NULL. */
 int argus_refused_count(argus_ctx* ctx, uint64_t* n_requeued, uint64_t* n_overflow);

@@ -21,11 +21,12 @@
 // hot path (64-bit shared atomic adds are CAS loops on sm_100a).
 // An event the compact cell cannot take (a range wider than four buckets: the second mode of a kernel
 // whose durations "differ by several multiples" between positions) is RE-QUEUED: the lane
-// appends the raw event to its CTA's region of a spill buffer (workspace) and goes on; a second launch
-// of this same kernel (REQUEUE: cells only, spans and counters were taken the first time) folds every
-// CTA's region, where the sig's remaining events now find the cell empty and open a window of their
-// own.  What that launch still refuses, events of 2^32 ns or more, and everything when the spill area
-// is absent or full, is parked in the CTA's overflow list (global memory, workspace) and applied to the
+// appends {sig, duration} to its CTA's spill region (workspace) and goes on — span and counters are taken
+// at once.  At the flush of the key, after the table has been written and cleared, the CTA folds the
+// key's spilled events into the empty table, where the sig's remaining events open a window of their own,
+// and merges that second table into the (now live) record with L2 reductions on the non-empty cells.  What
+// the replay still refuses, events of 2^32 ns or more, and everything when the spill area is absent or
+// full, is parked in the CTA's overflow list (global memory, workspace) and applied to the
 // record with L2 reductions at the flush; when the record is already live it goes there at once.  When the
 // (rank, step) key changes the table is flushed: the first CTA to reach a record claims it and
 // writes the whole 160-byte cells with coalesced 128-bit stores (no read-modify-write, no separate
@@ -62,6 +63,7 @@ struct Hdr {
   uint32_t ovf_n;                     // events parked in this CTA's overflow list since the last flush
   uint32_t spill_n;                   // events this CTA re-queued into its spill region
   uint32_t n_refused;                 // events that took the overflow list or L2 atomics
+  uint32_t n_requeued;                // events replayed from the spill region (a CTA's span holds < 2^26 events)
 };
 constexpr uint32_t OVF_CAP = ARGUS_OVF_CAP;   // entries of a CTA's overflow list (16 bytes each, workspace)
 constexpr unsigned long long NEXT_NONE = ~0ull;
@@ -188,6 +190,8 @@ struct Glob {             // global-memory side of the kernel
   uint8_t* records;
   uint32_t* state;
   uint4* ovf;             // this CTA's overflow list: {sig, 0, duration lo, duration hi} of events the compact cell refused
+  uint2* spill;           // this CTA's spill region: {sig, duration} of the current key's re-queued events
+  uint32_t spill_cap;     // its capacity in events (0: no spill area)
   argus_dims D;
 };
 
@@ -272,6 +276,54 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
 
+// The compact-cell update of one event (sig, d32 < 2^32) outside the hot loop (the replay of re-queued
+// events): same protocol as ARGUS_COMPACT_ADD in the kernel.  True if the cell took the event.
+template <uint32_t SCAP>
+__device__ __forceinline__ bool compact_add(uint32_t sbase, uint32_t sig, uint32_t d32) {
+  const uint32_t a_slots = sbase + TAB_OFF, a_m = a_slots + 24u * SCAP + sig * 8u;
+  const uint2 m = lds64(a_m);
+  const uint32_t nd = ~d32, b = bucket32(d32);
+  bool took = (b >= bucket32(~m.x)) & (b <= bucket32(m.y));
+  reds_max_if(a_m, nd, took & (nd > m.x));
+  reds_max_if(a_m + 4u, d32, took & (d32 > m.y));
+  if (!took) took = mm_extend(a_m, d32);
+  if (took) {
+    reds_add(a_slots + sig * 16u + ((b & 3u) << 2), 1u);
+    const uint32_t old = atoms_add(a_slots + 16u * SCAP + sig * 4u, d32);
+    if (old > nd) reds_add(a_slots + 20u * SCAP + sig * 4u, 1u);
+  }
+  return took;
+}
+
+// The non-empty cells of the shared table into the LIVE record `key` with L2 reductions.
+template <int NC, uint32_t SCAP>
+__device__ __forceinline__ void merge_cells(uint8_t* rec, const argus_dims& D, uint32_t key) {
+  const Table tb{SCAP};
+  argus_cell* cells = reinterpret_cast<argus_cell*>(rec + D.cell_off);
+  for (uint32_t sig = threadIdx.x; sig < D.S; sig += NC) {
+    const uint4 s = *tb.slots(sig);
+    const uint2 m = *tb.mm(sig);
+    if ((m.x | m.y) != 0u) {
+      const uint32_t sl[4] = {s.x, s.y, s.z, s.w};
+      const uint32_t bl = bucket32(~m.x);
+      unsigned long long cnt = 0;
+#pragma unroll
+      for (uint32_t k = 0; k < 4u; ++k) {
+        if (sl[k]) {
+          atomicAdd(&cells[sig].hist[bl + ((k - bl) & 3u)], sl[k]);   // the bucket >= bl with bucket & 3 == k
+          cnt += sl[k];
+        }
+      }
+      atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].count), cnt);
+      const unsigned long long sm = ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig);
+      atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].sum_ns), sm);
+      if (D.sums) atomicAdd(&D.sums[(size_t)key * D.S + sig], sm);
+      atomicMin(reinterpret_cast<unsigned long long*>(&cells[sig].min_ns), (unsigned long long)(~m.x));
+      atomicMax(reinterpret_cast<unsigned long long*>(&cells[sig].max_ns), (unsigned long long)m.y);
+    }
+  }
+}
+
 // Flush the shared table of record `key` to global memory and clear it.  All NC consumer threads
 // call between the rendezvous barrier (the table is final: every warp has flushed its WarpSpan)
 // and the closing barrier of park().  The claim on the record was taken when the key was adopted
@@ -288,6 +340,8 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
   uint32_t mode = *reinterpret_cast<volatile uint32_t*>(&H->mode);
   uint32_t n_ovf = *reinterpret_cast<volatile uint32_t*>(&H->ovf_n);
   n_ovf = n_ovf < OVF_CAP ? n_ovf : OVF_CAP;
+  uint32_t n_sp = *reinterpret_cast<volatile uint32_t*>(&H->spill_n);   // re-queued events of this key
+  n_sp = n_sp < g.spill_cap ? n_sp : g.spill_cap;
   if (mode == ARGUS_ST_BUSY) {
     // another (resident, running) CTA owns this record and is writing it: wait for it, then merge
     if (tid == 0) {
@@ -351,34 +405,10 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
       for (uint32_t sig = tid; sig < D.S; sig += NC)
         row[sig] = ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig);
     }
-    if (fence_all || n_ovf) __threadfence();   // L2 atomics on this record follow at once
+    if (fence_all || n_ovf || n_sp) __threadfence();   // L2 atomics on this record follow at once
   } else {
     // merge into a live record with L2 reductions (non-empty fields only)
-    argus_cell* cells = reinterpret_cast<argus_cell*>(rec + D.cell_off);
-    for (uint32_t sig = tid; sig < D.S; sig += NC) {
-      const uint4 s = *tb.slots(sig);
-      const uint2 m = *tb.mm(sig);
-      if ((m.x | m.y) != 0u) {
-        const uint32_t sl[4] = {s.x, s.y, s.z, s.w};
-        const uint32_t bl = bucket32(~m.x);
-        unsigned long long cnt = 0;
-#pragma unroll
-        for (uint32_t k = 0; k < 4u; ++k) {
-          if (sl[k]) {
-            atomicAdd(&cells[sig].hist[bl + ((k - bl) & 3u)], sl[k]);   // the bucket >= bl with bucket & 3 == k
-            cnt += sl[k];
-          }
-        }
-        atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].count), cnt);
-        const unsigned long long sm = ((unsigned long long)*tb.sum_hi(sig) << 32) | *tb.sum_lo(sig);
-        atomicAdd(reinterpret_cast<unsigned long long*>(&cells[sig].sum_ns), sm);
-        if (D.sums) atomicAdd(&D.sums[(size_t)key * D.S + sig], sm);
-        atomicMin(reinterpret_cast<unsigned long long*>(&cells[sig].min_ns),
-                  (unsigned long long)(~m.x));
-        atomicMax(reinterpret_cast<unsigned long long*>(&cells[sig].max_ns),
-                  (unsigned long long)m.y);
-      }
-    }
+    merge_cells<NC, SCAP>(rec, D, key);
     argus_span* sp = reinterpret_cast<argus_span*>(rec + D.span_off);
     for (uint32_t k = tid; k < D.P; k += NC) {
       const SpanAcc a = spans[k];
@@ -404,6 +434,28 @@ __device__ __noinline__ void flush_table(const Glob& g, uint32_t key, bool fence
   tb.clear(D.S, (uint32_t)tid, (uint32_t)NC);
   for (uint32_t k = tid; k < D.P; k += NC) {
     spans[k].mn = INT64_MAX; spans[k].mx = INT64_MIN; spans[k].n = 0ull; spans[k].pad = 0ull;
+  }
+  if (n_sp) {   // CTA-uniform
+    // Replay of the key's re-queued events (cells only: spans and counters were taken when they were set
+    // aside).  The record is live (published above, or by its owner), the table is empty: a sig whose
+    // events fell outside the first window opens a second one here; what even that refuses takes L2
+    // reductions one by one.  Then the second table is merged into the record and cleared.
+    bar_consumers(NC);                      // table cleared; every lane's spill stores are visible to the CTA
+    const uint32_t sbase = smem_u32(smem);
+    uint32_t refused = 0;
+    for (uint32_t i = tid; i < n_sp; i += NC) {
+      const uint2 e = __ldcg(g.spill + i);
+      if (!compact_add<SCAP>(sbase, e.x, e.y)) {
+        global_cell_add(g.records, D, key, e.x, (unsigned long long)e.y);
+        ++refused;
+      }
+    }
+    if (refused) atomicAdd(&H->n_refused, refused);
+    bar_consumers(NC);
+    merge_cells<NC, SCAP>(rec, D, key);
+    if (tid == 0) { H->spill_n = 0u; H->n_requeued += n_sp; }
+    bar_consumers(NC);                      // everybody has read its cells: clear
+    tb.clear(D.S, (uint32_t)tid, (uint32_t)NC);
   }
 }
 
@@ -464,14 +516,11 @@ __host__ __device__ constexpr int ring_depth(uint32_t scap, uint32_t stage_bytes
 
 // CW consumer warps + 1 producer warp; a stage = WPSTG warps' worth of events (WPSTG KB); the table
 // layout is compiled for SCAP sigs (S <= SCAP), so every table address is base + sig * c + constant.
-// REQUEUE = the second launch: CTA i folds the spill_cnt[i] events the first launch's CTA i re-queued into
-// region i of the spill buffer (ev), cells only.
-template <int CW, int WPSTG, uint32_t SCAP, int MINB, bool REQUEUE>
+template <int CW, int WPSTG, uint32_t SCAP, int MINB>
 __global__ void __launch_bounds__((CW + 1) * 32, MINB)
 aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __restrict__ ev, uint64_t n,
                      uint64_t per_cta, uint8_t* records, uint32_t* state, unsigned long long* counters,
-                     uint4* ovf, argus_dims D, uint4* __restrict__ spill, uint32_t* __restrict__ spill_cnt,
-                     uint32_t spill_cap) {
+                     uint4* ovf, argus_dims D, uint2* spill, uint32_t spill_cap) {
   constexpr int K = ring_depth(SCAP, (uint32_t)WPSTG * 1024u, CW / WPSTG, MINB);
   static_assert(K >= 2 * (CW / WPSTG), "ring too shallow for this geometry");
   constexpr int NC = CW * 32;            // consumer threads
@@ -481,6 +530,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   Glob gl;
   gl.records = records; gl.state = state; gl.D = D;
   gl.ovf = ovf + (size_t)blockIdx.x * OVF_CAP;
+  gl.spill = spill + (size_t)blockIdx.x * spill_cap; gl.spill_cap = spill_cap;
   const Table tb{SCAP};
   Hdr* H = hdr();
   constexpr uint32_t stages = (TAB_OFF + 32u * SCAP + 127u) & ~127u;   // byte offset of the stage ring in smem
@@ -489,8 +539,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   const uint64_t e0 = (uint64_t)blockIdx.x * per_cta;
   if (e0 >= n) return;
   const uint64_t e1 = (e0 + per_cta < n) ? e0 + per_cta : n;
-  const uint32_t n_ev = REQUEUE ? spill_cnt[blockIdx.x] : (uint32_t)(e1 - e0);
-  if (REQUEUE && n_ev == 0u) return;
+  const uint32_t n_ev = (uint32_t)(e1 - e0);
   const uint32_t n_sub = (n_ev + SUBE - 1) / SUBE;
   const uint32_t n_iter = (n_ev + NC - 1) / NC;
 
@@ -499,7 +548,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       mbar_init(smem_u32(&H->full[k]), 1u);
       mbar_init(smem_u32(&H->empty[k]), (uint32_t)WPSTG);
     }
-    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u; H->ovf_n = 0u; H->spill_n = 0u; H->n_refused = 0u;
+    H->next = NEXT_NONE; H->mode = ARGUS_ST_LIVE; H->n_finished = 0u; H->ovf_n = 0u; H->spill_n = 0u; H->n_refused = 0u; H->n_requeued = 0u;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   {
@@ -603,20 +652,17 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     }                                                                                    \
   } while (0)
 
-  // A refused event of the current key (d < 2^32) is appended, as a raw 32-byte record rebuilt from the
-  // decoded fields (the stream id is not part of the method and is dropped), to this CTA's spill region.
-  uint4* const my_spill = spill + 2 * (size_t)blockIdx.x * spill_cap;
-#define ARGUS_SPILL(okv)                                                                              \
-  do {                                                                                               \
-    if (!REQUEUE && spill_cap != 0u) {                                                               \
-      const uint32_t sp_ = atomicAdd(&H->spill_n, 1u);                                               \
-      if (sp_ < spill_cap) {                                                                         \
-        my_spill[2 * (size_t)sp_] = make_uint4(cur_rank, cur_step, sig, phase << 16);                \
-        my_spill[2 * (size_t)sp_ + 1] = make_uint4((uint32_t)start, (uint32_t)((unsigned long long)start >> 32), \
-                                                   (uint32_t)end, (uint32_t)((unsigned long long)end >> 32));   \
-        okv = true;                                                                                  \
-      }                                                                                              \
-    }                                                                                                \
+  // A refused event of the current key (d < 2^32) is appended as {sig, duration} to this CTA's spill region
+  // and replayed at the flush of the key; its span and its place in the counters are taken here.
+#define ARGUS_SPILL(okv)                                          \
+  do {                                                           \
+    if (spill_cap != 0u) {                                       \
+      const uint32_t sp_ = atomicAdd(&H->spill_n, 1u);           \
+      if (sp_ < spill_cap) {                                     \
+        gl.spill[sp_] = make_uint2(sig, d32);                    \
+        okv = true;                                              \
+      }                                                          \
+    }                                                            \
   } while (0)
 
   const uint32_t n_full = n_ev / (uint32_t)NC;   // iterations in which every lane of every warp has an event
@@ -682,9 +728,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       // ---- hot path: the whole warp folds into the current table -------------------------------------
       ARGUS_COMPACT_ADD(ok);
       if (!ok) ARGUS_SPILL(ok);
-      if (REQUEUE) {
-        if (__all_sync(FULL, ok)) return;  // cells only
-      } else if (__all_sync(FULL, ok && phase == ws.phase)) {
+      if (__all_sync(FULL, ok && phase == ws.phase)) {
         ws.mn = start < ws.mn ? start : ws.mn;
         ws.mx = end > ws.mx ? end : ws.mx;
         ws.n += 32u;                       // warp-uniform count
@@ -694,7 +738,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
     } else {
       // full validity (R2, R3) of the lanes that failed the fast test
       pending = mine && argus_event_key(D, lo.x, lo.y, sig, phase, start, end, key);
-      n_invalid += (!REQUEUE && mine && !pending) ? 1u : 0u;
+      n_invalid += (mine && !pending) ? 1u : 0u;
       fast = pending && key == cur_key && (uint32_t)(d >> 32) == 0u;
     }
 
@@ -729,7 +773,7 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
       // registers; a warp with mixed phases (ungrouped or boundary input) updates the shared
       // accumulators lane by lane: test min/max with a plain load first (they rarely improve after
       // the first few events), count with a 32-bit add (a CTA's span holds < 2^26 events: no carry).
-      if (!REQUEUE) {
+      {
         const uint32_t ph0 = __shfl_sync(FULL, phase, 0);
         if (__all_sync(FULL, ok && phase == ph0)) {
           if (ph0 != ws.phase) { ws.flush(lane); ws.phase = ph0; }
@@ -770,15 +814,9 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
   if (lane == 0 && n_invalid) atomicAdd(&counters[1], (unsigned long long)n_invalid);
   if (tid == 0) {
     // H->* are final: every warp has passed the last rendezvous
-    if (!REQUEUE) {
-      atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
-      if (spill_cap != 0u) {
-        uint32_t ns = *reinterpret_cast<volatile uint32_t*>(&H->spill_n);
-        ns = ns < spill_cap ? ns : spill_cap;
-        spill_cnt[blockIdx.x] = ns;
-        if (ns) atomicAdd(&counters[3], (unsigned long long)ns);
-      }
-    }
+    atomicAdd(&counters[0], (unsigned long long)n_ev);   // seen; valid = seen - invalid
+    const uint32_t nq = *reinterpret_cast<volatile uint32_t*>(&H->n_requeued);
+    if (nq) atomicAdd(&counters[3], (unsigned long long)nq);
     const uint32_t nr = *reinterpret_cast<volatile uint32_t*>(&H->n_refused);
     if (nr) atomicAdd(&counters[2], (unsigned long long)nr);
   }
@@ -794,11 +832,7 @@ constexpr size_t geom_smem() {
 template <int CW, int WPSTG, uint32_t SCAP, int MINB>
 cudaError_t configure_cap() {
   static_assert(geom_smem<CW, WPSTG, SCAP, MINB>() <= smem_budget(MINB), "shared memory");
-  cudaError_t e = cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, false>,
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)geom_smem<CW, WPSTG, SCAP, MINB>());
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, true>,
+  return cudaFuncSetAttribute(aggregate_seg_kernel<CW, WPSTG, SCAP, MINB>,
                               cudaFuncAttributeMaxDynamicSharedMemorySize,
                               (int)geom_smem<CW, WPSTG, SCAP, MINB>());
 }
@@ -840,24 +874,14 @@ cudaError_t launch_cap(argus_ctx* ctx, const argus_event* ev, uint64_t n, void* 
   CUtensorMap tmap;
   cudaError_t e = encode_events(ctx, ev, n >> 2, (uint32_t)(WPSTG * 8), &tmap);
   if (e != cudaSuccess) return e;
-  // spill regions: one per CTA, whole 128-byte rows (0: refused events go to the overflow lists)
-  uint64_t scap = ctx->d_spill ? ((uint64_t)ctx->cfg.max_spill_events / ctas) & ~3ull : 0u;
+  // spill regions: one per CTA, 8 bytes per re-queued event of the CTA's CURRENT key (0: refused events go to
+  // the overflow lists)
+  uint64_t scap = ctx->d_spill ? (uint64_t)ctx->cfg.max_spill_events / ctas : 0u;
   if (scap > per_cta) scap = per_cta;
-  uint4* spill = reinterpret_cast<uint4*>(ctx->d_spill);
-  aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, false><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
+  aggregate_seg_kernel<CW, WPSTG, SCAP, MINB><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
       tmap, reinterpret_cast<const uint4*>(ev), n, per_cta, static_cast<uint8_t*>(d_records), ctx->d_state,
-      ctx->d_counters, ctx->d_ovf, ctx->dims, spill, ctx->d_spill_cnt, (uint32_t)scap);
+      ctx->d_counters, ctx->d_ovf, ctx->dims, reinterpret_cast<uint2*>(ctx->d_spill), (uint32_t)scap);
   ctx->n_kernels += 1;
-  if (scap != 0u) {
-    // second launch: every CTA folds what its twin re-queued (most CTAs find nothing and leave at once)
-    CUtensorMap tmap2;
-    e = encode_events(ctx, spill, (ctas * scap) >> 2, (uint32_t)(WPSTG * 8), &tmap2);
-    if (e != cudaSuccess) return e;
-    aggregate_seg_kernel<CW, WPSTG, SCAP, MINB, true><<<(unsigned)ctas, (CW + 1) * 32, smem_bytes, s>>>(
-        tmap2, spill, ctas * scap, scap, static_cast<uint8_t*>(d_records), ctx->d_state, ctx->d_counters,
-        ctx->d_ovf, ctx->dims, nullptr, ctx->d_spill_cnt, 0u);
-    ctx->n_kernels += 1;
-  }
   return cudaGetLastError();
 }
 

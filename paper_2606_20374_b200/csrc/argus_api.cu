@@ -69,12 +69,8 @@ void argus_ws_plan(const argus_config* c, int sm_count, int max_smem_optin, argu
     L->group = o;
     o += up256((size_t)c->max_ungrouped_events * sizeof(argus_event));
   }
-  L->spill_cnt = o; L->spill = o;
-  if (c->max_spill_events) {
-    o += up256(sizeof(uint32_t) * ARGUS_MAX_SEG_CTAS);
-    L->spill = o;
-    o += up256((size_t)c->max_spill_events * sizeof(argus_event));
-  }
+  L->spill = o;
+  if (c->max_spill_events) o += up256((size_t)c->max_spill_events * 8u);
   L->total = o;
 }
 
@@ -132,10 +128,7 @@ extern "C" int argus_create(const argus_config* cfg, void* d_workspace, size_t w
     D.sums = reinterpret_cast<unsigned long long*>(ctx->d_ws + L.sums);
     ctx->d_ovf = reinterpret_cast<uint4*>(ctx->d_ws + L.ovf);
     ctx->d_diag_todo = ctx->d_ws + L.diag_todo;
-    if (cfg->max_spill_events) {
-      ctx->d_spill_cnt = reinterpret_cast<uint32_t*>(ctx->d_ws + L.spill_cnt);
-      ctx->d_spill = ctx->d_ws + L.spill;
-    }
+    if (cfg->max_spill_events) ctx->d_spill = ctx->d_ws + L.spill;
     if (cfg->max_ungrouped_events) {
       ctx->d_part = (L.part_smem || L.part_two_level) ? reinterpret_cast<uint32_t*>(ctx->d_ws + L.part) : nullptr;
       ctx->d_coarse = L.part_two_level ? ctx->d_ws + L.coarse : nullptr;

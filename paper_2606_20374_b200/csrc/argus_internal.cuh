@@ -30,7 +30,7 @@ struct argus_dims {
 #define ARGUS_MAX_SEG_CTAS 1024u      // CTAs of one segmented launch (bounds the overflow-list area)
 #define ARGUS_OVF_CAP 4096u           // entries (16 B) of one CTA's overflow list
 struct argus_ws_layout {
-  size_t state, counters, hist, sums, ovf, diag_todo, part, group, spill_cnt, spill, total;
+  size_t state, counters, hist, sums, ovf, diag_todo, part, group, spill, total;
   size_t coarse;                      // two-level grouping: the packed events grouped by coarse bin (16 B per event)
   uint32_t part_ctas;                 // CTAs of the grouping pass (0: no grouping area)
   bool part_smem;                     // its key histograms fit shared memory
@@ -56,8 +56,7 @@ struct argus_ctx {
                               // state of the two-level pass
   uint8_t* d_coarse;          // two-level grouping: coarse area [cfg.max_ungrouped_events] x 16 B
   uint8_t* d_diag_todo;       // argus_diagnose: one byte per series, set by the 32-bit pass for the 64-bit pass
-  uint8_t* d_spill;           // spill regions of the segmented kernel [cfg.max_spill_events] raw events (null when 0)
-  uint32_t* d_spill_cnt;      // events re-queued by each CTA of the last segmented launch [ARGUS_MAX_SEG_CTAS]
+  uint8_t* d_spill;           // spill regions of the segmented kernel: {sig, duration} of re-queued events, 8 B x cfg.max_spill_events (null when 0)
   uint4* d_ovf;               // per-CTA overflow lists of the segmented kernel [ARGUS_MAX_SEG_CTAS][ARGUS_OVF_CAP]
   void* d_records;            // table given to the last argus_reset
   cudaEvent_t ingest_event;   // recorded after every argus_ingest copy

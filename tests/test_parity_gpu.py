@@ -180,7 +180,7 @@ def test_unsorted_scaled():
 def test_multimodal_sigs_requeued():
     # same-name kernels "differ in duration by several multiples" between positions.  A share of
     # the sigs gets a second mode 8-4096x the first: the compact cell refuses it, the event is re-queued into
-    # the CTA's spill region and folded by the second launch; a third mode (or an exhausted region) falls
+    # the CTA's spill region and folded at the flush of its rank-step; a third mode (or an exhausted region) falls
     # back to the overflow list.
     import dataclasses
     for name, kw, frac in (("mid", dict(n_ranks=24, n_steps=2), 0.5),
@@ -192,7 +192,7 @@ def test_multimodal_sigs_requeued():
         for grid, spill in ((None, ev.size), (7, ev.size // 16), (None, 0), (3, 1000)):
             assert_parity(ev, *_dims(wl.spec), path=PATH_SEG, grid=grid, spill=spill)
     # the invariant sweep of test_bucket_window_invariant_cells (five spread buckets in one sig: a chain of
-    # refusals in the second launch) with a spill area, chunked
+    # refusals in the replay) with a spill area, chunked
     wl = build_workload(dataclasses.replace(scaled("unsorted", n_ranks=32, n_events=6000), bimodal_frac=0.0))
     ev = wl.expand_host()
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False, spill=ev.size, cuts=[0, 50_001, ev.size])
