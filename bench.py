@@ -473,7 +473,7 @@ def run_ours(args, world):
         "clocks": clocks, "e2e": e2e,
         "gpu_launches": k1 - k0, "gpu_memsets": m1 - m0,     # counted by the library (argus_launch_count)
         # events a compact shared-memory cell refused (range wider than four log2 buckets, >= 2^32 ns), per step:
-        # re-queued through the spill area and a second launch / taken one by one by L2 reductions
+        # re-queued through the spill area and replayed at the flush of their rank-step / taken one by one by L2 reductions
         "counters": {"n_valid": n_valid, "n_invalid": n_invalid, "n_requeued": n_requeued,
                      "n_overflow": n_overflow, "requeued_frac": n_requeued / max(1, n_valid),
                      "overflow_frac": n_overflow / max(1, n_valid)},

@@ -171,17 +171,75 @@ kde_hist_kernel(const uint32_t* __restrict__ hist, uint64_t n_cells, argus_kde_p
            density ? density + cell * P.n_bins : nullptr);
 }
 
-// the 32-bucket histograms of the finalised record table (per_octave = 1, n_bins = 32)
-__global__ void __launch_bounds__(256)
+// The 32-bucket histograms of the finalised record table (per_octave = 1, n_bins = 32).  A valley needs a bin
+// strictly inside the occupied range (R27): a cell whose occupied buckets span fewer than three (nearly every
+// cell: the compact cells of the aggregation hold four buckets at most, and 10 % jitter fills one or two) is ONE
+// cluster whatever its density looks like, and its (count, p50, p99) are integer work — one thread does it,
+// no floating point but the ceil(0.99 count) the wide path takes too.  The other cells are queued in shared
+// memory and get the full KDE, one warp each (kde_cell), in the second half of the kernel.
+constexpr int KDE_REC_NT = 256;
+__global__ void __launch_bounds__(KDE_REC_NT)
 kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_params P, argus_cluster* clusters,
                    uint8_t* n_clusters) {
-  __shared__ KdeSmem sm[8];
-  const uint64_t cell = (uint64_t)blockIdx.x * 8u + (threadIdx.x >> 5);
-  if (cell >= (uint64_t)D.R * D.T * D.S) return;
-  const uint64_t rec = cell / D.S;
-  const uint32_t sig = (uint32_t)(cell % D.S);
-  const argus_cell* c = reinterpret_cast<const argus_cell*>(records + rec * D.rec_bytes + D.cell_off) + sig;
-  kde_cell(c->hist, P, sm[threadIdx.x >> 5], clusters + cell * P.max_clusters, n_clusters + cell, nullptr);
+  __shared__ KdeSmem sm[KDE_REC_NT / 32];
+  __shared__ uint32_t s_wide[KDE_REC_NT];
+  __shared__ uint32_t s_nwide;
+  const uint64_t n_cells = (uint64_t)D.R * D.T * D.S;
+  const uint64_t cell0 = (uint64_t)blockIdx.x * KDE_REC_NT;
+  if (threadIdx.x == 0) s_nwide = 0u;
+  __syncthreads();
+  const uint64_t cell = cell0 + threadIdx.x;
+  if (cell < n_cells) {
+    const uint64_t rec = cell / D.S;
+    const uint32_t sig = (uint32_t)(cell - rec * D.S);
+    const argus_cell* c = reinterpret_cast<const argus_cell*>(records + rec * D.rec_bytes + D.cell_off) + sig;
+    const uint4* h4 = reinterpret_cast<const uint4*>(c->hist);
+    uint32_t lo = 32u, hi = 0u;
+    unsigned long long n = 0ull;
+#pragma unroll
+    for (uint32_t q = 0; q < 8u; ++q) {
+      const uint4 v = __ldg(h4 + q);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (uint32_t k = 0; k < 4u; ++k) {
+        if (w[k]) {
+          const uint32_t b = 4u * q + k;
+          n += w[k];
+          lo = b < lo ? b : lo;
+          hi = b;
+        }
+      }
+    }
+    if (n != 0ull && hi - lo >= 2u) {
+      s_wide[atomicAdd(&s_nwide, 1u)] = threadIdx.x;
+    } else {
+      argus_cluster* out = clusters + cell * P.max_clusters;
+      argus_cluster first;
+      first.count = 0u; first.p50_bin = 0; first.p99_bin = 0;
+      if (n != 0ull) {
+        const unsigned long long t50 = (n + 1ull) / 2ull, t99 = (unsigned long long)ceil(0.99 * (double)n);
+        const unsigned long long c_lo = c->hist[lo];
+        first.count = (uint32_t)n;
+        first.p50_bin = (uint16_t)(c_lo >= t50 ? lo : hi);
+        first.p99_bin = (uint16_t)(c_lo >= t99 ? lo : hi);
+      }
+      out[0] = first;
+      argus_cluster z;
+      z.count = 0u; z.p50_bin = 0; z.p99_bin = 0;
+      for (uint32_t k = 1; k < P.max_clusters; ++k) out[k] = z;
+      n_clusters[cell] = n != 0ull ? 1 : 0;
+    }
+  }
+  __syncthreads();
+  const uint32_t n_wide = s_nwide;
+  for (uint32_t i = threadIdx.x >> 5; i < n_wide; i += KDE_REC_NT / 32) {
+    const uint64_t wc = cell0 + s_wide[i];
+    const uint64_t rec = wc / D.S;
+    const uint32_t sig = (uint32_t)(wc - rec * D.S);
+    const argus_cell* c = reinterpret_cast<const argus_cell*>(records + rec * D.rec_bytes + D.cell_off) + sig;
+    kde_cell(c->hist, P, sm[threadIdx.x >> 5], clusters + wc * P.max_clusters, n_clusters + wc, nullptr);
+    __syncwarp();
+  }
 }
 
 // clusters [R][T][S][mc] (rank-major, as argus_kde_clusters_records writes them) -> the L3 input
@@ -628,8 +686,8 @@ cudaError_t argus_launch_kde_hist(argus_ctx* ctx, const uint32_t* d_hist, uint64
 cudaError_t argus_launch_kde_records(argus_ctx* ctx, const void* d_records, const argus_kde_params* P,
                                      argus_cluster* d_clusters, uint8_t* d_n, cudaStream_t s) {
   const uint64_t n_cells = (uint64_t)ctx->dims.R * ctx->dims.T * ctx->dims.S;
-  kde_records_kernel<<<(unsigned)((n_cells + 7) / 8), 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, *P,
-                                                                   d_clusters, d_n);
+  kde_records_kernel<<<(unsigned)((n_cells + KDE_REC_NT - 1) / KDE_REC_NT), KDE_REC_NT, 0, s>>>(
+      static_cast<const uint8_t*>(d_records), ctx->dims, *P, d_clusters, d_n);
   ctx->n_kernels += 1;
   return cudaGetLastError();
 }
