@@ -212,7 +212,7 @@ def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=512, fine_limit_bytes=6 <
     ms, best = timed(lambda: ctx.kde_clusters_records(rec, p32, d_c, d_n))
     ncl = d_n.to(torch.int64)
     n_clusters = int(ncl.sum())
-    out["next1_kde_records"] = line(ms, best, n_cells * (128 + 8 * MC + 1), "alu (fp64 exp per occupied bin pair)",
+    out["next1_kde_records"] = line(ms, best, n_cells * (128 + 8 * MC + 1), "hbm (a thread per narrow cell; fp64 exp only for cells that can hold a valley)",
                                     cells=n_cells, cells_per_s=n_cells / (ms * 1e-3), clusters=n_clusters,
                                     cells_with_2plus=int((ncl >= 2).sum()))
     # NEXT-4b record encodings: read the table once, write the stream
