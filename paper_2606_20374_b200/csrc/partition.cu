@@ -3,22 +3,25 @@
 //
 // Folding shuffled events straight into a dense table that is far larger than L2 costs several
 // random 32-byte read-modify-writes in HBM per event (aggregate_global.cu: 6 G events/s).  Moving
-// each 32-byte record ONCE to its (rank, step) group costs two sequential reads (count, scatter) and
-// one sector-sized write (a single 256-bit store) that L2 merges into full lines — after which the
-// segmented kernel runs at streaming speed.
-// Kernels, all on the caller's stream; key = rank*T + step - step_base, and
-// key-invalid events go to bin R*T:
-//   count   : every CTA owns a contiguous chunk of the buffer and counts its keys in a shared-memory
-//             histogram (no global atomics), then writes its row H[cta][key]
-//   offsets : per key, exclusive running sum over the CTAs (H[cta][key] becomes the CTA's offset
-//             inside the key's group) and the group size total[key]
-//   scan    : exclusive prefix sum of total in place (one CTA, running carry)
-//   scatter : the same CTA re-reads its chunk with cursor[key] = total[key] + H[cta][key] in shared
-//             memory: pos = atomicAdd(&cursor[key], 1); grouped[pos] = event (one 256-bit store)
-// When R*T + 1 counters do not fit shared memory, count and scatter use L2 atomics on one global
-// counter array instead (same results, slower).  All buffers are areas of the ctx workspace.
-// Events whose key fields are out of range travel in the last bin, so that the segmented kernel
-// still sees (and counts) every event; sig / phase / timestamp validity is its business.
+// each record to its (rank, step) group first lets the segmented kernel run on contiguous segments.
+// key = rank*T + step - step_base.  Three layouts of the pass, chosen per table geometry when the
+// context is created; all buffers are areas of the caller's workspace:
+//   two-level (R*T <= 24576, the default; second half of this file): count, scan, a coarse pass into
+//             <= 256 bins of 16-byte packed events, a fine pass back to raw events per key, pad —
+//             every tile counting-sorted in shared memory and written out as contiguous runs
+//   single scatter, shared-memory cursors (R*T + 1 counters fit shared memory):
+//     count   : every CTA owns a contiguous chunk of the buffer and counts its keys in a shared-memory
+//               histogram (no global atomics), then writes its row H[cta][key]
+//     offsets : per key, exclusive running sum over the CTAs (H[cta][key] becomes the CTA's offset
+//               inside the key's group) and the group size total[key]
+//     scan    : exclusive prefix sum of total in place (one CTA, running carry)
+//     scatter : the same CTA re-reads its chunk with cursor[key] = total[key] + H[cta][key] in shared
+//               memory: pos = atomicAdd(&cursor[key], 1); grouped[pos] = event (one 256-bit store)
+//   single scatter, global cursors (anything larger): count and scatter use L2 atomics on one global
+//             counter array (same results, slower)
+// In the single-scatter layouts key-invalid events go to bin R*T, in the two-level layout invalid events
+// are dropped and re-appear as padding: either way the segmented kernel still sees (and counts) every
+// event of the call; sig / phase / timestamp validity is its business.
 #include "argus_internal.cuh"
 
 namespace {
