@@ -268,7 +268,7 @@ __device__ __forceinline__ double normal_cdf(double z) { return 0.5 * erfc(-z * 
 extern __shared__ unsigned char l3_smem[];
 
 // bitonic sort of n (power of two) doubles with their payload, ascending; all threads of the CTA call
-__device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
+__device__ void bitonic_sort_simple(double* v, uint16_t* id, uint32_t n) {
   for (uint32_t k = 2; k <= n; k <<= 1) {
     for (uint32_t j = k >> 1; j > 0; j >>= 1) {
       for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
@@ -281,6 +281,55 @@ __device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
             const uint16_t t = id[i]; id[i] = id[p]; id[p] = t;
           }
         }
+      }
+      __syncthreads();
+    }
+  }
+}
+
+// The same network, four elements per thread: a thread that holds {i, i^jb, i^j, i^j^jb} (jb = j/2) runs the
+// stages j and j/2 in registers, so two stages cost one trip through shared memory and one barrier (42 passes
+// instead of 78 stages at n = 4096; every thread busy instead of half of them).  Identical compare-exchanges,
+// hence identical output (ties included).  n >= 4, n / 4 <= blockDim.x.
+__device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
+  if (n < 4u || (n >> 2) > blockDim.x) { bitonic_sort_simple(v, id, n); return; }
+  const uint32_t t = threadIdx.x, nt = n >> 2;
+  for (uint32_t k = 2; k <= n; k <<= 1) {
+    uint32_t j = k >> 1;
+    while (j >= 2u) {
+      if (t < nt) {
+        const uint32_t jb = j >> 1, b = (uint32_t)__ffs((int)jb) - 1u;
+        const uint32_t base = ((t >> b) << (b + 2u)) | (t & (jb - 1u));
+        const bool up = (base & k) == 0u;
+        const uint32_t e[4] = {base, base | jb, base | j, base | j | jb};
+        double x[4];
+        uint16_t q[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { x[a] = v[e[a]]; q[a] = id[e[a]]; }
+#define ARGUS_CE(a, c)                                                         \
+  if ((x[a] > x[c]) == up && x[a] != x[c]) {                                   \
+    const double tx = x[a]; x[a] = x[c]; x[c] = tx;                            \
+    const uint16_t tq = q[a]; q[a] = q[c]; q[c] = tq;                          \
+  }
+        ARGUS_CE(0, 2) ARGUS_CE(1, 3) ARGUS_CE(0, 1) ARGUS_CE(2, 3)
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { v[e[a]] = x[a]; id[e[a]] = q[a]; }
+      }
+      __syncthreads();
+      j >>= 2;
+    }
+    if (j == 1u) {
+      if (t < nt) {
+        const uint32_t i = 4u * t;
+        double x[4];
+        uint16_t q[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { x[a] = v[i + a]; q[a] = id[i + a]; }
+        { const bool up = (i & k) == 0u; ARGUS_CE(0, 1) }
+        { const bool up = ((i + 2u) & k) == 0u; ARGUS_CE(2, 3) }
+#undef ARGUS_CE
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { v[i + a] = x[a]; id[i + a] = q[a]; }
       }
       __syncthreads();
     }
@@ -384,10 +433,12 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
   __syncthreads();
   const bool empty = !(s_hi > 0.0);
   if (!empty) {
-    // per-thread totals and, when they fit, the cached parameters of this thread's (rank, cluster) pairs
-    const uint32_t per_thread = (n2 + blockDim.x - 1u) / blockDim.x;      // ranks per thread, <= 4
-    const bool cached = per_thread * C <= (uint32_t)L3_CACHE;
+    // per-thread totals and, when they fit, the cached parameters of this thread's NON-EMPTY (rank, cluster)
+    // pairs in (rank slot, cluster) order — the order the sums below take; a thread with more than L3_CACHE of
+    // them recomputes its parameters at every grid point
     L3Par par[L3_CACHE];
+    uint32_t slot[L3_CACHE];
+    uint32_t n_ent = 0;
     double tot[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
     for (int a = 0; a < 4; ++a) {
@@ -395,15 +446,26 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
       if (r < R)
         for (uint32_t c = 0; c < C; ++c) tot[a] += (double)cnt[r * C + c];
     }
-    if (cached) {
 #pragma unroll
-      for (int q = 0; q < L3_CACHE; ++q) {
-        const uint32_t a = (uint32_t)q / C, c = (uint32_t)q % C;
-        const uint32_t r = threadIdx.x + a * blockDim.x;
-        par[q].mu = 0.0; par[q].isg = 0.0; par[q].w = 0.0;
-        if (a < per_thread && r < R && cnt[r * C + c]) par[q] = l3_par(cnt[r * C + c], tot[a], p50[r * C + c], p99[r * C + c]);
-      }
+    for (int q = 0; q < L3_CACHE; ++q) { par[q].mu = 0.0; par[q].isg = 0.0; par[q].w = 0.0; slot[q] = 4u; }
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      const uint32_t r = threadIdx.x + (uint32_t)a * blockDim.x;
+      if (r < R && tot[a] > 0.0)
+        for (uint32_t c = 0; c < C; ++c) {
+          const uint32_t k = cnt[r * C + c];
+          if (k) {
+            if (n_ent < (uint32_t)L3_CACHE) {
+              const L3Par v = l3_par(k, tot[a], p50[r * C + c], p99[r * C + c]);
+#pragma unroll
+              for (int q = 0; q < L3_CACHE; ++q)
+                if ((uint32_t)q == n_ent) { par[q] = v; slot[q] = (uint32_t)a; }
+            }
+            ++n_ent;
+          }
+        }
     }
+    const bool cached = n_ent <= (uint32_t)L3_CACHE;
     const double llo = log(0.5 * s_lo), lhi = log(2.0 * s_hi);
     for (uint32_t j = 0; j < G; ++j) {
       const double lx = llo + (lhi - llo) * (double)j / (double)(G - 1u);
@@ -414,30 +476,48 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
       const double wj = 0.5 * (xp - xm);
       // F_r(x_j), eq. (2); log(x) of the oracle is log(exp(lx)): take it the same way
       const double lgx = log(x);
+      double Fa[4] = {0.0, 0.0, 0.0, 0.0};
+      if (cached) {
+#pragma unroll
+        for (int q = 0; q < L3_CACHE; ++q) {
+          if (slot[q] < 4u) {
+            const double tq = l3_term(par[q], lgx);
+#pragma unroll
+            for (int a = 0; a < 4; ++a) if (slot[q] == (uint32_t)a) Fa[a] += tq;
+          }
+        }
+      } else {
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+          const uint32_t r = threadIdx.x + (uint32_t)a * blockDim.x;
+          if (r < R && tot[a] > 0.0)
+            for (uint32_t c = 0; c < C; ++c) {
+              const uint32_t k = cnt[r * C + c];
+              if (k) Fa[a] += l3_term(l3_par(k, tot[a], p50[r * C + c], p99[r * C + c]), lgx);
+            }
+        }
+      }
+      bool same = true;                            // every value of this thread equals rank 0's?
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
         const uint32_t r = threadIdx.x + (uint32_t)a * blockDim.x;
-        if (r >= n2) break;
-        double F = INFINITY;                       // padding sorts to the end
-        if (r < R) {
-          F = 0.0;
-          if (tot[a] > 0.0) {
-            if (cached) {
-#pragma unroll
-              for (int q = 0; q < L3_CACHE; ++q)
-                if ((uint32_t)q / C == (uint32_t)a && (uint32_t)q < per_thread * C) F += l3_term(par[q], lgx);
-            } else {
-              for (uint32_t c = 0; c < C; ++c) {
-                const uint32_t k = cnt[r * C + c];
-                if (k) F += l3_term(l3_par(k, tot[a], p50[r * C + c], p99[r * C + c]), lgx);
-              }
-            }
-          }
+        if (r < n2) {
+          val[r] = r < R ? Fa[a] : INFINITY;       // padding sorts to the end
+          id[r] = (uint16_t)r;
         }
-        val[r] = F;
-        id[r] = (uint16_t)r;
       }
       __syncthreads();
+      {
+        const double f0 = val[0];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+          const uint32_t r = threadIdx.x + (uint32_t)a * blockDim.x;
+          if (r < R) same = same && Fa[a] == f0;
+        }
+      }
+      // all ranks agree at this grid point (below every distribution, above every one, or identical triples):
+      // every |F_a - F_b| is 0, nothing to sort and nothing to add
+      if (__syncthreads_and(same)) continue;
       bitonic_sort(val, id, n2);
       // sum_b |F_r - F_b| at every sorted position, from the gaps
       double d[4];
@@ -712,7 +792,12 @@ cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l
   const size_t smem = argus_l3_smem_bytes(in->n_ranks);
   cudaError_t e = cudaFuncSetAttribute(l3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  l3_kernel<<<in->n_keys, 1024, smem, s>>>(*in, *P, d_score, d_stat, d_flags);
+  // one CTA per key: every thread owns <= 4 ranks, and a rank each in the scan when R <= 1024 — small jobs get
+  // small CTAs, so that several keys share an SM
+  uint32_t n2 = 1;
+  while (n2 < in->n_ranks) n2 <<= 1;
+  const unsigned threads = n2 >= 1024u ? 1024u : (n2 < 64u ? 64u : n2);
+  l3_kernel<<<in->n_keys, threads, smem, s>>>(*in, *P, d_score, d_stat, d_flags);
   ctx->n_kernels += 1;
   return cudaGetLastError();
 }
