@@ -45,13 +45,17 @@ fine_hist_kernel(const uint4* __restrict__ ev, uint64_t n, argus_dims D, uint32_
 
 // ---- NEXT-1: KDE -> valleys -> filters -> triples, one warp per histogram ---------------------------------
 constexpr int KDE_MAX_BINS = 256;
-struct KdeSmem {
-  double f[KDE_MAX_BINS];
-  uint32_t c[KDE_MAX_BINS];
+template <int NB>
+struct KdeSmemT {
+  double f[NB];
+  double e[NB];                  // kernel weight by distance in grid steps
+  uint32_t c[NB];
 };
+typedef KdeSmemT<KDE_MAX_BINS> KdeSmem;
 
 // hist: n_bins counters of this cell (global, stride 1).  Lanes share the grid points; lane 0 walks the valleys.
-__device__ void kde_cell(const uint32_t* __restrict__ hist, const argus_kde_params& P, KdeSmem& sm,
+template <class SM>
+__device__ void kde_cell(const uint32_t* __restrict__ hist, const argus_kde_params& P, SM& sm,
                          argus_cluster* __restrict__ out, uint8_t* __restrict__ out_n, double* __restrict__ dens) {
   const int lane = threadIdx.x & 31;
   const uint32_t nb = P.n_bins;
@@ -100,16 +104,21 @@ __device__ void kde_cell(const uint32_t* __restrict__ hist, const argus_kde_para
       const double norm = 1.0 / (n * h * 2.5066282746310002);         // 1 / (n h sqrt(2 pi)): eq. (1), R22
       // the density is needed where valleys can lie: the occupied range (it is tabulated on the whole grid
       // only when the caller asks for it)
+      // The grid is equally spaced, so the kernel weight of a (grid point, sample bin) pair depends on their
+      // distance in grid steps only: tabulate K(d step / h) once per distance (hi - lo + 1 values of exp for
+      // the occupied range instead of its square; sm.e) and sum with it, in bin order as before.
       const uint32_t j0 = dens ? 0u : lo, j1 = dens ? nb - 1u : hi;
+      const uint32_t dmax = (j1 > hi ? j1 - lo : hi - lo) > (hi - j0) ? (j1 > hi ? j1 - lo : hi - lo) : (hi - j0);
+      for (uint32_t d = lane; d <= dmax; d += 32) {
+        const double u = ((double)d * step) / h;
+        sm.e[d] = exp(-0.5 * u * u);
+      }
+      __syncwarp();
       for (uint32_t j = j0 + lane; j <= j1; j += 32) {
-        const double xj = ((double)j + 0.5) * step;
         double acc = 0.0;
         for (uint32_t b = lo; b <= hi; ++b) {
           const uint32_t c = sm.c[b];
-          if (c) {
-            const double u = (xj - ((double)b + 0.5) * step) / h;
-            acc += (double)c * exp(-0.5 * u * u);
-          }
+          if (c) acc += (double)c * sm.e[j > b ? j - b : b - j];
         }
         sm.f[j] = acc * norm;
       }
@@ -181,7 +190,7 @@ constexpr int KDE_REC_NT = 256;
 __global__ void __launch_bounds__(KDE_REC_NT)
 kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_params P, argus_cluster* clusters,
                    uint8_t* n_clusters) {
-  __shared__ KdeSmem sm[KDE_REC_NT / 32];
+  __shared__ KdeSmemT<32> sm[KDE_REC_NT / 32];
   __shared__ uint32_t s_wide[KDE_REC_NT];
   __shared__ uint32_t s_nwide;
   const uint64_t n_cells = (uint64_t)D.R * D.T * D.S;

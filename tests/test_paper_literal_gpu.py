@@ -202,6 +202,55 @@ def test_l3_scores_and_fence(R, C, K, G):
     ctx.close()
 
 
+@pytest.mark.parametrize("R,C,G", [(4096, 2, 24), (1500, 3, 16), (1024, 1, 16)])
+def test_l3_large_rank_counts_sampled(R, C, G):
+    """The launch shapes of the full-size job (1,024 threads, 2 or 4 sorted positions per thread, every cached /
+    uncached parameter path): the oracle's R x R matrix is out of reach, so the scores of SAMPLED ranks are
+    compared with the oracle's own mixture_cdf / w1 summed over all the other ranks, the quartiles and the fence
+    with numpy's percentile of the kernel's scores (R33's definition), the flags with score > fence."""
+    import torch
+    from paper_2606_20374_b200 import argus as A
+    rnd = np.random.default_rng(7 + R)
+    K = 2
+    cnt = np.zeros((K, R, C), dtype=np.uint32)
+    p50 = np.ones((K, R, C), dtype=np.float64)
+    p99 = np.ones((K, R, C), dtype=np.float64)
+    for k in range(K):
+        base = 5e4 * (25.0 ** np.arange(C))
+        have = rnd.random((R, C)) < (0.95 if k == 0 else 0.6)          # key 1: many ranks lack a cluster
+        cnt[k] = np.where(have, rnd.integers(1, 4000, (R, C)), 0)
+        p50[k] = base * (1 + 0.03 * rnd.random((R, C)))
+        p99[k] = p50[k] * np.where(rnd.random((R, C)) < 0.15, 1.0, 1 + 0.5 * rnd.random((R, C)))
+        p50[k, 17] *= 1.7; p99[k, 17] *= 1.7                           # one rank is slow on every cluster
+        cnt[k, 17] = np.maximum(cnt[k, 17], 1)
+        cnt[k, 33] = 0                                                 # one rank never ran the kernel
+    ctx = A.Argus(1, 1, 1, 1)
+    d_score = torch.zeros(K * R, dtype=torch.float64, device="cuda")
+    d_stat = torch.zeros(K * 5, dtype=torch.float64, device="cuda")
+    d_flags = torch.full((K * R,), 7, dtype=torch.uint8, device="cuda")
+    ctx.l3_detect(_cuda(cnt), _cuda(p50), _cuda(p99), K, R, C, d_score, d_stat, d_flags, n_grid=G, alpha=1.5)
+    score = d_score.cpu().numpy().reshape(K, R)
+    stat = d_stat.cpu().numpy().view(A.L3_STAT_DTYPE).reshape(K)
+    flags = d_flags.cpu().numpy().reshape(K, R)
+    for k in range(K):
+        tr = [[(int(cnt[k, r, c]), float(p50[k, r, c]), float(p99[k, r, c])) for c in range(C)] for r in range(R)]
+        live = [(t[1], t[2]) for row in tr for t in row if t[0] > 0]
+        xs = PL.log_grid(0.5 * min(a for a, _ in live), 2.0 * max(b for _, b in live), G)
+        assert stat[k]["x_lo"] == pytest.approx(xs[0], rel=1e-12) and stat[k]["x_hi"] == pytest.approx(xs[-1], rel=1e-12)
+        F = np.stack([PL.mixture_cdf(row, xs) for row in tr])
+        scale = float(score[k].max())
+        for r in [0, 1, 17, 33, R // 2, R - 1] + [int(v) for v in rnd.integers(0, R, 10)]:
+            want = sum(PL.w1(F[r], F[b], xs) for b in range(R) if b != r) / (R - 1)
+            assert score[k, r] == pytest.approx(want, rel=1e-8, abs=1e-9 * scale), (k, r)
+        q1, q3 = np.percentile(score[k], [25.0, 75.0])
+        assert stat[k]["q1"] == pytest.approx(q1, rel=1e-12) and stat[k]["q3"] == pytest.approx(q3, rel=1e-12)
+        fence = q3 + 1.5 * (q3 - q1)
+        assert stat[k]["fence"] == pytest.approx(fence, rel=1e-12)
+        assert (flags[k] == (score[k] > stat[k]["fence"])).all()
+        assert np.isfinite(score[k]).all() and (score[k] >= 0).all()
+    ctx.close()
+
+
 def test_events_to_l3_end_to_end():
     """The paper's whole L3 route on one table (PAPER.md:176-198 then 234-251): events -> fine histograms ->
     clusters (argus_kde_clusters) -> regrouped triples in ns (argus_clusters_to_l3) -> scores, fence, flags
