@@ -378,12 +378,15 @@ __device__ __forceinline__ uint32_t warp_median(const uint32_t (&v)[VPL], uint32
   return lo + (hi - lo) / 2u;
 }
 
-template <int VPL>
-__global__ void __launch_bounds__(256)
+// WPC warps per CTA.  The kernel is a chain of dependent warp-wide steps per series (latency, not bandwidth):
+// what helps is more resident warps.  R <= 256 keeps 8 values per lane, fits 56 registers and runs 9 CTAs of 4
+// warps per SM, so that the 5,210 series of `mid` are ONE wave of 148 x 36 warps instead of one and a half.
+template <int VPL, int WPC, int MINB>
+__global__ void __launch_bounds__(WPC * 32, MINB)
 diagnose_warp_kernel(DiagSrc src, argus_dims D, argus_diag_out out, uint8_t* __restrict__ todo, uint32_t n_series) {
-  __shared__ uint32_t s_hist[8][256];
+  __shared__ uint32_t s_hist[WPC][256];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const uint32_t series_id = blockIdx.x * 8u + (uint32_t)w;
+  const uint32_t series_id = blockIdx.x * (uint32_t)WPC + (uint32_t)w;
   if (series_id >= n_series) return;
   uint32_t* hist = s_hist[w];
   const uint32_t F = D.S + D.P + 1u;
@@ -484,10 +487,10 @@ static cudaError_t launch_select(argus_ctx* ctx, const DiagSrc& src, const argus
   // that span 2^32 or more (marked in todo) in 64 bits, by a handful of CTAs that walk the marks
   const unsigned wide_grid = nb < (unsigned)ctx->sm_count * 2u ? nb : (unsigned)ctx->sm_count * 2u;
   if (D.R <= 256u) {
-    diagnose_warp_kernel<8><<<(nb + 7u) / 8u, 256, 0, s>>>(src, D, *o, todo, nb);
+    diagnose_warp_kernel<8, 4, 9><<<(nb + 3u) / 4u, 128, 0, s>>>(src, D, *o, todo, nb);
     diagnose_kernel<64, unsigned long long><<<wide_grid, 64, 0, s>>>(src, D, *o, todo, nb);
   } else if (D.R <= 1024u) {
-    diagnose_warp_kernel<32><<<(nb + 7u) / 8u, 256, 0, s>>>(src, D, *o, todo, nb);
+    diagnose_warp_kernel<32, 8, 1><<<(nb + 7u) / 8u, 256, 0, s>>>(src, D, *o, todo, nb);
     diagnose_kernel<64, unsigned long long><<<wide_grid, 64, 0, s>>>(src, D, *o, todo, nb);
   } else if (D.R <= 256u * EPT) {
     diagnose_kernel<256, uint32_t><<<nb, 256, 0, s>>>(src, D, *o, todo, nb);
