@@ -734,6 +734,15 @@ aggregate_seg_kernel(const __grid_constant__ CUtensorMap tmap, const uint4* __re
         ws.n += 32u;                       // warp-uniform count
         return;
       }
+      if (__all_sync(FULL, ok) && !__all_sync(FULL, phase == __shfl_sync(FULL, phase, 0))) {
+        // every event folded, phases mixed inside the warp (input that was grouped by key but not by time:
+        // the output of the grouping pass): the shared span accumulators lane by lane, nothing else to do
+        SpanAcc* sp = span_tab() + phase;
+        if (start < *reinterpret_cast<volatile long long*>(&sp->mn)) atomicMin(&sp->mn, start);
+        if (end > *reinterpret_cast<volatile long long*>(&sp->mx)) atomicMax(&sp->mx, end);
+        atomicAdd(reinterpret_cast<uint32_t*>(&sp->n), 1u);
+        return;
+      }
       pending = true; tried = true;        // a refused event or a phase change: general handling below
     } else {
       // full validity (R2, R3) of the lanes that failed the fast test
