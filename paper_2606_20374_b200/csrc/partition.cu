@@ -148,7 +148,7 @@ partition_scatter_smem_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t
 // ==== two-level grouping (the default when R*T <= P2_MAX_KEYS) =========================================
 // A single scatter into R*T groups leaves every CTA with thousands of open 32-byte write streams: L2
 // evicts the lines before they fill and HBM sees row-missing sector writes (2.1 TB/s).
-// Two levels of at most 256 bins each, every tile of 2048 events counting-sorted in shared memory and copied
+// Two levels of at most 256 bins each, every tile of 1024 events counting-sorted in shared memory and copied
 // out as runs of whole lines reserved with ONE global atomic per (tile, bin), stream instead:
 //   count   valid events per key (shared-memory histogram per CTA, merged with L2 atomics) and packable
 //           events per coarse bin (key >> shift)
@@ -160,7 +160,6 @@ partition_scatter_smem_kernel(const uint4* __restrict__ ev, uint64_t n, uint64_t
 //           method, R16) grouped by key
 //   pad     the n - n_valid slots behind the grouped events become invalid records (rank 2^32 - 1), so that
 //           the segmented kernel still sees and counts every event of the call
-constexpr uint32_t P2_TILE = 2048, P2_NT = 512, P2_EPT = P2_TILE / P2_NT;
 constexpr uint32_t P2_MAX_BINS = 256;
 
 struct P2Small {          // small device-side state of one grouping pass (in the `part` area of the workspace)
@@ -266,9 +265,8 @@ struct P2SharedT {
   uint32_t n_packed, unused;
   uint8_t binof[TILE];
 };
-typedef P2SharedT<P2_TILE> P2Shared;
 
-// exclusive scan of cnt[0..256) by the first 256 threads (all P2_NT threads call); also resets cnt
+// exclusive scan of cnt[0..256) by the first 256 threads (all threads of the CTA call; NT >= 256); also resets cnt
 template <class SH>
 __device__ __forceinline__ void p2_bins_scan(SH* S, uint32_t& my_cnt, uint32_t& my_pre) {
   const uint32_t t = threadIdx.x;
@@ -288,25 +286,36 @@ __device__ __forceinline__ void p2_bins_scan(SH* S, uint32_t& my_cnt, uint32_t& 
   if (t < P2_MAX_BINS) { S->off[t] = my_pre; S->cnt[t] = 0u; }
 }
 
-__global__ void __launch_bounds__(P2_NT, 3)
+template <uint32_t NT, uint32_t EPT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
 p2_coarse_kernel(const uint4* __restrict__ ev, uint64_t n, argus_dims D, uint32_t shift, uint32_t* __restrict__ kcur,
                  P2Small* __restrict__ sm, uint4* __restrict__ coarse, uint4* __restrict__ grouped) {
+  constexpr uint32_t TILE = NT * EPT;
+  typedef P2SharedT<TILE> SH;
   extern __shared__ __align__(16) uint8_t p2_smem[];
-  P2Shared* S = reinterpret_cast<P2Shared*>(p2_smem);
-  uint4* sorted = reinterpret_cast<uint4*>(p2_smem + ((sizeof(P2Shared) + 15u) & ~15u));
-  for (uint32_t k = threadIdx.x; k < P2_MAX_BINS; k += P2_NT) S->cnt[k] = 0u;
+  SH* S = reinterpret_cast<SH*>(p2_smem);
+  uint4* sorted = reinterpret_cast<uint4*>(p2_smem + ((sizeof(SH) + 15u) & ~15u));
+  for (uint32_t k = threadIdx.x; k < P2_MAX_BINS; k += NT) S->cnt[k] = 0u;
   __syncthreads();
-  const uint64_t n_tiles = (n + P2_TILE - 1) / P2_TILE;
-  for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    uint4 pk[P2_EPT];
-    uint32_t where[P2_EPT];                       // bin << 16 | position inside the tile's bin; ~0 = not packed
-    const uint64_t base = tile * P2_TILE;
+  const uint64_t n_tiles = (n + TILE - 1) / TILE;
+  // software pipeline: the raw events of the NEXT tile are requested before this tile is sorted and copied out
+  uint4 nlo[EPT], nhi[EPT];
 #pragma unroll
-    for (uint32_t j = 0; j < P2_EPT; ++j) {
-      const uint64_t i = base + j * P2_NT + threadIdx.x;
+  for (uint32_t j = 0; j < EPT; ++j) {
+    const uint64_t i = (uint64_t)blockIdx.x * TILE + j * NT + threadIdx.x;
+    nlo[j] = make_uint4(0u, 0u, 0u, 0u); nhi[j] = nlo[j];
+    if (i < n) { nlo[j] = ldcs128(ev + 2 * i); nhi[j] = ldcs128(ev + 2 * i + 1); }
+  }
+  for (uint64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    uint4 pk[EPT];
+    uint32_t where[EPT];                          // bin << 16 | position inside the tile's bin; ~0 = not packed
+    const uint64_t base = tile * TILE;
+#pragma unroll
+    for (uint32_t j = 0; j < EPT; ++j) {
+      const uint64_t i = base + j * NT + threadIdx.x;
       where[j] = 0xFFFFFFFFu;
       if (i < n) {
-        const uint4 lo = ldcs128(ev + 2 * i), hi = ldcs128(ev + 2 * i + 1);
+        const uint4 lo = nlo[j], hi = nhi[j];
         uint32_t key; bool packable;
         if (p2_decode(D, lo, hi, key, packable)) {
           if (packable) {
@@ -321,6 +330,11 @@ p2_coarse_kernel(const uint4* __restrict__ ev, uint64_t n, argus_dims D, uint32_
         }
       }
     }
+#pragma unroll
+    for (uint32_t j = 0; j < EPT; ++j) {
+      const uint64_t i = (tile + gridDim.x) * TILE + j * NT + threadIdx.x;
+      if (i < n) { nlo[j] = ldcs128(ev + 2 * i); nhi[j] = ldcs128(ev + 2 * i + 1); }
+    }
     __syncthreads();
     uint32_t c, pre;
     p2_bins_scan(S, c, pre);
@@ -328,7 +342,7 @@ p2_coarse_kernel(const uint4* __restrict__ ev, uint64_t n, argus_dims D, uint32_
     if (threadIdx.x == P2_MAX_BINS - 1u) S->n_packed = pre + c;   // packed events of this tile
     __syncthreads();
 #pragma unroll
-    for (uint32_t j = 0; j < P2_EPT; ++j) {
+    for (uint32_t j = 0; j < EPT; ++j) {
       if (where[j] != 0xFFFFFFFFu) {
         const uint32_t bin = where[j] >> 16, slot = S->off[bin] + (where[j] & 0xFFFFu);
         sorted[slot] = pk[j];
@@ -337,7 +351,7 @@ p2_coarse_kernel(const uint4* __restrict__ ev, uint64_t n, argus_dims D, uint32_
     }
     __syncthreads();
     const uint32_t m = S->n_packed;
-    for (uint32_t i = threadIdx.x; i < m; i += P2_NT) coarse[(size_t)S->gbase[S->binof[i]] + i] = sorted[i];
+    for (uint32_t i = threadIdx.x; i < m; i += NT) coarse[(size_t)S->gbase[S->binof[i]] + i] = sorted[i];
     __syncthreads();
   }
 }
@@ -357,14 +371,34 @@ p2_fine_kernel(const uint4* __restrict__ coarse, argus_dims D, uint32_t shift, u
   __syncthreads();
   const uint32_t n_tiles = s_tb[P2_MAX_BINS], RT = D.R * D.T, kpb = 1u << shift;
   uint32_t cur_bin = 0xFFFFFFFFu;
-  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    // the coarse bin of this tile: the last b with tiles_before[b] <= tile
+  // where tile `t` lives: its coarse bin (the last b with tiles_before[b] <= t), first slot and length
+  auto locate = [&](uint32_t t, uint32_t& bin, uint32_t& s0, uint32_t& m) {
     uint32_t lo_b = 0u, hi_b = P2_MAX_BINS - 1u;
     while (lo_b < hi_b) {
       const uint32_t mid = (lo_b + hi_b + 1u) >> 1;
-      if (s_tb[mid] <= tile) lo_b = mid; else hi_b = mid - 1u;
+      if (s_tb[mid] <= t) lo_b = mid; else hi_b = mid - 1u;
     }
-    const uint32_t bin = lo_b;
+    bin = lo_b;
+    s0 = sm->cstart[bin] + (t - s_tb[bin]) * TILE;
+    const uint32_t s_end = sm->cstart[bin + 1u];
+    m = s_end - s0 < TILE ? s_end - s0 : TILE;
+  };
+  // software pipeline: the packed events of the NEXT tile are requested before this tile is sorted and copied
+  // out, so that their latency hides behind four barriers' worth of shared-memory work
+  uint4 nx[EPT];
+#pragma unroll
+  for (uint32_t j = 0; j < EPT; ++j) nx[j] = make_uint4(0u, 0u, 0u, 0u);
+  uint32_t nbin = 0u, ns0 = 0u, nm = 0u;
+  if (blockIdx.x < n_tiles) {
+    locate(blockIdx.x, nbin, ns0, nm);
+#pragma unroll
+    for (uint32_t j = 0; j < EPT; ++j) {
+      const uint32_t i = j * NT + threadIdx.x;
+      if (i < nm) nx[j] = ldcs128(coarse + (size_t)ns0 + i);
+    }
+  }
+  for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const uint32_t bin = nbin, m = nm;
     if (bin != cur_bin) {                          // block-uniform
       cur_bin = bin;
       for (uint32_t j = threadIdx.x; j < kpb; j += NT) {
@@ -373,18 +407,24 @@ p2_fine_kernel(const uint4* __restrict__ coarse, argus_dims D, uint32_t shift, u
         S->rank[j] = r; S->step[j] = D.step_base + (key - r * D.T);
       }
     }
-    const uint32_t s0 = sm->cstart[bin] + (tile - s_tb[bin]) * TILE, s_end = sm->cstart[bin + 1u];
-    const uint32_t m = s_end - s0 < TILE ? s_end - s0 : TILE;
     uint4 pk[EPT];
     uint32_t where[EPT];
 #pragma unroll
     for (uint32_t j = 0; j < EPT; ++j) {
       const uint32_t i = j * NT + threadIdx.x;
       where[j] = 0xFFFFFFFFu;
+      pk[j] = nx[j];
       if (i < m) {
-        pk[j] = ldcs128(coarse + (size_t)s0 + i);
         const uint32_t kib = pk[j].x >> 19;
         where[j] = (kib << 16) | atomicAdd(&S->cnt[kib], 1u);
+      }
+    }
+    if (tile + gridDim.x < n_tiles) {
+      locate(tile + gridDim.x, nbin, ns0, nm);
+#pragma unroll
+      for (uint32_t j = 0; j < EPT; ++j) {
+        const uint32_t i = j * NT + threadIdx.x;
+        if (i < nm) nx[j] = ldcs128(coarse + (size_t)ns0 + i);
       }
     }
     __syncthreads();
@@ -448,7 +488,21 @@ bool argus_partition2_plan(const argus_config* cfg, uint32_t* shift, size_t* sma
   return true;
 }
 
-static size_t p2_sorted_off() { return (sizeof(P2Shared) + 15u) & ~(size_t)15u; }
+template <uint32_t NT, uint32_t EPT, int MINB>
+static cudaError_t p2_coarse_go(argus_ctx* ctx, const uint4* src, uint64_t n, cudaStream_t s, bool configure) {
+  const size_t smem = ((sizeof(P2SharedT<NT * EPT>) + 15u) & ~(size_t)15u) + (size_t)NT * EPT * 16u;
+  if (configure)
+    return cudaFuncSetAttribute(p2_coarse_kernel<NT, EPT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  p2_coarse_kernel<NT, EPT, MINB><<<(unsigned)ctx->sm_count * MINB, NT, smem, s>>>(
+      src, n, ctx->dims, ctx->ws.part_shift, ctx->d_hist, reinterpret_cast<P2Small*>(ctx->d_part),
+      reinterpret_cast<uint4*>(ctx->d_coarse), reinterpret_cast<uint4*>(ctx->d_group));
+  return cudaGetLastError();
+}
+// coarse pass geometry: 256 threads x 4 events, three CTAs per SM.  Tiles of 512 events cost 20 % (128-byte
+// runs per bin), 2,048-event tiles leave too few CTAs for the prefetched loads (register budget).
+static cudaError_t p2_coarse_variant(argus_ctx* ctx, const uint4* src, uint64_t n, cudaStream_t s, bool configure) {
+  return p2_coarse_go<256, 4, 3>(ctx, src, n, s, configure);
+}
 
 template <uint32_t NT, uint32_t EPT, int MINB>
 static cudaError_t p2_fine_go(argus_ctx* ctx, const uint4* coarse, cudaStream_t s, bool configure, uint32_t* tile) {
@@ -461,20 +515,19 @@ static cudaError_t p2_fine_go(argus_ctx* ctx, const uint4* coarse, cudaStream_t 
       reinterpret_cast<uint4*>(ctx->d_group));
   return cudaGetLastError();
 }
-static uint32_t g_p2_tile = P2_TILE;
-// fine pass geometry: 512 threads x 4 events, three CTAs per SM (tiles of 1024 .. 2048 events and 2 .. 5 CTAs per
-// SM all measured within 5 %: the pass is bound by its 1 KB write runs, not by latency)
+static uint32_t g_p2_tile = 1024u;            // tile of the fine pass (set by its configure call)
+// fine pass geometry: 256 threads x 4 events, four CTAs per SM (64 registers hold the tile in hand and the
+// prefetched one).  Geometries from 128 x 4 x 8 to 512 x 4 x 2 measured within 3 % once the loads are
+// prefetched; without the prefetch the pass was 20 % slower at every geometry.
 static cudaError_t p2_fine_variant(argus_ctx* ctx, const uint4* coarse, uint64_t, cudaStream_t s, bool configure) {
-  return p2_fine_go<P2_NT, P2_EPT, 3>(ctx, coarse, s, configure, &g_p2_tile);
+  return p2_fine_go<256, 4, 4>(ctx, coarse, s, configure, &g_p2_tile);
 }
 
 cudaError_t argus_configure_partition(argus_ctx* ctx) {
   if (ctx->ws.part_two_level) {
     const int cnt_bytes = (int)(sizeof(uint32_t) * ((size_t)ctx->dims.R * ctx->dims.T + P2_MAX_BINS));
     cudaError_t e = cudaFuncSetAttribute(p2_count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, cnt_bytes);
-    if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(p2_coarse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               (int)(p2_sorted_off() + P2_TILE * 16u));
+    if (e == cudaSuccess) e = p2_coarse_variant(ctx, nullptr, 0, cudaStream_t(0), true);
     if (e == cudaSuccess) e = p2_fine_variant(ctx, nullptr, 0, cudaStream_t(0), true);
     return e;
   }
@@ -509,8 +562,8 @@ cudaError_t argus_launch_partition(argus_ctx* ctx, const argus_event* ev, uint64
     n_cta = (uint32_t)((n + chunk - 1) / chunk);
     p2_count_kernel<<<n_cta, 1024, cnt_bytes, s>>>(src, n, chunk, D, shift, ctx->d_hist, sm);
     p2_scan_kernel<<<1, 1024, 0, s>>>(ctx->d_hist, RT, sm, g_p2_tile);
-    const unsigned grid = (unsigned)ctx->sm_count * 3u;
-    p2_coarse_kernel<<<grid, P2_NT, p2_sorted_off() + P2_TILE * 16u, s>>>(src, n, D, shift, ctx->d_hist, sm, coarse, grouped);
+    e = p2_coarse_variant(ctx, src, n, s, false);
+    if (e != cudaSuccess) return e;
     e = p2_fine_variant(ctx, coarse, n, s, false);
     if (e != cudaSuccess) return e;
     p2_pad_kernel<<<(unsigned)ctx->sm_count * 4u, 256, 0, s>>>(grouped, n, sm);
