@@ -232,10 +232,17 @@ kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_
         first.p50_bin = (uint16_t)(c_lo >= t50 ? lo : hi);
         first.p99_bin = (uint16_t)(c_lo >= t99 ? lo : hi);
       }
-      out[0] = first;
-      argus_cluster z;
-      z.count = 0u; z.p50_bin = 0; z.p99_bin = 0;
-      for (uint32_t k = 1; k < P.max_clusters; ++k) out[k] = z;
+      const uint32_t w1 = (uint32_t)first.p50_bin | ((uint32_t)first.p99_bin << 16);
+      if ((P.max_clusters & 1u) == 0u) {           // slots of a cell are 16-byte aligned: whole-sector stores
+        uint4* o4 = reinterpret_cast<uint4*>(out);
+        o4[0] = make_uint4(first.count, w1, 0u, 0u);
+        for (uint32_t k = 1; k < P.max_clusters / 2u; ++k) o4[k] = make_uint4(0u, 0u, 0u, 0u);
+      } else {
+        out[0] = first;
+        argus_cluster z;
+        z.count = 0u; z.p50_bin = 0; z.p99_bin = 0;
+        for (uint32_t k = 1; k < P.max_clusters; ++k) out[k] = z;
+      }
       n_clusters[cell] = n != 0ull ? 1 : 0;
     }
   }
@@ -256,6 +263,11 @@ kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_
 __global__ void __launch_bounds__(256)
 clusters_to_l3_kernel(const argus_cluster* __restrict__ cl, argus_dims D, uint32_t mc, uint32_t per_octave,
                       uint32_t* __restrict__ count, double* __restrict__ p50, double* __restrict__ p99) {
+  // a bin stands for 2^((bin + 0.5) / per_octave) ns: 65,536 possible bins at most 256 of which a grid uses —
+  // tabulate the first 256 with the very expression used for the others
+  __shared__ double s_val[256];
+  for (uint32_t b = threadIdx.x; b < 256u; b += blockDim.x) s_val[b] = exp2(((double)b + 0.5) / (double)per_octave);
+  __syncthreads();
   const uint64_t n = (uint64_t)D.R * D.T * D.S * mc;
   for (uint64_t o = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (uint64_t)gridDim.x * blockDim.x) {
     // o walks the OUTPUT (coalesced writes): o = ((key * R) + r) * mc + c
@@ -265,8 +277,8 @@ clusters_to_l3_kernel(const argus_cluster* __restrict__ cl, argus_dims D, uint32
     const uint64_t key = kr / D.R;
     const argus_cluster q = cl[(((uint64_t)r * D.T * D.S) + key) * mc + c];
     count[o] = q.count;
-    p50[o] = q.count ? exp2(((double)q.p50_bin + 0.5) / (double)per_octave) : 1.0;
-    p99[o] = q.count ? exp2(((double)q.p99_bin + 0.5) / (double)per_octave) : 1.0;
+    p50[o] = q.count ? (q.p50_bin < 256u ? s_val[q.p50_bin] : exp2(((double)q.p50_bin + 0.5) / (double)per_octave)) : 1.0;
+    p99[o] = q.count ? (q.p99_bin < 256u ? s_val[q.p99_bin] : exp2(((double)q.p99_bin + 0.5) / (double)per_octave)) : 1.0;
   }
 }
 
