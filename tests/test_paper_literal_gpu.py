@@ -1,6 +1,6 @@
 """-m gpu parity tests of the paper-literal float rows (SURVEY §8(f) NEXT-1..3) through the C ABI against
 oracle/paper_literal.py on the same seeded inputs.
-Tolerances (DESIGN.md §7.3): integers (bins, cluster counts, boundaries as cluster extents, flags, classes,
+Tolerances (DESIGN.md §6.6): integers (bins, cluster counts, boundaries as cluster extents, flags, classes,
 interval ends, widths, change-point steps) exact; fp64 quantities rel 1e-9 (the kernels and numpy sum in
 different orders and call different exp / erfc / log implementations: a few ulp each over <= 4096 terms)."""
 import math

@@ -167,7 +167,7 @@ def test_unsorted_scaled():
     ev = wl.expand_host()
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False)
     assert_parity(ev, *_dims(wl.spec), sorted_hint=False, path=PATH_GLOBAL)
-    # S <= 1024 runs three 9-warp CTAs per SM with a short stage ring (the geometry that once exposed a
+    # S <= 1024 runs three CTAs per SM with a short stage ring (5 stages of 8 KB; the geometry that once exposed a
     # stage released before its loads had landed): repeat, the race was timing dependent
     wl2 = build_workload(scaled("unsorted", n_ranks=64, n_events=20000, n_sigs=1000))
     ev2 = wl2.expand_host()
