@@ -170,14 +170,166 @@ __device__ void kde_cell(const uint32_t* __restrict__ hist, const argus_kde_para
   }
 }
 
+// The same algorithm with EIGHT lanes per histogram (four histograms per warp), for cells whose occupied bins span
+// at most KDE_WIN grid steps (8 octaves on the fine grid: all but pathological cells).  A warp per cell leaves most
+// lanes idle — the occupied range is a dozen bins — and the kernel is bound by instruction issue, so four cells per
+// warp instruction is what counts.  Shared arrays are indexed relative to the first occupied bin.  Every formula
+// and every decision is kde_cell's; only the order of the partial sums of the mean and the variance differs (8
+// lanes instead of 32).  Returns false, having written nothing, when the cell is too wide.
+constexpr uint32_t KDE_WIN = 64;
+struct KdeGrp {
+  double f[KDE_WIN];
+  double e[KDE_WIN];
+  uint32_t c[KDE_WIN];
+};
+
+__device__ bool kde_cell_group(const uint32_t* __restrict__ hist, const argus_kde_params& P, KdeGrp& sm,
+                               argus_cluster* __restrict__ out, uint8_t* __restrict__ out_n) {
+  const int lane = threadIdx.x & 31, gl = lane & 7;
+  const uint32_t gmask = 0xFFu << (lane & 24);
+  const uint32_t nb = P.n_bins;
+  const double step = 0.6931471805599453 / (double)P.per_octave;
+  // occupied range and n (integers: exact in any order)
+  unsigned long long cnt = 0ull;
+  uint32_t lo = nb, hi = 0;
+  if ((nb & 3u) == 0u && (reinterpret_cast<size_t>(hist) & 15u) == 0u) {
+    const uint4* h4 = reinterpret_cast<const uint4*>(hist);
+    for (uint32_t q = gl; q < nb / 4u; q += 8) {
+      const uint4 v = __ldg(h4 + q);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (uint32_t k = 0; k < 4u; ++k)
+        if (w[k]) { const uint32_t b = 4u * q + k; cnt += w[k]; lo = b < lo ? b : lo; hi = b > hi ? b : hi; }
+    }
+  } else {
+    for (uint32_t b = gl; b < nb; b += 8) {
+      const uint32_t c = __ldg(hist + b);
+      if (c) { cnt += c; lo = b < lo ? b : lo; hi = b > hi ? b : hi; }
+    }
+  }
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1) {
+    cnt += __shfl_xor_sync(gmask, cnt, o);
+    const uint32_t l2 = __shfl_xor_sync(gmask, lo, o), h2 = __shfl_xor_sync(gmask, hi, o);
+    lo = l2 < lo ? l2 : lo; hi = h2 > hi ? h2 : hi;
+  }
+  if (cnt != 0ull && hi - lo >= KDE_WIN) return false;
+  for (uint32_t k = gl; k < P.max_clusters; k += 8) { out[k].count = 0u; out[k].p50_bin = 0; out[k].p99_bin = 0; }
+  if (cnt == 0ull) {
+    if (gl == 0) *out_n = 0;
+    return true;
+  }
+  const double n = (double)cnt;
+  double sx = 0.0;
+  for (uint32_t b = lo + gl; b <= hi; b += 8) {
+    const uint32_t c = __ldg(hist + b);
+    sm.c[b - lo] = c;
+    sm.f[b - lo] = 0.0;
+    if (c) sx += (double)c * (((double)b + 0.5) * step);
+  }
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1) sx += __shfl_xor_sync(gmask, sx, o);
+  __syncwarp(gmask);
+  double h = 0.0;
+  if (n >= 2.0 && hi > lo) {            // R26
+    const double mean = sx / n;
+    double ss = 0.0;
+    for (uint32_t b = lo + gl; b <= hi; b += 8) {
+      const double dx = ((double)b + 0.5) * step - mean;
+      ss += (double)sm.c[b - lo] * dx * dx;
+    }
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) ss += __shfl_xor_sync(gmask, ss, o);
+    const double sigma = sqrt(ss / (n - 1.0));                        // R25
+    h = 1.06 * sigma * pow(n, -0.2);                                  // Scott's rule
+    const double norm = 1.0 / (n * h * 2.5066282746310002);           // eq. (1), R22
+    for (uint32_t d = gl; d <= hi - lo; d += 8) {
+      const double u = ((double)d * step) / h;
+      sm.e[d] = exp(-0.5 * u * u);
+    }
+    __syncwarp(gmask);
+    for (uint32_t j = lo + gl; j <= hi; j += 8) {
+      double acc = 0.0;
+      for (uint32_t b = lo; b <= hi; ++b) {
+        const uint32_t c = sm.c[b - lo];
+        if (c) acc += (double)c * sm.e[j > b ? j - b : b - j];
+      }
+      sm.f[j - lo] = acc * norm;
+    }
+  }
+  __syncwarp(gmask);
+  if (gl == 0) {
+    double need = P.min_frac * n;
+    if ((double)P.min_count > need) need = (double)P.min_count;
+    uint32_t n_out = 0;
+    uint32_t seg_lo = lo;
+    double since = 0.0, right = n;
+    uint32_t last_bound = 0;
+    bool have_bound = false;
+    auto emit = [&](uint32_t a, uint32_t b) {          // cluster of the bins [a, b)
+      unsigned long long cn = 0;
+      for (uint32_t q = a; q < b; ++q) cn += sm.c[q - lo];
+      if (cn == 0ull || n_out >= P.max_clusters) return;
+      const unsigned long long t50 = (cn + 1ull) / 2ull;
+      const unsigned long long t99 = (unsigned long long)ceil(0.99 * (double)cn);
+      unsigned long long cum = 0;
+      uint32_t p50 = b - 1u, p99 = b - 1u;
+      bool got50 = false, got99 = false;
+      for (uint32_t q = a; q < b; ++q) {
+        cum += sm.c[q - lo];
+        if (!got50 && cum >= t50) { p50 = q; got50 = true; }
+        if (!got99 && cum >= t99) { p99 = q; got99 = true; }
+      }
+      out[n_out].count = (uint32_t)cn; out[n_out].p50_bin = (uint16_t)p50; out[n_out].p99_bin = (uint16_t)p99;
+      ++n_out;
+    };
+    if (h > 0.0) {
+      for (uint32_t j = lo + 1u; j < hi; ++j) {
+        since += (double)sm.c[j - 1u - lo];
+        right -= (double)sm.c[j - 1u - lo];
+        if (sm.f[j - lo] < sm.f[j - 1u - lo] && sm.f[j - lo] <= sm.f[j + 1u - lo]) {
+          const bool spaced = !have_bound || j - last_bound >= P.min_gap_bins;
+          if (since >= need && right >= need && spaced && n_out + 1u < P.max_clusters) {
+            emit(seg_lo, j);
+            seg_lo = j; since = 0.0; last_bound = j; have_bound = true;
+          }
+        }
+      }
+    }
+    emit(seg_lo, hi + 1u);
+    *out_n = (uint8_t)n_out;
+  }
+  __syncwarp(gmask);
+  return true;
+}
+
+// 32 cells per CTA: eight lanes each; the cells that are too wide for the group path — and every cell when the
+// caller wants the density on the whole grid — are queued and take the warp path in the second half.
 __global__ void __launch_bounds__(256)
 kde_hist_kernel(const uint32_t* __restrict__ hist, uint64_t n_cells, argus_kde_params P, argus_cluster* clusters,
                 uint8_t* n_clusters, double* density) {
-  __shared__ KdeSmem sm[8];
-  const uint64_t cell = (uint64_t)blockIdx.x * 8u + (threadIdx.x >> 5);
-  if (cell >= n_cells) return;
-  kde_cell(hist + cell * P.n_bins, P, sm[threadIdx.x >> 5], clusters + cell * P.max_clusters, n_clusters + cell,
-           density ? density + cell * P.n_bins : nullptr);
+  __shared__ union { KdeGrp g[32]; KdeSmem w[8]; } sm;
+  __shared__ uint32_t s_wide[32];
+  __shared__ uint32_t s_nwide;
+  const uint64_t cell0 = (uint64_t)blockIdx.x * 32u;
+  const uint32_t grp = threadIdx.x >> 3;
+  if (threadIdx.x == 0) s_nwide = 0u;
+  __syncthreads();
+  const uint64_t cell = cell0 + grp;
+  if (cell < n_cells) {
+    bool done = false;
+    if (density == nullptr)
+      done = kde_cell_group(hist + cell * P.n_bins, P, sm.g[grp], clusters + cell * P.max_clusters, n_clusters + cell);
+    if (!done && (threadIdx.x & 7) == 0) s_wide[atomicAdd(&s_nwide, 1u)] = grp;
+  }
+  __syncthreads();
+  const uint32_t n_wide = s_nwide;
+  for (uint32_t i = threadIdx.x >> 5; i < n_wide; i += 8) {
+    const uint64_t wc = cell0 + s_wide[i];
+    kde_cell(hist + wc * P.n_bins, P, sm.w[threadIdx.x >> 5], clusters + wc * P.max_clusters, n_clusters + wc,
+             density ? density + wc * P.n_bins : nullptr);
+    __syncwarp();
+  }
 }
 
 // The 32-bucket histograms of the finalised record table (per_octave = 1, n_bins = 32).  A valley needs a bin
@@ -779,7 +931,7 @@ cudaError_t argus_launch_fine_hist(argus_ctx* ctx, const argus_event* ev, uint64
 cudaError_t argus_launch_kde_hist(argus_ctx* ctx, const uint32_t* d_hist, uint64_t n_cells, const argus_kde_params* P,
                                   argus_cluster* d_clusters, uint8_t* d_n, double* d_density, cudaStream_t s) {
   if (n_cells == 0) return cudaSuccess;
-  kde_hist_kernel<<<(unsigned)((n_cells + 7) / 8), 256, 0, s>>>(d_hist, n_cells, *P, d_clusters, d_n, d_density);
+  kde_hist_kernel<<<(unsigned)((n_cells + 31) / 32), 256, 0, s>>>(d_hist, n_cells, *P, d_clusters, d_n, d_density);
   ctx->n_kernels += 1;
   return cudaGetLastError();
 }
