@@ -176,15 +176,19 @@ __device__ void kde_cell(const uint32_t* __restrict__ hist, const argus_kde_para
 // warp instruction is what counts.  Shared arrays are indexed relative to the first occupied bin.  Every formula
 // and every decision is kde_cell's; only the order of the partial sums of the mean and the variance differs (8
 // lanes instead of 32).  Returns false, having written nothing, when the cell is too wide.
-constexpr uint32_t KDE_WIN = 64;
-struct KdeGrp {
-  double f[KDE_WIN];
-  double e[KDE_WIN];
-  uint32_t c[KDE_WIN];
+template <uint32_t WIN>
+struct KdeGrpT {
+  static constexpr uint32_t win = WIN;
+  double f[WIN];
+  double e[WIN];
+  uint32_t c[WIN];
 };
+typedef KdeGrpT<64> KdeGrp;
 
-__device__ bool kde_cell_group(const uint32_t* __restrict__ hist, const argus_kde_params& P, KdeGrp& sm,
+template <class GS>
+__device__ bool kde_cell_group(const uint32_t* __restrict__ hist, const argus_kde_params& P, GS& sm,
                                argus_cluster* __restrict__ out, uint8_t* __restrict__ out_n) {
+  constexpr uint32_t KDE_WIN = GS::win;
   const int lane = threadIdx.x & 31, gl = lane & 7;
   const uint32_t gmask = 0xFFu << (lane & 24);
   const uint32_t nb = P.n_bins;
@@ -337,12 +341,12 @@ kde_hist_kernel(const uint32_t* __restrict__ hist, uint64_t n_cells, argus_kde_p
 // cell: the compact cells of the aggregation hold four buckets at most, and 10 % jitter fills one or two) is ONE
 // cluster whatever its density looks like, and its (count, p50, p99) are integer work — one thread does it,
 // no floating point but the ceil(0.99 count) the wide path takes too.  The other cells are queued in shared
-// memory and get the full KDE, one warp each (kde_cell), in the second half of the kernel.
+// memory and get the full KDE, eight lanes each (kde_cell_group), in the second half of the kernel.
 constexpr int KDE_REC_NT = 256;
 __global__ void __launch_bounds__(KDE_REC_NT)
 kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_params P, argus_cluster* clusters,
                    uint8_t* n_clusters) {
-  __shared__ KdeSmemT<32> sm[KDE_REC_NT / 32];
+  __shared__ KdeGrpT<32> sm[KDE_REC_NT / 8];
   __shared__ uint32_t s_wide[KDE_REC_NT];
   __shared__ uint32_t s_nwide;
   const uint64_t n_cells = (uint64_t)D.R * D.T * D.S;
@@ -400,13 +404,12 @@ kde_records_kernel(const uint8_t* __restrict__ records, argus_dims D, argus_kde_
   }
   __syncthreads();
   const uint32_t n_wide = s_nwide;
-  for (uint32_t i = threadIdx.x >> 5; i < n_wide; i += KDE_REC_NT / 32) {
+  for (uint32_t i = threadIdx.x >> 3; i < n_wide; i += KDE_REC_NT / 8) {      // eight lanes per wide cell
     const uint64_t wc = cell0 + s_wide[i];
     const uint64_t rec = wc / D.S;
     const uint32_t sig = (uint32_t)(wc - rec * D.S);
     const argus_cell* c = reinterpret_cast<const argus_cell*>(records + rec * D.rec_bytes + D.cell_off) + sig;
-    kde_cell(c->hist, P, sm[threadIdx.x >> 5], clusters + wc * P.max_clusters, n_clusters + wc, nullptr);
-    __syncwarp();
+    kde_cell_group(c->hist, P, sm[threadIdx.x >> 3], clusters + wc * P.max_clusters, n_clusters + wc);   // 32 bins: never too wide
   }
 }
 
