@@ -106,6 +106,16 @@ def test_kde_clusters_on_seeded_histograms():
         for i, h in enumerate(hists):
             f = PL.kde_clusters(h)[0]
             assert np.allclose(got_f[i], f, rtol=RTOL, atol=1e-13 * max(1e-300, f.max())), i   # far tails underflow differently
+        # without the density the kernel gives eight lanes to a histogram whose occupied bins span <= 64 grid steps and
+        # a warp to the wider ones (the strays of kind 2, the heavy tails): the same clusters either way
+        spans = [int(np.nonzero(h)[0][-1] - np.nonzero(h)[0][0]) if h.any() else 0 for h in hists]
+        assert min(spans) < 64 <= max(spans)
+        d_c2 = torch.full((len(hists) * mc * 8,), 0xAB, dtype=torch.uint8, device="cuda")
+        d_n2 = torch.full((len(hists),), 0xAB, dtype=torch.uint8, device="cuda")
+        ctx.kde_clusters(_cuda(H), len(hists), p, d_c2, d_n2, None)
+        assert torch.equal(d_n2, d_n) and torch.equal(d_c2, d_c)
+        _compare_clusters(d_c2.cpu().numpy().view(A.CLUSTER_DTYPE).reshape(len(hists), mc), d_n2.cpu().numpy(), hists, 8,
+                          max_clusters=mc)
     ctx.close()
 
 
