@@ -746,7 +746,7 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
 
 // ---- NEXT-3: L2 ---------------------------------------------------------------------------------------------
 // One CTA per routed event k (phase span, index P = whole iteration): x_r = mean over the T steps of span_ns.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(1024)
 l2_kernel(const uint8_t* __restrict__ records, argus_dims D, const uint8_t* __restrict__ route,
           const uint32_t* __restrict__ group_id, double z_thr, argus_l2_group* __restrict__ groups,
           double* __restrict__ z_out, uint8_t* __restrict__ flag_out, double* __restrict__ xbar_ws) {
@@ -981,7 +981,8 @@ cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l
 cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
                             double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
                             cudaStream_t s) {
-  l2_kernel<<<ctx->dims.P + 1u, 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, d_route, d_group_id, z_thr,
+  // few CTAs (one per routed event), each a chain of strided loads and fenced phases: as many threads as a CTA takes
+  l2_kernel<<<ctx->dims.P + 1u, ctx->dims.R >= 1024u ? 1024 : 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, d_route, d_group_id, z_thr,
                                              d_groups, d_z, d_flags, d_xbar);
   ctx->n_kernels += 1;
   return cudaGetLastError();
