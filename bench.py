@@ -3,13 +3,15 @@
 spans -> cross-rank median/MAD diagnosis (BASELINE.json `metric`), on seeded synthetic events.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload production] [--impl ours|reference]
-                  [--scaling weak|strong]
+                  [--scaling weak|strong] [--exchange a2a|p2p] [--bimodal F] [--no-e2e] [--no-cpu-baseline] [--no-next]
 
 One step = one pass of the whole path over the workload: argus_reset + argus_aggregate +
 argus_phase_times + argus_diagnose.  `value` is timed with CUDA events with the events resident in
 HBM; `e2e` is the same step through argus_aggregate_host with HOST (pinned) buffers: the 256 MiB
 chunked host->device copies and the device->host read of the diagnosis are inside the timed region,
-and its outputs are compared with the resident leg's.  Prints ONE JSON line on rank 0.
+and its outputs are compared with the resident leg's.  `next_rows` times every NEXT-row call (KDE
+clustering, record encodings, L3 / L2 / L1) alone on the finalised table, outside the step.  Prints ONE
+JSON line on rank 0.
 `--impl reference` times the CPU oracle (oracle/) instead.  `--gpus N` (N > 1) outside torchrun
 re-launches itself under torch.distributed.run with N ranks, or fails if the box has fewer GPUs.
 """
