@@ -444,14 +444,15 @@ __device__ __forceinline__ double normal_cdf(double z) { return 0.5 * erfc(-z * 
 extern __shared__ unsigned char l3_smem[];
 
 // bitonic sort of n (power of two) doubles with their payload, ascending; all threads of the CTA call
-__device__ void bitonic_sort_simple(double* v, uint16_t* id, uint32_t n) {
+template <typename KT>
+__device__ void bitonic_sort_simple(KT* v, uint16_t* id, uint32_t n) {
   for (uint32_t k = 2; k <= n; k <<= 1) {
     for (uint32_t j = k >> 1; j > 0; j >>= 1) {
       for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
         const uint32_t p = i ^ j;
         if (p > i) {
           const bool up = (i & k) == 0u;
-          const double a = v[i], b = v[p];
+          const KT a = v[i], b = v[p];
           if ((a > b) == up && a != b) {
             v[i] = b; v[p] = a;
             const uint16_t t = id[i]; id[i] = id[p]; id[p] = t;
@@ -467,7 +468,8 @@ __device__ void bitonic_sort_simple(double* v, uint16_t* id, uint32_t n) {
 // stages j and j/2 in registers, so two stages cost one trip through shared memory and one barrier (42 passes
 // instead of 78 stages at n = 4096; every thread busy instead of half of them).  Identical compare-exchanges,
 // hence identical output (ties included).  n >= 4, n / 4 <= blockDim.x.
-__device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
+template <typename KT>
+__device__ void bitonic_sort(KT* v, uint16_t* id, uint32_t n) {
   if (n < 4u || (n >> 2) > blockDim.x) { bitonic_sort_simple(v, id, n); return; }
   const uint32_t t = threadIdx.x, nt = n >> 2;
   for (uint32_t k = 2; k <= n; k <<= 1) {
@@ -478,13 +480,13 @@ __device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
         const uint32_t base = ((t >> b) << (b + 2u)) | (t & (jb - 1u));
         const bool up = (base & k) == 0u;
         const uint32_t e[4] = {base, base | jb, base | j, base | j | jb};
-        double x[4];
+        KT x[4];
         uint16_t q[4];
 #pragma unroll
         for (int a = 0; a < 4; ++a) { x[a] = v[e[a]]; q[a] = id[e[a]]; }
 #define ARGUS_CE(a, c)                                                         \
   if ((x[a] > x[c]) == up && x[a] != x[c]) {                                   \
-    const double tx = x[a]; x[a] = x[c]; x[c] = tx;                            \
+    const KT tx = x[a]; x[a] = x[c]; x[c] = tx;                            \
     const uint16_t tq = q[a]; q[a] = q[c]; q[c] = tq;                          \
   }
         ARGUS_CE(0, 2) ARGUS_CE(1, 3) ARGUS_CE(0, 1) ARGUS_CE(2, 3)
@@ -497,7 +499,7 @@ __device__ void bitonic_sort(double* v, uint16_t* id, uint32_t n) {
     if (j == 1u) {
       if (t < nt) {
         const uint32_t i = 4u * t;
-        double x[4];
+        KT x[4];
         uint16_t q[4];
 #pragma unroll
         for (int a = 0; a < 4; ++a) { x[a] = v[i + a]; q[a] = id[i + a]; }
@@ -578,6 +580,62 @@ __device__ __forceinline__ double l3_term(const L3Par& q, double lgx) {
   return q.w * normal_cdf(z);
 }
 
+// ---- ranks with identical mixtures ------------------------------------------------------------------------------
+// The triples are quantised summaries (a bin stands for one duration, R30), so most ranks of a key carry the SAME
+// mixture: same weights count_c / total, same p50, same p99 in every cluster slot, hence bit-identical CDF values
+// at every grid point.  Grouping them first turns sum_b |F_a - F_b| over R ranks into a sum over the D distinct
+// mixtures weighted by their multiplicities — exact algebra, no sort per grid point, O(D^2) instead of
+// O(R log^2 R).  Classes are found by sorting a 64-bit hash of the mixture parameters and comparing neighbours
+// field by field (a hash collision only splits work, it never merges two different mixtures).
+constexpr uint32_t L3_MAX_CLASSES = 256;
+__device__ __forceinline__ unsigned long long l3_mix(unsigned long long h, unsigned long long v) {
+  h ^= v; h *= 0x100000001b3ull; h ^= h >> 29;
+  return h;
+}
+__device__ __forceinline__ double l3_total(const uint32_t* cnt, uint32_t r, uint32_t C) {
+  double tot = 0.0;
+  for (uint32_t c = 0; c < C; ++c) tot += (double)cnt[r * C + c];
+  return tot;
+}
+__device__ unsigned long long l3_hash(const uint32_t* cnt, const double* p50, const double* p99, uint32_t r, uint32_t C) {
+  const double tot = l3_total(cnt, r, C);
+  unsigned long long h = 0xcbf29ce484222325ull;
+  for (uint32_t c = 0; c < C; ++c) {
+    const uint32_t k = cnt[r * C + c];
+    if (k) {
+      h = l3_mix(h, (unsigned long long)__double_as_longlong((double)k / tot));
+      h = l3_mix(h, (unsigned long long)__double_as_longlong(p50[r * C + c]));
+      h = l3_mix(h, (unsigned long long)__double_as_longlong(p99[r * C + c]));
+    } else {
+      h = l3_mix(h, 0x9e3779b97f4a7c15ull);
+    }
+  }
+  return h & 0x7FFFFFFFFFFFFFFFull;            // the padding key (all ones) sorts behind every rank
+}
+__device__ bool l3_same_mixture(const uint32_t* cnt, const double* p50, const double* p99, uint32_t a, uint32_t b, uint32_t C) {
+  const double ta = l3_total(cnt, a, C), tb = l3_total(cnt, b, C);
+  for (uint32_t c = 0; c < C; ++c) {
+    const uint32_t ka = cnt[a * C + c], kb = cnt[b * C + c];
+    if ((ka == 0u) != (kb == 0u)) return false;
+    if (ka == 0u) continue;
+    if (__double_as_longlong((double)ka / ta) != __double_as_longlong((double)kb / tb)) return false;
+    if (__double_as_longlong(p50[a * C + c]) != __double_as_longlong(p50[b * C + c])) return false;
+    if (__double_as_longlong(p99[a * C + c]) != __double_as_longlong(p99[b * C + c])) return false;
+  }
+  return true;
+}
+// F_r(x) of eq. (2) for one rank, parameters recomputed (the class path evaluates a handful of ranks only)
+__device__ double l3_cdf_of(const uint32_t* cnt, const double* p50, const double* p99, uint32_t r, uint32_t C, double lgx) {
+  const double tot = l3_total(cnt, r, C);
+  double F = 0.0;
+  if (tot > 0.0)
+    for (uint32_t c = 0; c < C; ++c) {
+      const uint32_t k = cnt[r * C + c];
+      if (k) F += l3_term(l3_par(k, tot, p50[r * C + c], p99[r * C + c]), lgx);
+    }
+  return F;
+}
+
 __global__ void __launch_bounds__(1024)
 l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, argus_l3_stat* __restrict__ stat_out,
           uint8_t* __restrict__ flags_out) {
@@ -587,7 +645,12 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
   double* val = reinterpret_cast<double*>(l3_smem);                 // [n2]
   double* score = val + n2;                                         // [R]
   uint16_t* id = reinterpret_cast<uint16_t*>(score + R);            // [n2]
+  uint16_t* class_of = id + n2;                                     // [n2]: class of every rank (class path)
   __shared__ double s_red[64];
+  __shared__ uint16_t s_rep[L3_MAX_CLASSES];                         // a rank of every class
+  __shared__ uint32_t s_mult[L3_MAX_CLASSES];                        // ranks in every class
+  __shared__ double s_fv[L3_MAX_CLASSES], s_sc[L3_MAX_CLASSES];
+  __shared__ uint32_t s_scan[33];
   __shared__ double s_lo, s_hi, s_fence;
   const uint32_t* cnt = in.count + (size_t)key * R * C;
   const double* p50 = in.p50 + (size_t)key * R * C;
@@ -608,7 +671,78 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
   }
   __syncthreads();
   const bool empty = !(s_hi > 0.0);
+  bool by_class = false;
   if (!empty) {
+    // ---- classes of identical mixtures ------------------------------------------------------------------
+    unsigned long long* hkey = reinterpret_cast<unsigned long long*>(val);
+    for (uint32_t r = threadIdx.x; r < n2; r += blockDim.x) {
+      hkey[r] = r < R ? l3_hash(cnt, p50, p99, r, C) : ~0ull;
+      id[r] = (uint16_t)r;
+    }
+    for (uint32_t d = threadIdx.x; d < L3_MAX_CLASSES; d += blockDim.x) { s_mult[d] = 0u; s_sc[d] = 0.0; }
+    __syncthreads();
+    bitonic_sort(hkey, id, n2);
+    // sorted position i opens a class unless its mixture equals its left neighbour's; PER consecutive positions
+    // per thread, block-wide inclusive scan of the flags
+    const uint32_t PER = (n2 + blockDim.x - 1u) / blockDim.x;
+    uint32_t fl[4] = {0u, 0u, 0u, 0u}, loc = 0u;
+    for (uint32_t k = 0; k < PER; ++k) {
+      const uint32_t i = threadIdx.x * PER + k;
+      if (i < R) {
+        fl[k] = (i == 0u || hkey[i] != hkey[i - 1u] || !l3_same_mixture(cnt, p50, p99, id[i], id[i - 1u], C)) ? 1u : 0u;
+        loc += fl[k];
+      }
+    }
+    uint32_t inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_up_sync(FULL, inc, o);
+      if ((threadIdx.x & 31) >= (uint32_t)o) inc += v;
+    }
+    if ((threadIdx.x & 31) == 31) s_scan[threadIdx.x >> 5] = inc;
+    __syncthreads();
+    uint32_t before = 0u, n_cls = 0u;
+    for (uint32_t w = 0; w < (blockDim.x >> 5); ++w) {
+      if (w < (threadIdx.x >> 5)) before += s_scan[w];
+      n_cls += s_scan[w];
+    }
+    by_class = n_cls <= L3_MAX_CLASSES;
+    if (by_class) {
+      uint32_t run = before + inc - loc;                   // classes opened before this thread's first position
+      for (uint32_t k = 0; k < PER; ++k) {
+        const uint32_t i = threadIdx.x * PER + k;
+        if (i < R) {
+          run += fl[k];
+          const uint32_t c = run - 1u;
+          class_of[id[i]] = (uint16_t)c;
+          if (fl[k]) s_rep[c] = id[i];
+          atomicAdd(&s_mult[c], 1u);
+        }
+      }
+      __syncthreads();
+      const double llo = log(0.5 * s_lo), lhi = log(2.0 * s_hi);
+      for (uint32_t j = 0; j < G; ++j) {
+        const double lx = llo + (lhi - llo) * (double)j / (double)(G - 1u);
+        const double x = exp(lx);
+        const double xm = j ? exp(llo + (lhi - llo) * (double)(j - 1u) / (double)(G - 1u)) : x;
+        const double xp = j + 1u < G ? exp(llo + (lhi - llo) * (double)(j + 1u) / (double)(G - 1u)) : x;
+        const double wj = 0.5 * (xp - xm);
+        const double lgx = log(x);
+        for (uint32_t d = threadIdx.x; d < n_cls; d += blockDim.x) s_fv[d] = l3_cdf_of(cnt, p50, p99, s_rep[d], C, lgx);
+        __syncthreads();
+        for (uint32_t d = threadIdx.x; d < n_cls; d += blockDim.x) {
+          const double fd = s_fv[d];
+          double s = 0.0;
+          for (uint32_t b = 0; b < n_cls; ++b) s += (double)s_mult[b] * fabs(fd - s_fv[b]);
+          s_sc[d] += wj * s;
+        }
+        __syncthreads();
+      }
+      for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) score[r] = s_sc[class_of[r]];
+    }
+    __syncthreads();
+  }
+  if (!empty && !by_class) {
     // per-thread totals and, when they fit, the cached parameters of this thread's NON-EMPTY (rank, cluster)
     // pairs in (rank slot, cluster) order — the order the sums below take; a thread with more than L3_CACHE of
     // them recomputes its parameters at every grid point
@@ -959,7 +1093,7 @@ cudaError_t argus_launch_clusters_to_l3(argus_ctx* ctx, const argus_cluster* d_c
 size_t argus_l3_smem_bytes(uint32_t R) {
   uint32_t n2 = 1;
   while (n2 < R) n2 <<= 1;
-  return sizeof(double) * ((size_t)n2 + R) + sizeof(uint16_t) * n2;
+  return sizeof(double) * ((size_t)n2 + R) + sizeof(uint16_t) * 2u * n2;
 }
 
 cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,

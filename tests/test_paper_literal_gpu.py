@@ -212,12 +212,16 @@ def test_l3_scores_and_fence(R, C, K, G):
     ctx.close()
 
 
-@pytest.mark.parametrize("R,C,G", [(4096, 2, 24), (1500, 3, 16), (1024, 1, 16)])
-def test_l3_large_rank_counts_sampled(R, C, G):
+@pytest.mark.parametrize("R,C,G,quantised", [(4096, 2, 24, False), (1500, 3, 16, False), (1024, 1, 16, False),
+                                             (4096, 1, 24, True), (3000, 2, 16, True)])
+def test_l3_large_rank_counts_sampled(R, C, G, quantised):
     """The launch shapes of the full-size job (1,024 threads, 2 or 4 sorted positions per thread, every cached /
     uncached parameter path): the oracle's R x R matrix is out of reach, so the scores of SAMPLED ranks are
     compared with the oracle's own mixture_cdf / w1 summed over all the other ranks, the quartiles and the fence
-    with numpy's percentile of the kernel's scores (R33's definition), the flags with score > fence."""
+    with numpy's percentile of the kernel's scores (R33's definition), the flags with score > fence.
+    quantised: p50 / p99 take a few bin values and the counts a few values, as the triples of NEXT-1 do — most ranks
+    then carry identical mixtures and the kernel scores the distinct ones with their multiplicities instead of
+    sorting R values per grid point; the random cases have R distinct mixtures and take the sort."""
     import torch
     from paper_2606_20374_b200 import argus as A
     rnd = np.random.default_rng(7 + R)
@@ -231,6 +235,11 @@ def test_l3_large_rank_counts_sampled(R, C, G):
         cnt[k] = np.where(have, rnd.integers(1, 4000, (R, C)), 0)
         p50[k] = base * (1 + 0.03 * rnd.random((R, C)))
         p99[k] = p50[k] * np.where(rnd.random((R, C)) < 0.15, 1.0, 1 + 0.5 * rnd.random((R, C)))
+        if quantised:
+            b50 = rnd.integers(0, 3, (R, C)) + (rnd.random((R, C)) < 0.01) * 5
+            p50[k] = base * 2.0 ** ((b50 + 0.5) / 8.0)
+            p99[k] = p50[k] * 2.0 ** (rnd.integers(0, 2, (R, C)) / 8.0)
+            cnt[k] = np.where(have, rnd.choice([100, 200], (R, C)), 0)
         p50[k, 17] *= 1.7; p99[k, 17] *= 1.7                           # one rank is slow on every cluster
         cnt[k, 17] = np.maximum(cnt[k, 17], 1)
         cnt[k, 33] = 0                                                 # one rank never ran the kernel
