@@ -175,7 +175,7 @@ def _ms(pairs):
     return [a.elapsed_time(b) for a, b in pairs]
 
 
-def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=592, fine_limit_bytes=6 << 30):
+def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=4096, fine_limit_bytes=6 << 30):
     """The SURVEY 8(f) NEXT rows on the table the timed steps left behind (finalised), each call timed alone
     with CUDA events (1 warm-up, median of `reps`); outside the step's timed region.  Bytes are the
     algorithmic ones of DESIGN.md 6.6 / 6.7 (what the call must read and write), GB/s = bytes / median time.
