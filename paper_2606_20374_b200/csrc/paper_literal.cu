@@ -588,6 +588,7 @@ __device__ __forceinline__ double l3_term(const L3Par& q, double lgx) {
 // O(R log^2 R).  Classes are found by sorting a 64-bit hash of the mixture parameters and comparing neighbours
 // field by field (a hash collision only splits work, it never merges two different mixtures).
 constexpr uint32_t L3_MAX_CLASSES = 256;
+constexpr uint32_t L3_CHUNK = 256;              // grid points per chunk of the class path
 __device__ __forceinline__ unsigned long long l3_mix(unsigned long long h, unsigned long long v) {
   h ^= v; h *= 0x100000001b3ull; h ^= h >> 29;
   return h;
@@ -649,7 +650,9 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
   __shared__ double s_red[64];
   __shared__ uint16_t s_rep[L3_MAX_CLASSES];                         // a rank of every class
   __shared__ uint32_t s_mult[L3_MAX_CLASSES];                        // ranks in every class
-  __shared__ double s_fv[L3_MAX_CLASSES], s_sc[L3_MAX_CLASSES];
+  __shared__ double s_sc[L3_MAX_CLASSES];
+  __shared__ double s_wj[L3_CHUNK], s_lg[L3_CHUNK];                  // trapezoid weight and log x of a chunk of grid points
+  __shared__ double s_part[1024];
   __shared__ uint32_t s_scan[33];
   __shared__ double s_lo, s_hi, s_fence;
   const uint32_t* cnt = in.count + (size_t)key * R * C;
@@ -720,21 +723,47 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
         }
       }
       __syncthreads();
+      // Grid points in chunks of JB: (1) the chunk's abscissae and trapezoid weights, one thread each; (2) eq. 2 for
+      // every (class, grid point) pair of the chunk, all threads; (3) thread (class d, group g) sums
+      // w_j sum_b m_b |F_d - F_b| over the grid points j = g, g + groups, ...; (4) thread d adds its groups'
+      // partial sums in a fixed order.  No atomics: the result does not depend on scheduling.
       const double llo = log(0.5 * s_lo), lhi = log(2.0 * s_hi);
-      for (uint32_t j = 0; j < G; ++j) {
-        const double lx = llo + (lhi - llo) * (double)j / (double)(G - 1u);
-        const double x = exp(lx);
-        const double xm = j ? exp(llo + (lhi - llo) * (double)(j - 1u) / (double)(G - 1u)) : x;
-        const double xp = j + 1u < G ? exp(llo + (lhi - llo) * (double)(j + 1u) / (double)(G - 1u)) : x;
-        const double wj = 0.5 * (xp - xm);
-        const double lgx = log(x);
-        for (uint32_t d = threadIdx.x; d < n_cls; d += blockDim.x) s_fv[d] = l3_cdf_of(cnt, p50, p99, s_rep[d], C, lgx);
+      uint32_t JB = n2 / n_cls;
+      JB = JB > L3_CHUNK ? L3_CHUNK : JB;
+      const uint32_t groups = blockDim.x / n_cls;                  // >= 1: n_cls <= min(R, 256) <= blockDim.x
+      const uint32_t my_d = threadIdx.x % n_cls, my_g = threadIdx.x / n_cls;
+      for (uint32_t j0 = 0; j0 < G; j0 += JB) {
+        const uint32_t nj = G - j0 < JB ? G - j0 : JB;
+        for (uint32_t jj = threadIdx.x; jj < nj; jj += blockDim.x) {
+          const uint32_t j = j0 + jj;
+          const double lx = llo + (lhi - llo) * (double)j / (double)(G - 1u);
+          const double x = exp(lx);
+          const double xm = j ? exp(llo + (lhi - llo) * (double)(j - 1u) / (double)(G - 1u)) : x;
+          const double xp = j + 1u < G ? exp(llo + (lhi - llo) * (double)(j + 1u) / (double)(G - 1u)) : x;
+          s_wj[jj] = 0.5 * (xp - xm);
+          s_lg[jj] = log(x);                               // log(x) of the oracle is log(exp(lx)): take it the same way
+        }
         __syncthreads();
-        for (uint32_t d = threadIdx.x; d < n_cls; d += blockDim.x) {
-          const double fd = s_fv[d];
-          double s = 0.0;
-          for (uint32_t b = 0; b < n_cls; ++b) s += (double)s_mult[b] * fabs(fd - s_fv[b]);
-          s_sc[d] += wj * s;
+        for (uint32_t p = threadIdx.x; p < n_cls * nj; p += blockDim.x) {
+          const uint32_t d = p % n_cls, jj = p / n_cls;
+          val[p] = l3_cdf_of(cnt, p50, p99, s_rep[d], C, s_lg[jj]);      // val[jj * n_cls + d]
+        }
+        __syncthreads();
+        double acc = 0.0;
+        if (my_g < groups)
+          for (uint32_t jj = my_g; jj < nj; jj += groups) {
+            const double* row = val + (size_t)jj * n_cls;
+            const double fd = row[my_d];
+            double s = 0.0;
+            for (uint32_t b2 = 0; b2 < n_cls; ++b2) s += (double)s_mult[b2] * fabs(fd - row[b2]);
+            acc += s_wj[jj] * s;
+          }
+        s_part[threadIdx.x] = acc;
+        __syncthreads();
+        if (threadIdx.x < n_cls) {
+          double s = s_sc[threadIdx.x];
+          for (uint32_t g2 = 0; g2 < groups; ++g2) s += s_part[g2 * n_cls + threadIdx.x];
+          s_sc[threadIdx.x] = s;
         }
         __syncthreads();
       }
