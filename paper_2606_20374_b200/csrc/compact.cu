@@ -25,6 +25,24 @@ struct Src {
 
 __device__ __forceinline__ uint32_t bucket_u64(unsigned long long d) { return argus_bucket64(d); }
 
+// 16 bytes of a cell head.  The sizing loop reads one 32-byte sector of every 160-byte cell: ask L2 for 64-byte
+// fills instead of whole 128-byte lines (every line of the table holds part of some head).
+__device__ __forceinline__ unsigned long long ld64_sparse(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.global.nc.L2::64B.u64 %0, [%1];" : "=l"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint32_t ld32_sparse(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.global.nc.L2::64B.u32 %0, [%1];" : "=r"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint4 ld_head(const uint4* p) {
+  uint4 v;
+  asm volatile("ld.global.nc.L2::64B.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+
 // bytes of the entry of cell (key, sig); 0 = the cell is left out.  SPARSE: also returns b0 / nb.
 template <bool TRIPLE>
 __device__ __forceinline__ uint32_t entry_bytes(const Src& src, const argus_dims& D, uint32_t key, uint32_t sig,
@@ -35,9 +53,9 @@ __device__ __forceinline__ uint32_t entry_bytes(const Src& src, const argus_dims
     return n ? 8u + 8u * n : 0u;
   }
   const uint4* c = reinterpret_cast<const uint4*>(src.records + (size_t)key * D.rec_bytes + D.cell_off + (size_t)sig * 160u);
-  const uint4 h0 = __ldg(c);                   // {count, sum}
+  const uint4 h0 = ld_head(c);                 // {count, sum}
   if ((h0.x | h0.y) == 0u) { b0 = nb = 0u; return 0u; }
-  const uint4 h1 = __ldg(c + 1);               // {min, max}
+  const uint4 h1 = ld_head(c + 1);             // {min, max}
   b0 = bucket_u64(((unsigned long long)h1.y << 32) | h1.x);
   nb = bucket_u64(((unsigned long long)h1.w << 32) | h1.z) - b0 + 1u;
   return 40u + 4u * (nb + (nb & 1u));
@@ -286,10 +304,10 @@ compact_fused_kernel(Src src, argus_dims D, unsigned long long* offsets, uint32_
       } else {
         const unsigned long long* c = reinterpret_cast<const unsigned long long*>(rec + D.cell_off + (size_t)sig * 160u);
         st64(e, (unsigned long long)sig | ((unsigned long long)b0 << 32) | ((unsigned long long)nb << 40));
-        st64(e + 8, c[0]); st64(e + 16, c[1]); st64(e + 24, c[2]); st64(e + 32, c[3]);
+        st64(e + 8, ld64_sparse(c)); st64(e + 16, ld64_sparse(c + 1)); st64(e + 24, ld64_sparse(c + 2)); st64(e + 32, ld64_sparse(c + 3));
         const uint32_t* h = reinterpret_cast<const uint32_t*>(c + 4) + b0;
         for (uint32_t j = 0; j < nb; j += 2u) {
-          const unsigned long long lo = h[j], hi = j + 1u < nb ? h[j + 1u] : 0u;
+          const unsigned long long lo = ld32_sparse(h + j), hi = j + 1u < nb ? ld32_sparse(h + j + 1u) : 0u;
           st64(e + 40u + 4u * j, lo | (hi << 32));
         }
       }
