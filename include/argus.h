@@ -259,6 +259,31 @@ int argus_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t sig_lo, ui
  * step_anomalous [T]; T and P are the ctx's, R = planes->n_ranks.  [host] planes, [host] outs. */
 int argus_diagnose_planes(argus_ctx* ctx, const argus_planes* planes, const argus_diag_out* outs, void* stream);
 
+/* The same rule for callers that must not allocate device memory: no ctx, no workspace, no cudaMalloc /
+ * cudaFree / allocating library call anywhere on this path.  Who that is: a monitor living inside the training
+ * process it observes (the paper's collector is injected into the job and reuses pre-allocated buffers) — the framework's
+ * caching allocator has usually claimed the HBM already, so a cudaMalloc from the side can fail outright, and
+ * when it succeeds it takes a device-wide lock and may stall the very iteration being measured; the same goes
+ * for code that runs from a callback or another context in which the CUDA runtime forbids allocation.  Such a
+ * caller hands in buffers it carved out at start-up (planes and outputs, exactly as for
+ * argus_diagnose_planes) and this entry point supplies the one piece of scratch the selection needs — a mark
+ * byte per series, set by the 32-bit pass for the series the 64-bit pass must redo — from a fixed array that
+ * is part of the library image: ARGUS_STATIC_MAX_SERIES bytes (256 KiB) of global memory on every device that
+ * loads libargus.so, held until the process exits.
+ *   n_steps = T >= 1, n_phases = P in 1..ARGUS_MAX_PHASES (what the ctx would have carried);
+ *   T * (planes->n_sigs + P + 1) series must fit the array, else ARGUS_ESIZE and nothing is launched.
+ * Works on the CURRENT device of the calling thread, which must be the one that holds the buffers.  The first
+ * call on each device looks up the array's device address and the SM count (host-side, once, under a lock):
+ * make that first call outside any stream capture.  Every call on a device shares the one array and leaves
+ * its marks behind; each call clears the bytes it is about to use on `stream` first, so calls ordered on one
+ * stream (or by events) are independent, but two calls that can overlap on the same device race on the marks
+ * and may return wrong medians for series whose values span 2^32 ns or more — serialise them.  Outputs and
+ * errors as argus_diagnose_planes (ARGUS_EINVAL for more than ARGUS_STATIC_MAX_DEVICES device ordinals). */
+#define ARGUS_STATIC_MAX_SERIES  262144u
+#define ARGUS_STATIC_MAX_DEVICES 64
+int argus_diagnose_planes_static(const argus_planes* planes, uint32_t n_steps, uint32_t n_phases,
+                                 const argus_diag_out* outs, void* stream);
+
 /* ---- compact record encodings (second half: "sparse/bit-packed record encoding (non-empty
  * bins only) to raise the compression ratio"; the paper's per-rank record of "approximately 200 triples ... about
  * 2.7 KB").  Both turn this ctx's FINALISED table (argus_phase_times ran; ARGUS_ESTATE otherwise)

@@ -42,7 +42,7 @@ L1_OUT_DTYPE = np.dtype([("cls", "<u4"), ("n_intervals", "<u4"), ("cp_found", "<
 EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes",
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
            "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
-           "argus_diagnose_planes", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
+           "argus_diagnose_planes", "argus_diagnose_planes_static", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
            "argus_sparse_bound", "argus_sparse_encode", "argus_triple_bound", "argus_triple_encode",
            "argus_clusters_to_l3", "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
@@ -134,6 +134,9 @@ def load() -> ctypes.CDLL:
                                       ctypes.c_uint32, vp]
     lib.argus_diagnose_planes.restype = i32
     lib.argus_diagnose_planes.argtypes = [vp, ctypes.POINTER(ArgusPlanes), ctypes.POINTER(ArgusDiagOut), vp]
+    lib.argus_diagnose_planes_static.restype = i32
+    lib.argus_diagnose_planes_static.argtypes = [ctypes.POINTER(ArgusPlanes), ctypes.c_uint32, ctypes.c_uint32,
+                                                 ctypes.POINTER(ArgusDiagOut), vp]
     lib.argus_fine_hist.restype = i32
     lib.argus_fine_hist.argtypes = [vp, vp, u64, vp, vp]
     lib.argus_kde_clusters.restype = i32
@@ -194,6 +197,26 @@ def _stream(s) -> Optional[int]:
     if isinstance(s, int):
         return s or None
     return s.cuda_stream or None
+
+
+STATIC_MAX_SERIES = 262144
+
+
+def diagnose_planes_static(d_sig_plane, d_span_plane, n_ranks: int, rank_stride: int, n_sigs: int, n_steps: int,
+                           n_phases: int, outs: dict, stream=None) -> None:
+    """argus_diagnose_planes_static: the cross-rank rule on planes with no context and no device allocation,
+    for a monitor that shares a process with a training job whose allocator already owns the HBM (a cudaMalloc
+    from the side may fail, and stalls the device when it does not).  The only scratch, a mark byte per series,
+    is a fixed 256 KiB array inside libargus.so, so n_steps * (n_sigs + n_phases + 1) <= STATIC_MAX_SERIES
+    (ArgusError ESIZE beyond).  Runs on the current device; the array is shared by all calls on that device, so
+    calls that could overlap on the GPU must be ordered by the caller."""
+    lib = load()
+    pl = ArgusPlanes(_ptr(d_sig_plane), _ptr(d_span_plane), n_ranks, rank_stride, n_sigs, 0)
+    o = ArgusDiagOut(*[_ptr(outs.get(k)) for k in ("sig_stats", "sig_flags", "span_stats",
+                                                   "span_flags", "rank_score", "step_anomalous")])
+    rc = lib.argus_diagnose_planes_static(ctypes.byref(pl), n_steps, n_phases, ctypes.byref(o), _stream(stream))
+    if rc != OK:
+        raise ArgusError(rc, lib.argus_strerror(rc).decode())
 
 
 class Argus:

@@ -10,6 +10,8 @@
 // sampling, no floating point.
 #include "argus_internal.cuh"
 
+#include <mutex>
+
 namespace {
 
 constexpr int EPT = 16;
@@ -584,4 +586,79 @@ cudaError_t argus_launch_pack_planes(argus_ctx* ctx, const void* d_records, uint
     ctx->n_kernels += 1;
   }
   return cudaGetLastError();
+}
+
+// ---- argus_diagnose_planes_static: the rule on planes for callers that may not allocate -------------------
+// See include/argus.h for who needs this and why.  Everything the selection kernels touch beyond the caller's
+// planes and outputs is the mark byte per series; here those bytes live in an array that is part of the
+// library image, so the path has no ctx, no workspace and no allocation of any kind.
+//
+// g_static_marks is a DEVICE symbol.  In host code its name stands for a host-side shadow of the symbol, not for
+// an address a kernel can use (a kernel handed &g_static_marks[0] from host code would fault, or scribble over
+// host memory on a system where the GPU can reach it).  The address the kernels get comes from
+// cudaGetSymbolAddress, asked once per device with that device current, and is cached below.
+static __device__ __align__(256) uint8_t g_static_marks[ARGUS_STATIC_MAX_SERIES];
+
+namespace {
+struct StaticDevice {
+  uint8_t* marks;     // device address of g_static_marks on this device (null: not looked up yet)
+  int sm_count;
+};
+StaticDevice g_static_dev[ARGUS_STATIC_MAX_DEVICES];
+std::mutex g_static_mu;
+
+// First call on `dev` (which is current): symbol address + SM count.  Host-side queries only.
+cudaError_t static_device(int dev, StaticDevice* out) {
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  StaticDevice& d = g_static_dev[dev];
+  if (d.marks == nullptr) {
+    uint8_t* p = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_marks);
+    if (e != cudaSuccess) return e;
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return e;
+    if (p == nullptr || sms <= 0) return cudaErrorInvalidSymbol;
+    d.sm_count = sms;
+    d.marks = p;
+  }
+  *out = d;
+  return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int argus_diagnose_planes_static(const argus_planes* pl, uint32_t n_steps, uint32_t n_phases,
+                                            const argus_diag_out* outs, void* stream) {
+  if (!pl || !outs) return ARGUS_EINVAL;
+  if (n_steps == 0 || n_phases == 0 || n_phases > ARGUS_MAX_PHASES) return ARGUS_EINVAL;
+  if (pl->n_ranks == 0 || pl->n_ranks > ARGUS_MAX_RANKS || pl->rank_stride < pl->n_ranks) return ARGUS_EINVAL;
+  if ((pl->n_sigs != 0) != (pl->sig_sums != nullptr)) return ARGUS_EINVAL;
+  if (((uintptr_t)pl->sig_sums & 7u) || ((uintptr_t)pl->span_ns & 7u)) return ARGUS_EINVAL;
+  if (((uintptr_t)outs->sig_stats & 15u) || ((uintptr_t)outs->span_stats & 15u)) return ARGUS_EINVAL;
+  if (((uintptr_t)outs->rank_score & 3u) || ((uintptr_t)outs->step_anomalous & 3u)) return ARGUS_EINVAL;
+  // the fixed array bounds the job: one mark byte per (step, sig or span) series
+  const uint64_t n_series = (uint64_t)n_steps * ((uint64_t)pl->n_sigs + n_phases + 1u);
+  if (n_series > ARGUS_STATIC_MAX_SERIES) return ARGUS_ESIZE;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return ARGUS_ECUDA;
+  if (dev < 0 || dev >= ARGUS_STATIC_MAX_DEVICES) return ARGUS_EINVAL;
+  StaticDevice sd;
+  if (static_device(dev, &sd) != cudaSuccess) return ARGUS_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  // The array keeps whatever the previous call (of any geometry) left in it: start from clean marks.
+  if (cudaMemsetAsync(sd.marks, 0, (size_t)n_series, s) != cudaSuccess) return ARGUS_ECUDA;
+  // launch_select reads three things of a ctx — where the marks are, the SM count, the launch counters —
+  // so a stand-in on the stack carries them; nothing else of it is looked at in planes mode.
+  argus_ctx tmp{};
+  tmp.d_diag_todo = sd.marks;
+  tmp.sm_count = sd.sm_count;
+  DiagSrc src;
+  src.records = nullptr;
+  src.sig_plane = reinterpret_cast<const unsigned long long*>(pl->sig_sums);
+  src.span_plane = reinterpret_cast<const unsigned long long*>(pl->span_ns);
+  src.rank_stride = pl->rank_stride; src.use_sums = false;
+  argus_dims D{};
+  D.R = pl->n_ranks; D.T = n_steps; D.S = pl->n_sigs; D.P = n_phases; D.sums = nullptr;
+  if (launch_select(&tmp, src, D, outs, s) != cudaSuccess) return ARGUS_ECUDA;
+  return ARGUS_OK;
 }
