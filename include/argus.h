@@ -224,6 +224,19 @@ int argus_phase_times(argus_ctx* ctx, void* d_records, argus_span* d_spans_out, 
  * plus the roll-ups of R15.  [host] outs holds [device] pointers. */
 int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus_diag_out* outs, void* stream);
 
+/* Ownership of a table, made explicit.  "This ctx's table" is the buffer last given to argus_reset, and the
+ * library tells it from a foreign one by that address alone: for its own table argus_diagnose takes the sig
+ * series from the sum plane of the workspace (kept in step by the aggregation kernels), for any other address
+ * it gathers them from the record bytes.  So the bytes of a ctx's table must change only through that ctx.  If
+ * the buffer is re-used for other contents (a stored table copied into it, another ctx aggregating into it),
+ * call argus_forget first: the ctx then owns no table, argus_diagnose reads every table from its records, and
+ * the entry points that need the ctx's own accumulation (argus_aggregate, argus_phase_times, argus_pack_planes)
+ * return ARGUS_ESTATE until the next argus_reset.  The encoders, argus_kde_clusters_records and argus_l2_groups
+ * read record bytes only: they take any finalised table of the ctx's geometry, forgotten or not.
+ * Skipping it is a usage error the library cannot detect: medians and flags of the sig series would come from
+ * the stale sum plane while the spans come from the new bytes.  Host-side only; queues nothing. */
+int argus_forget(argus_ctx* ctx);
+
 /* ---- one job sharded by trace rank over several GPUs (the paper's comparison of "the same
  * kernel across different ranks", when the ranks' events live on different devices) --------
  * Every GPU g aggregates its own ranks [r0_g, r0_g + R_g) with a ctx of n_ranks = R_g (events carry
@@ -303,7 +316,11 @@ int argus_diagnose_planes_static(const argus_planes* planes, uint32_t n_steps, u
  *     per cell with n_clusters > 0, ascending sig:  u32 sig | u32 n_clusters | n_clusters x argus_cluster
  * [device] d_out (8-byte aligned, out_capacity bytes), [device] d_offsets [R*T + 1] u64.  A record that would end
  * beyond out_capacity is not written (d_offsets is still complete: compare d_offsets[R*T] with out_capacity);
- * argus_sparse_bound / argus_triple_bound give a capacity that always suffices.  Asynchronous on `stream`. */
+ * argus_sparse_bound / argus_triple_bound give a capacity that always suffices.  Asynchronous on `stream`.
+ * The encoders of ONE ctx share a ticket word in its workspace, cleared by every call: two encodes of the same
+ * ctx (sparse and triple, or two of a kind) must not overlap on the GPU — queue them on one stream or order them
+ * with events, else records are handed out twice and the look-back never completes.  Different ctxs are
+ * independent.  TRIPLE: a d_n_clusters entry larger than max_clusters is read as max_clusters. */
 size_t argus_sparse_bound(const argus_config* cfg);
 int argus_sparse_encode(argus_ctx* ctx, const void* d_records, uint8_t* d_out, uint64_t out_capacity,
                         uint64_t* d_offsets, void* stream);
@@ -379,9 +396,12 @@ int argus_l3_detect(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params
  * (0 balanced < 0.02 <= 1 mild < 0.05 <= 2 severe); per rank z = (x - mu)/sigma, flag = z > z_threshold. */
 typedef struct argus_l2_group { uint32_t n, cls; double mu, sigma, cv; } argus_l2_group;   /* 32 B */
 /* [device] d_groups [P+1][R] (indexed by group id; n = 0: no such group), d_z [P+1][R] f64, d_flags [P+1][R]
- * u8, d_xbar [P+1][R] f64 (the x_r; also scratch). */
-int argus_l2_groups(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
-                    double z_threshold, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
+ * u8, d_xbar [P+1][R] f64 (the x_r; also scratch).  n_dims in 1..256 is the first extent of d_group_id; an
+ * event whose route byte is >= n_dims joins no group (z = 0, no flag, no group entries) rather than reading past
+ * the array.  Group sums are taken in a fixed order (no floating-point atomics): results are the same bits in
+ * every run, so a CV class or a z flag cannot flip between runs. */
+int argus_l2_groups(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, uint32_t n_dims,
+                    const uint32_t* d_group_id, double z_threshold, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
                     void* stream);
 
 /* ---- NEXT-3: L1 iteration-level detection ----------------------------------------------

@@ -41,7 +41,7 @@ L1_OUT_DTYPE = np.dtype([("cls", "<u4"), ("n_intervals", "<u4"), ("cp_found", "<
 
 EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_bytes",
            "argus_workspace_bytes", "argus_reset", "argus_ingest", "argus_aggregate",
-           "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_pack_planes",
+           "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_forget", "argus_pack_planes",
            "argus_diagnose_planes", "argus_diagnose_planes_static", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
            "argus_sparse_bound", "argus_sparse_encode", "argus_triple_bound", "argus_triple_encode",
            "argus_clusters_to_l3", "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
@@ -129,6 +129,8 @@ def load() -> ctypes.CDLL:
     lib.argus_phase_times.argtypes = [vp, vp, vp, vp]
     lib.argus_diagnose.restype = i32
     lib.argus_diagnose.argtypes = [vp, vp, ctypes.POINTER(ArgusDiagOut), vp]
+    lib.argus_forget.restype = i32
+    lib.argus_forget.argtypes = [vp]
     lib.argus_pack_planes.restype = i32
     lib.argus_pack_planes.argtypes = [vp, vp, ctypes.c_uint32, ctypes.c_uint32, vp, vp, ctypes.c_uint32,
                                       ctypes.c_uint32, vp]
@@ -156,7 +158,7 @@ def load() -> ctypes.CDLL:
     lib.argus_l3_detect.restype = i32
     lib.argus_l3_detect.argtypes = [vp, ctypes.POINTER(ArgusL3In), ctypes.POINTER(ArgusL3Params), vp, vp, vp, vp]
     lib.argus_l2_groups.restype = i32
-    lib.argus_l2_groups.argtypes = [vp, vp, vp, vp, ctypes.c_double, vp, vp, vp, vp, vp]
+    lib.argus_l2_groups.argtypes = [vp, vp, vp, ctypes.c_uint32, vp, ctypes.c_double, vp, vp, vp, vp, vp]
     lib.argus_l1_detect.restype = i32
     lib.argus_l1_detect.argtypes = [vp, vp, u64, u64, ctypes.c_uint32, ctypes.c_uint32,
                                     ctypes.POINTER(ArgusL1Params), vp, vp]
@@ -326,6 +328,9 @@ class Argus:
         self._check(self.lib.argus_diagnose(self._h, _ptr(d_records), ctypes.byref(o),
                                             _stream(stream)))
 
+    def forget(self) -> None:
+        self._check(self.lib.argus_forget(self._h))
+
     def pack_planes(self, d_records, sig_lo: int, sig_hi: int, d_sig_plane, d_span_plane,
                     rank_stride: int, rank_offset: int, stream=None) -> None:
         self._check(self.lib.argus_pack_planes(self._h, _ptr(d_records), sig_lo, sig_hi, _ptr(d_sig_plane),
@@ -384,8 +389,11 @@ class Argus:
                                              _ptr(d_flags), _stream(stream)))
 
     def l2_groups(self, d_records, d_route, d_group_id, z_threshold: float, d_groups, d_z, d_flags, d_xbar,
-                  stream=None) -> None:
-        self._check(self.lib.argus_l2_groups(self._h, _ptr(d_records), _ptr(d_route), _ptr(d_group_id), z_threshold,
+                  stream=None, n_dims: Optional[int] = None) -> None:
+        """d_group_id: [n_dims][R] u32; n_dims defaults to its size / R (a torch tensor or numpy array)."""
+        if n_dims is None:
+            n_dims = (d_group_id.numel() if hasattr(d_group_id, "numel") else d_group_id.size) // self.R
+        self._check(self.lib.argus_l2_groups(self._h, _ptr(d_records), _ptr(d_route), n_dims, _ptr(d_group_id), z_threshold,
                                              _ptr(d_groups), _ptr(d_z), _ptr(d_flags), _ptr(d_xbar), _stream(stream)))
 
     def l1_detect(self, d_base, series_stride: int, step_stride: int, n_series: int, n_steps: int, d_out,

@@ -350,6 +350,13 @@ extern "C" int argus_diagnose(argus_ctx* ctx, const void* d_records, const argus
   return ARGUS_OK;
 }
 
+extern "C" int argus_forget(argus_ctx* ctx) {
+  if (!ctx) return ARGUS_EINVAL;
+  ctx->d_records = nullptr;      // no address compares equal to it any more: every table is foreign
+  ctx->finalized = false;
+  return ARGUS_OK;
+}
+
 static bool aligned8(const void* p) { return ((uintptr_t)p & 7u) == 0; }
 
 extern "C" int argus_pack_planes(argus_ctx* ctx, const void* d_records, uint32_t sig_lo, uint32_t sig_hi,
@@ -480,14 +487,15 @@ extern "C" int argus_l3_detect(argus_ctx* ctx, const argus_l3_in* in, const argu
   return ARGUS_OK;
 }
 
-extern "C" int argus_l2_groups(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
-                               double z_threshold, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags,
+extern "C" int argus_l2_groups(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, uint32_t n_dims,
+                               const uint32_t* d_group_id, double z_threshold, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags,
                                double* d_xbar, void* stream) {
   if (!ctx || !d_records || !d_route || !d_group_id || !d_groups || !d_z || !d_flags || !d_xbar) return ARGUS_EINVAL;
+  if (n_dims == 0 || n_dims > 256u) return ARGUS_EINVAL;          // a route entry is one byte
   if (!aligned8(d_groups) || !aligned8(d_z) || !aligned8(d_xbar) || ((uintptr_t)d_group_id & 3u)) return ARGUS_EINVAL;
   if (d_records == ctx->d_records && !ctx->finalized) return ARGUS_ESTATE;
   ARGUS_ENTER(ctx, stream);
-  CU(ctx, argus_launch_l2(ctx, d_records, d_route, d_group_id, z_threshold, d_groups, d_z, d_flags, d_xbar, s));
+  CU(ctx, argus_launch_l2(ctx, d_records, d_route, n_dims, d_group_id, z_threshold, d_groups, d_z, d_flags, d_xbar, s));
   return ARGUS_OK;
 }
 

@@ -106,8 +106,8 @@ cudaError_t argus_launch_triple_encode(argus_ctx* ctx, const void* d_records, co
 size_t argus_l3_smem_bytes(uint32_t R);
 cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,
                             argus_l3_stat* d_stat, uint8_t* d_flags, cudaStream_t s);
-cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
-                            double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
+cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, uint32_t n_dims,
+                            const uint32_t* d_group_id, double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
                             cudaStream_t s);
 cudaError_t argus_launch_l1(argus_ctx* ctx, const void* d_base, uint64_t sstride, uint64_t tstride, uint32_t n_series,
                             uint32_t T, const argus_l1_params* P, argus_l1_out* d_out, cudaStream_t s);
@@ -118,9 +118,23 @@ bool argus_partition2_plan(const argus_config* cfg, uint32_t* shift, size_t* sma
 // opt-in shared-memory sizes of the kernels this ctx will launch (argus_create, once)
 cudaError_t argus_configure_seg(argus_ctx* ctx);
 cudaError_t argus_configure_partition(argus_ctx* ctx);
+cudaError_t argus_configure_compact(argus_ctx* ctx);
+cudaError_t argus_configure_paper_literal(argus_ctx* ctx);
 inline cudaError_t argus_configure_kernels(argus_ctx* ctx) {
   cudaError_t e = argus_configure_seg(ctx);
-  return e == cudaSuccess ? argus_configure_partition(ctx) : e;
+  if (e == cudaSuccess) e = argus_configure_partition(ctx);
+  if (e == cudaSuccess) e = argus_configure_compact(ctx);
+  return e == cudaSuccess ? argus_configure_paper_literal(ctx) : e;
+}
+// Let `kernel` ask for all the dynamic shared memory the device can give it (what is left beside its static
+// arrays).  The attribute is per function and process-wide: setting it ONCE, in argus_create, to a value that
+// does not depend on the call means contexts on other threads can only ever write the same number.
+template <typename K>
+inline cudaError_t argus_optin_all_smem(K kernel, int max_smem_optin) {
+  cudaFuncAttributes a;
+  cudaError_t e = cudaFuncGetAttributes(&a, kernel);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin - (int)a.sharedSizeBytes);
 }
 
 // ---- device helpers shared by the kernels ------------------------------------------------------

@@ -48,7 +48,8 @@ template <bool TRIPLE>
 __device__ __forceinline__ uint32_t entry_bytes(const Src& src, const argus_dims& D, uint32_t key, uint32_t sig,
                                                 uint32_t& b0, uint32_t& nb) {
   if (TRIPLE) {
-    const uint32_t n = src.n_clusters[(size_t)key * D.S + sig];
+    uint32_t n = src.n_clusters[(size_t)key * D.S + sig];
+    n = n < src.mc ? n : src.mc;                 // a count beyond the slots of the cell cannot be honoured (and would not fit s_info)
     nb = n; b0 = 0u;
     return n ? 8u + 8u * n : 0u;
   }
@@ -342,9 +343,7 @@ cudaError_t launch(argus_ctx* ctx, const Src& src, uint8_t* d_out, uint64_t capa
     uint32_t* ticket = reinterpret_cast<uint32_t*>(ctx->d_counters + 8);    // spare word of the counters area
     cudaError_t e = cudaMemsetAsync(ticket, 0, sizeof(uint32_t), s);
     if (e == cudaSuccess) e = cudaMemsetAsync(d_offsets, 0, sizeof(unsigned long long) * ((size_t)n_rec + 1u), s);
-    if (e == cudaSuccess && info_bytes > 48u * 1024u)
-      e = cudaFuncSetAttribute(compact_fused_kernel<TRIPLE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)info_bytes);
-    if (e != cudaSuccess) return e;
+    if (e != cudaSuccess) return e;              // (the kernel's shared-memory opt-in was set in argus_create)
     compact_fused_kernel<TRIPLE><<<n_rec, NT, info_bytes, s>>>(src, ctx->dims, d_offsets, ticket, d_out, capacity);
     compact_strip_kernel<<<(n_rec + 256u) / 256u, 256, 0, s>>>(d_offsets, n_rec);
     ctx->n_memsets += 2;
@@ -359,6 +358,11 @@ cudaError_t launch(argus_ctx* ctx, const Src& src, uint8_t* d_out, uint64_t capa
 }
 
 }  // namespace
+
+cudaError_t argus_configure_compact(argus_ctx* ctx) {
+  cudaError_t e = argus_optin_all_smem(compact_fused_kernel<false>, ctx->max_smem_optin);
+  return e == cudaSuccess ? argus_optin_all_smem(compact_fused_kernel<true>, ctx->max_smem_optin) : e;
+}
 
 cudaError_t argus_launch_sparse_encode(argus_ctx* ctx, const void* d_records, uint8_t* d_out, uint64_t capacity,
                                        uint64_t* d_offsets, cudaStream_t s) {

@@ -540,17 +540,20 @@ __global__ void __launch_bounds__(256)
 pack_sig_plane_kernel(const unsigned long long* __restrict__ sums, argus_dims D, uint32_t s0, uint32_t ns,
                       unsigned long long* __restrict__ dst, uint32_t stride, uint32_t off) {
   __shared__ unsigned long long tile[32][33];
-  const uint32_t t = blockIdx.z;
   const uint32_t sb = blockIdx.x * 32u, rb = blockIdx.y * 32u;
   const uint32_t tx = threadIdx.x & 31u, ty = threadIdx.x >> 5;      // 32 x 8
-  for (uint32_t i = ty; i < 32u; i += 8u) {
-    const uint32_t r = rb + i, sg = sb + tx;
-    tile[i][tx] = (r < D.R && sg < ns) ? __ldg(sums + ((size_t)r * D.T + t) * D.S + s0 + sg) : 0ull;
-  }
-  __syncthreads();
-  for (uint32_t i = ty; i < 32u; i += 8u) {
-    const uint32_t sg = sb + i, r = rb + tx;
-    if (sg < ns && r < D.R) dst[((size_t)t * ns + sg) * stride + off + r] = tile[tx][i];
+  // gridDim.z = min(T, 65535) (the grid's z limit): a CTA walks the steps z, z + gridDim.z, ...
+  for (uint32_t t = blockIdx.z; t < D.T; t += gridDim.z) {
+    for (uint32_t i = ty; i < 32u; i += 8u) {
+      const uint32_t r = rb + i, sg = sb + tx;
+      tile[i][tx] = (r < D.R && sg < ns) ? __ldg(sums + ((size_t)r * D.T + t) * D.S + s0 + sg) : 0ull;
+    }
+    __syncthreads();
+    for (uint32_t i = ty; i < 32u; i += 8u) {
+      const uint32_t sg = sb + i, r = rb + tx;
+      if (sg < ns && r < D.R) dst[((size_t)t * ns + sg) * stride + off + r] = tile[tx][i];
+    }
+    __syncthreads();                                                 // the next step reuses the tile
   }
 }
 
@@ -558,9 +561,9 @@ pack_sig_plane_kernel(const unsigned long long* __restrict__ sums, argus_dims D,
 __global__ void __launch_bounds__(256)
 pack_span_plane_kernel(const uint8_t* __restrict__ records, argus_dims D, unsigned long long* __restrict__ dst,
                        uint32_t stride, uint32_t off) {
-  const uint32_t n = D.T * (D.P + 1u) * D.R;
-  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    const uint32_t r = i % D.R, tk = i / D.R, k = tk % (D.P + 1u), t = tk / (D.P + 1u);
+  const uint64_t n = (uint64_t)D.T * (D.P + 1u) * D.R;                // R*T < 2^31, P <= 64: up to 2^37
+  for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (uint64_t)gridDim.x * blockDim.x) {
+    const uint32_t r = (uint32_t)(i % D.R), tk = (uint32_t)(i / D.R), k = tk % (D.P + 1u), t = tk / (D.P + 1u);
     const argus_span* sp = reinterpret_cast<const argus_span*>(records + ((size_t)r * D.T + t) * D.rec_bytes + D.span_off) + k;
     dst[(size_t)tk * stride + off + r] = sp->span_ns;
   }
@@ -574,14 +577,15 @@ cudaError_t argus_launch_pack_planes(argus_ctx* ctx, const void* d_records, uint
   const argus_dims& D = ctx->dims;
   if (dst_sig && s1 > s0) {
     const uint32_t ns = s1 - s0;
-    dim3 grid((ns + 31u) / 32u, (D.R + 31u) / 32u, D.T);
+    dim3 grid((ns + 31u) / 32u, (D.R + 31u) / 32u, D.T < 65535u ? D.T : 65535u);
     pack_sig_plane_kernel<<<grid, 256, 0, s>>>(D.sums, D, s0, ns, reinterpret_cast<unsigned long long*>(dst_sig),
                                                stride, off);
     ctx->n_kernels += 1;
   }
   if (dst_span) {
-    const uint32_t n = D.T * (D.P + 1u) * D.R;
-    pack_span_plane_kernel<<<(n + 255u) / 256u, 256, 0, s>>>(static_cast<const uint8_t*>(d_records), D,
+    const uint64_t n = (uint64_t)D.T * (D.P + 1u) * D.R;
+    const uint64_t want = (n + 255u) / 256u;                         // grid-stride beyond 2^20 CTAs
+    pack_span_plane_kernel<<<(unsigned)(want < (1u << 20) ? want : (1u << 20)), 256, 0, s>>>(static_cast<const uint8_t*>(d_records), D,
                                                             reinterpret_cast<unsigned long long*>(dst_span), stride, off);
     ctx->n_kernels += 1;
   }

@@ -909,12 +909,31 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
 
 // ---- NEXT-3: L2 ---------------------------------------------------------------------------------------------
 // One CTA per routed event k (phase span, index P = whole iteration): x_r = mean over the T steps of span_ns.
+// Group sums are taken in a FIXED order (no floating-point atomics): the member count of every group comes from
+// integer atomics, a group of one is its member's value, and every larger group is summed by one warp — lane l
+// adds its members r = l, l + 32, ... in ascending order, then the 32 partial sums meet in a fixed shuffle tree —
+// so that mu, sigma, CV, z and with them the CV class and the z > threshold flag are the same bits in every run.
+__device__ __forceinline__ double l2_group_sum(const uint32_t* __restrict__ gid, const double* xb, uint32_t R, uint32_t g,
+                                               double mu, bool squared) {
+  const uint32_t lane = threadIdx.x & 31u;
+  double acc = 0.0;
+  for (uint32_t r = lane; r < R; r += 32u)
+    if (gid[r] == g) {
+      const double d = squared ? xb[r] - mu : xb[r];
+      acc += squared ? d * d : d;
+    }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);   // xor tree: all lanes, same order
+  return acc;
+}
+
 __global__ void __launch_bounds__(1024)
-l2_kernel(const uint8_t* __restrict__ records, argus_dims D, const uint8_t* __restrict__ route,
+l2_kernel(const uint8_t* __restrict__ records, argus_dims D, const uint8_t* __restrict__ route, uint32_t n_dims,
           const uint32_t* __restrict__ group_id, double z_thr, argus_l2_group* __restrict__ groups,
           double* __restrict__ z_out, uint8_t* __restrict__ flag_out, double* __restrict__ xbar_ws) {
   const uint32_t k = blockIdx.x, R = D.R;
-  const uint32_t* gid = group_id + (size_t)route[k] * R;
+  const bool routed = route[k] < n_dims;          // a route byte beyond the dimensions given: the event joins no group
+  const uint32_t* gid = group_id + (size_t)(routed ? route[k] : 0u) * R;
   argus_l2_group* G = groups + (size_t)k * R;
   double* xb = xbar_ws + (size_t)k * R;
   for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
@@ -928,39 +947,30 @@ l2_kernel(const uint8_t* __restrict__ records, argus_dims D, const uint8_t* __re
     g.n = 0u; g.cls = 0u; g.mu = 0.0; g.sigma = 0.0; g.cv = 0.0;
     G[r] = g;
   }
-  __syncthreads();
-  // group sums (fp64 L2 atomics: a few thousand adds), then means, then squared deviations
-  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
-    if (gid[r] >= R) continue;              // not a member of any group of this dimension: z = 0
-    atomicAdd(&G[gid[r]].n, 1u);
-    atomicAdd(&G[gid[r]].mu, xb[r]);
-  }
   __threadfence();
   __syncthreads();
-  for (uint32_t g = threadIdx.x; g < R; g += blockDim.x)
-    if (G[g].n) G[g].mu = G[g].mu / (double)G[g].n;
+  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x)
+    if (routed && gid[r] < R) atomicAdd(&G[gid[r]].n, 1u);       // integer: exact whatever the order
   __threadfence();
   __syncthreads();
-  for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
-    if (gid[r] >= R) continue;
-    const double d = xb[r] - G[gid[r]].mu;
-    atomicAdd(&G[gid[r]].sigma, d * d);
-  }
-  __threadfence();
-  __syncthreads();
-  for (uint32_t g = threadIdx.x; g < R; g += blockDim.x) {
-    argus_l2_group q = G[g];
-    if (!q.n) continue;
-    q.sigma = q.n > 1u ? sqrt(q.sigma / (double)(q.n - 1u)) : 0.0;             // eq. (5): |G| - 1
+  const uint32_t warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5, lane = threadIdx.x & 31u;
+  for (uint32_t g = warp; g < R; g += n_warps) {
+    const uint32_t n = G[g].n;
+    if (n == 0u) continue;
+    argus_l2_group q;
+    q.n = n;
+    q.mu = l2_group_sum(gid, xb, R, g, 0.0, false) / (double)n;
+    const double ss = n > 1u ? l2_group_sum(gid, xb, R, g, q.mu, true) : 0.0;
+    q.sigma = n > 1u ? sqrt(ss / (double)(n - 1u)) : 0.0;                       // eq. (5): |G| - 1
     q.cv = (q.mu > 0.0 && q.sigma > 0.0) ? q.sigma / q.mu : 0.0;                // R34
     q.cls = q.cv < 0.02 ? 0u : (q.cv < 0.05 ? 1u : 2u);
-    G[g] = q;
+    if (lane == 0u) G[g] = q;
   }
   __threadfence();
   __syncthreads();
   for (uint32_t r = threadIdx.x; r < R; r += blockDim.x) {
     double z = 0.0;
-    if (gid[r] < R) {
+    if (routed && gid[r] < R) {
       const argus_l2_group q = G[gid[r]];
       if (q.sigma > 0.0) z = (xb[r] - q.mu) / q.sigma;
     }
@@ -1125,12 +1135,15 @@ size_t argus_l3_smem_bytes(uint32_t R) {
   return sizeof(double) * ((size_t)n2 + R) + sizeof(uint16_t) * 2u * n2;
 }
 
+cudaError_t argus_configure_paper_literal(argus_ctx* ctx) {
+  cudaError_t e = argus_optin_all_smem(l3_kernel, ctx->max_smem_optin);
+  return e == cudaSuccess ? argus_optin_all_smem(l1_kernel, ctx->max_smem_optin) : e;
+}
+
 cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l3_params* P, double* d_score,
                             argus_l3_stat* d_stat, uint8_t* d_flags, cudaStream_t s) {
   if (in->n_keys == 0) return cudaSuccess;
   const size_t smem = argus_l3_smem_bytes(in->n_ranks);
-  cudaError_t e = cudaFuncSetAttribute(l3_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
   // one CTA per key: every thread owns <= 4 ranks, and a rank each in the scan when R <= 1024 — small jobs get
   // small CTAs, so that several keys share an SM
   uint32_t n2 = 1;
@@ -1141,11 +1154,11 @@ cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l
   return cudaGetLastError();
 }
 
-cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, const uint32_t* d_group_id,
-                            double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
+cudaError_t argus_launch_l2(argus_ctx* ctx, const void* d_records, const uint8_t* d_route, uint32_t n_dims,
+                            const uint32_t* d_group_id, double z_thr, argus_l2_group* d_groups, double* d_z, uint8_t* d_flags, double* d_xbar,
                             cudaStream_t s) {
   // few CTAs (one per routed event), each a chain of strided loads and fenced phases: as many threads as a CTA takes
-  l2_kernel<<<ctx->dims.P + 1u, ctx->dims.R >= 1024u ? 1024 : 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, d_route, d_group_id, z_thr,
+  l2_kernel<<<ctx->dims.P + 1u, ctx->dims.R >= 1024u ? 1024 : 256, 0, s>>>(static_cast<const uint8_t*>(d_records), ctx->dims, d_route, n_dims, d_group_id, z_thr,
                                              d_groups, d_z, d_flags, d_xbar);
   ctx->n_kernels += 1;
   return cudaGetLastError();
@@ -1155,8 +1168,6 @@ cudaError_t argus_launch_l1(argus_ctx* ctx, const void* d_base, uint64_t sstride
                             uint32_t T, const argus_l1_params* P, argus_l1_out* d_out, cudaStream_t s) {
   if (n_series == 0 || T == 0) return cudaSuccess;
   const size_t smem = sizeof(double) * 2u * T * 4u;
-  cudaError_t e = cudaFuncSetAttribute(l1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  if (e != cudaSuccess) return e;
   l1_kernel<<<(n_series + 3u) / 4u, 128, smem, s>>>(static_cast<const uint8_t*>(d_base), sstride, tstride, n_series, T, *P,
                                                    d_out);
   ctx->n_kernels += 1;

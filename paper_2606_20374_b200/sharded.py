@@ -287,6 +287,7 @@ def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
     total = D.sum_over_ranks(world, float(n))
     valid = D.sum_over_ranks(world, float(nv))
     if g != 0:
+        sh.close()                                   # every rank releases its context, not only the one that prints
         return
     peak, peak_src = measured_peak_gbs()
     table_bytes = s.n_ranks * s.n_steps * (64 + 32 * (s.n_phases + 1) + 160 * s.n_sigs)

@@ -142,6 +142,14 @@ def test_triple_stream_matches_oracle():
     got = out.cpu().numpy()
     for r in range(3):
         assert bytes(got[offs[r]:offs[r + 1]]) == bytes(gold["triple"][r]), r
+    # a count beyond the slots of a cell is read as max_clusters (include/argus.h): same stream as the clamped input
+    over = np.where(n == 2, 255, n).astype(np.uint8)
+    assert (over > 2).any()
+    out2 = torch.zeros_like(out)
+    off2 = torch.zeros_like(off)
+    ctx.triple_encode(rec, _cuda(c.view(np.uint8).reshape(-1)), _cuda(over.reshape(-1)), 2, out2, off2)
+    assert [int(v) for v in off2.cpu().numpy()] == offs
+    assert (out2.cpu().numpy()[:offs[-1]] == got[:offs[-1]]).all()
     ctx.close()
 
 

@@ -378,6 +378,21 @@ def test_l2_groups_on_a_table():
         assert np.allclose(z[k][member], wz, rtol=1e-8, atol=1e-9) and (z[k][~member] == 0).all()
         clear = np.abs(wz - 1.5) > 1e-6
         assert (fl[k][member][clear] == wf[clear]).all() and (fl[k][~member] == 0).all()
+    # Fixed-order group sums: a second run gives the same BITS (the kernel has no floating-point atomics); and a
+    # route byte beyond n_dims sends its event to no group instead of reading past d_group_id.
+    route2 = route.copy()
+    route2[0] = 7
+    d_g2, d_z2, d_f2 = torch.full_like(d_g, 0x5A), torch.full_like(d_z, 3.0), torch.full_like(d_f, 9)
+    ctx.l2_groups(rec, _cuda(route2), _cuda(gid), 1.5, d_g2, d_z2, d_f2, d_x)
+    ctx.stats()
+    G2 = d_g2.cpu().numpy().view(A.L2_GROUP_DTYPE).reshape(P + 1, R)
+    assert (G2[1:].view(np.uint8) == G[1:].view(np.uint8)).all()
+    assert (d_z2.cpu().numpy().reshape(P + 1, R)[1:].view(np.uint64) == z[1:].view(np.uint64)).all()
+    assert (d_f2.cpu().numpy().reshape(P + 1, R)[1:] == fl[1:]).all()
+    assert (G2[0]["n"] == 0).all() and (d_z2.cpu().numpy()[:R] == 0).all() and (d_f2.cpu().numpy()[:R] == 0).all()
+    with pytest.raises(A.ArgusError) as e:
+        ctx.l2_groups(rec, _cuda(route), _cuda(gid), 1.5, d_g, d_z, d_f, d_x, n_dims=0)
+    assert e.value.code == A.EINVAL
     ctx.close()
 
 

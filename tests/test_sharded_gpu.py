@@ -116,3 +116,35 @@ def test_planes_argument_errors():
     assert code(ctx.diagnose_planes, None, span, 8, 8, 0, big) == A.OK
     ctx.stats()
     ctx.close()
+
+
+def test_pack_planes_with_more_steps_than_one_grid_dimension():
+    """T > 65535 (the z limit of a grid): the sig-plane export walks the steps inside the kernel."""
+    import torch
+    from paper_2606_20374_b200 import argus as A
+    R, T, S, P = 2, 70000, 3, 1
+    steps = np.array([0, 1, 65534, 65535, 65536, 69999], dtype=np.uint32)
+    ev = np.zeros(steps.size * R, dtype=A.EVENT_DTYPE)
+    ev["rank"] = np.repeat(np.arange(R, dtype=np.uint32), steps.size)
+    ev["step"] = np.tile(steps, R)
+    ev["sig"] = np.arange(ev.size) % S
+    ev["start_ns"] = 1000 + np.arange(ev.size) * 10
+    ev["end_ns"] = ev["start_ns"] + 7 + np.arange(ev.size) * 3
+    ctx = A.Argus(R, T, S, P)
+    rec = ctx.alloc_records()
+    ctx.reset(rec)
+    ctx.aggregate(torch.from_numpy(ev.view(np.uint8).reshape(-1).copy()).cuda(), ev.size, rec)
+    ctx.phase_times(rec)
+    sig_plane = torch.full((T * S * R,), -1, dtype=torch.int64, device="cuda")
+    span_plane = torch.full((T * (P + 1) * R,), -1, dtype=torch.int64, device="cuda")
+    ctx.pack_planes(rec, 0, S, sig_plane, span_plane, R, 0)
+    ctx.stats()
+    got_sig = sig_plane.cpu().numpy().reshape(T, S, R)
+    got_span = span_plane.cpu().numpy().reshape(T, P + 1, R)
+    o, _, _ = run_oracle(ev, R, T, S, P, 0)
+    cells = o.cells().reshape(R, T, S)
+    spans = o.spans().reshape(R, T, P + 1)
+    assert (got_sig == cells["sum"].astype(np.int64).transpose(1, 2, 0)).all()
+    assert (got_span == spans["span"].astype(np.int64).transpose(1, 2, 0)).all()
+    assert int(got_sig[69999].sum()) > 0 and int(got_sig[65536].sum()) > 0
+    ctx.close()
