@@ -141,6 +141,18 @@ def oracle_sample(wl, n_ranks_sample: int, threads: int):
     return n_ev, dt, o
 
 
+def workload_config(s):
+    """The `config` object of the JSON line: the workload and what the timing rules ask to be said about it.
+    The same keys and values on both arms (the driver compares them)."""
+    n = s.total_events
+    return {"workload": s.name, "n_ranks": s.n_ranks, "n_steps": s.n_steps,
+            "events_per_rank_step": s.n_events, "n_sigs": s.n_sigs, "n_phases": s.n_phases,
+            "events": n, "raw_bytes": 32 * n,
+            "table_bytes": s.n_ranks * s.n_steps * (64 + 32 * (s.n_phases + 1) + 160 * s.n_sigs),
+            "l2": "inputs (raw events) are larger than L2; no flush needed",
+            "jobs": "one independent job of this size per GPU"}
+
+
 def run_reference(args, world):
     """--impl reference: the CPU oracle on this box's host cores (rank 0 only)."""
     from paper_2606_20374_b200.workload import build_workload
@@ -162,8 +174,7 @@ def run_reference(args, world):
         "impl": "reference", "metric": METRIC, "value": v, "unit": "events/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-        "config": {"workload": s.name, "n_ranks": s.n_ranks, "n_steps": s.n_steps,
-                   "events_per_rank_step": s.n_events, "n_sigs": s.n_sigs, "n_phases": s.n_phases},
+        "config": workload_config(s),
         "raw_event_gbs": 32 * v / 1e9,
         "cpu_baseline": {"value": v, "unit": "events/s", "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": "events/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -175,7 +186,7 @@ def _ms(pairs):
     return [a.elapsed_time(b) for a, b in pairs]
 
 
-def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=4096, fine_limit_bytes=6 << 30):
+def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=4096, fine_limit_bytes=24 << 30):
     """The SURVEY 8(f) NEXT rows on the table the timed steps left behind (finalised), each call timed alone
     with CUDA events (1 warm-up, median of `reps`); outside the step's timed region.  Bytes are the
     algorithmic ones of DESIGN.md 6.6 / 6.7 (what the call must read and write), GB/s = bytes / median time.
@@ -248,8 +259,9 @@ def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=4096, fine_limit_bytes=6 
         ms, best = timed(lambda: ctx.kde_clusters(hist, n_cells, p256, d_c8, d_n8))
         out["next1_kde_fine"] = line(ms, best, n_cells * (1024 + 8 * MC + 1), "hbm (1 KB of counters per cell) / alu",
                                      cells=n_cells, cells_per_s=n_cells / (ms * 1e-3), clusters=int(d_n8.sum()))
-        del hist, d_c8, d_n8
+        del hist, d_n8
     else:
+        d_c8 = None
         out["next1_fine_hist"] = {"skipped": f"[R][T][S][256] u32 = {fine_bytes / 2**30:.1f} GiB: measured on mid / scale"}
     # NEXT-2: regroup the triples per key, then score the first l3_keys keys over all R ranks
     d_cnt = torch.zeros(K * R * MC, dtype=torch.int32, device=dev)
@@ -262,10 +274,26 @@ def next_rows(ctx, rec, d_ev, s, peak, reps=5, l3_keys=4096, fine_limit_bytes=6 
     d_score = torch.zeros(kk * R, dtype=torch.float64, device=dev)
     d_stat = torch.zeros(kk * 5, dtype=torch.float64, device=dev)
     d_fl = u8(kk * R)
-    ms, best = timed(lambda: ctx.l3_detect(d_cnt, d_p50, d_p99, kk, R, MC, d_score, d_stat, d_fl, n_grid=G))
-    out["next2_l3_detect"] = line(ms, best, kk * R * (MC * 20 + 9), "alu / shared memory (a sort of R CDF values per grid point)",
-                                  keys=kk, ranks=R, n_grid=G, cdf_points_per_s=kk * R * G / (ms * 1e-3),
-                                  flagged=int(d_fl.sum()))
+    def l3_row(n_keys, what):
+        c0 = ctx.l3_path_count()
+        ms, best = timed(lambda: ctx.l3_detect(d_cnt, d_p50, d_p99, n_keys, R, MC, d_score, d_stat, d_fl, n_grid=G))
+        c1 = ctx.l3_path_count()
+        per = [(b - a) // (reps + 1) for a, b in zip(c0, c1)]            # counted by the kernel, per call
+        bound = "alu / shared memory: " + ("class path (weighted sums over <= 256 classes of identical mixtures)"
+                                           if per[1] == 0 else
+                                           "general path (a sort of R CDF values per grid point)" if per[0] == 0 else
+                                           "class path and general path mixed, see keys_*") + "; " + what
+        return line(ms, best, n_keys * R * (MC * 20 + 9), bound, keys=n_keys, ranks=R, n_grid=G,
+                    keys_class_path=per[0], keys_general_path=per[1], keys_empty=per[2], us_per_key=ms * 1e3 / n_keys,
+                    cdf_points_per_s=n_keys * R * G / (ms * 1e-3), flagged=int(d_fl[:n_keys * R].sum()))
+    out["next2_l3_detect"] = l3_row(kk, "clusters of the records' 32-bucket histograms")
+    if d_c8 is not None:
+        # NEXT-2 on the clusters of the FINE grid (8 bins per octave, what PAPER.md:178 describes): ranks rarely share
+        # a mixture there, so this is the general path of the L3 kernel (a sort of R CDF values per grid point)
+        kf = min(K, 512)
+        ctx.clusters_to_l3(d_c8, MC, 8, d_cnt, d_p50, d_p99)
+        out["next2_l3_detect_fine"] = l3_row(kf, "clusters of the fine grid (8 bins per octave)")
+        del d_c8
     del d_cnt, d_p50, d_p99, d_c, d_n
     # NEXT-3: L2 over every phase span (one group per 8 consecutive ranks), L1 over the R iteration-time series
     route = u8(P + 1)
@@ -303,6 +331,10 @@ def run_ours(args, world):
     if args.bimodal > 0.0:
         wl0 = build_workload(dataclasses.replace(wl0.spec, bimodal_frac=args.bimodal,
                                                  name=wl0.spec.name + f"+bimodal{args.bimodal:g}"))
+    if args.sigs > 0:
+        # the paper's key count (~100 active (kernel, stream) combinations, ~2 clusters each) on the
+        # named workload's event volume: the like-for-like figure beside "~10 MB -> ~2.7 KB" (context, not a target)
+        wl0 = build_workload(dataclasses.replace(wl0.spec, n_sigs=args.sigs, name=wl0.spec.name + f"+sigs{args.sigs}"))
     spec = dataclasses.replace(wl0.spec, seed=D.job_seed(wl0.spec.seed, world))
     wl = build_workload(spec) if world.rank else wl0
     s = wl.spec
@@ -381,16 +413,43 @@ def run_ours(args, world):
             h_out = {k: torch.empty(v.shape, dtype=v.dtype, pin_memory=True) for k, v in outs.items()}
             d2h = sum(v.numel() * v.element_size() for v in outs.values())
             rec_keep = rec.clone()
+            # The summary leaves the device too (NS (5): the reducer uploads the compressed
+            # records): the paper's (count, p50, p99) TRIPLE stream of every rank-step, encoded after the
+            # diagnosis and copied to pinned host memory with its offsets, all inside the timed region.
+            MC = 8
+            n_cells = s.n_ranks * s.n_steps * s.n_sigs
+            n_rec = s.n_ranks * s.n_steps
+            p32 = ctx.kde_params(per_octave=1, n_bins=32, max_clusters=MC)
+            d_c = torch.zeros(n_cells * MC * 8, dtype=torch.uint8, device=f"cuda:{dev}")
+            d_n = torch.zeros(n_cells, dtype=torch.uint8, device=f"cuda:{dev}")
+            d_stream = torch.empty(ctx.triple_bound(MC), dtype=torch.uint8, device=f"cuda:{dev}")
+            d_off = torch.zeros(n_rec + 1, dtype=torch.int64, device=f"cuda:{dev}")
+            ctx.kde_clusters_records(rec, p32, d_c, d_n)          # the resident leg's stream (rec is finalised)
+            ctx.triple_encode(rec, d_c, d_n, MC, d_stream, d_off)
+            ref_len = int(d_off[-1])
+            ref_stream, ref_off = d_stream[:ref_len].cpu(), d_off.cpu()
+            h_stream = torch.empty(d_stream.numel(), dtype=torch.uint8, pin_memory=True)
+            h_off = torch.empty(n_rec + 1, dtype=torch.int64, pin_memory=True)
+            h_len = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+            d_stream.zero_(); d_off.zero_()
             for v in outs.values():
                 v.zero_()
+            shipped = [0]
 
             def e2e_step():
                 ctx.reset(rec)
                 ctx.aggregate_host(h_ev, n, chunk, d_ring, RING_SLOTS, rec)
                 ctx.phase_times(rec)
                 ctx.diagnose(rec, outs)
+                ctx.kde_clusters_records(rec, p32, d_c, d_n)
+                ctx.triple_encode(rec, d_c, d_n, MC, d_stream, d_off)
                 for k in outs:
                     h_out[k].copy_(outs[k], non_blocking=True)
+                h_off.copy_(d_off, non_blocking=True)
+                h_len.copy_(d_off[-1:], non_blocking=True)
+                torch.cuda.current_stream().synchronize()     # the stream's length is known only now (8 bytes)
+                shipped[0] = int(h_len[0])
+                h_stream[:shipped[0]].copy_(d_stream[:shipped[0]], non_blocking=True)
 
             e2e_steps = max(1, min(args.steps, args.e2e_steps))
             e2e_step()
@@ -410,7 +469,11 @@ def run_ours(args, world):
             for k in outs:
                 verified = verified and bool(torch.equal(outs[k], resident[k])) and \
                     bool(torch.equal(h_out[k], resident[k].cpu()))
-            del rec_keep
+            # ... and the shipped record stream, byte for byte, with the one encoded from the resident leg's table
+            verified = verified and shipped[0] == ref_len and bool(torch.equal(h_off, ref_off)) and \
+                bool(torch.equal(h_stream[:ref_len], ref_stream))
+            d2h += ref_len + h_off.numel() * 8 + 8
+            del rec_keep, d_c, d_n, d_stream, ref_stream
             # overlap efficiency max(t_copy, t_agg) / t_total: the copies alone through
             # the same ring on the copy stream (argus_ingest), the aggregation alone from the resident
             # leg, and the overlapped host-streamed aggregation
@@ -437,6 +500,9 @@ def run_ours(args, world):
                    "steps": e2e_steps, "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": d2h,
                    "h2d_gbs": 32 * n / (e_ms * 1e-3) / 1e9, "chunk_bytes": chunk * 32,
                    "ring_slots": RING_SLOTS, "verified": verified,
+                   "shipped": {"encoding": "triple (R38: per cell its (count, p50, p99) clusters, max 8) + offsets + "
+                                           "the six diagnosis outputs", "stream_bytes": ref_len,
+                               "raw_over_stream": 32 * n / max(1, ref_len)},
                    "overlap": {"t_copy_ms": t_copy, "t_agg_ms": agg_ms, "t_total_ms": t_total,
                                "efficiency": max(t_copy, agg_ms) / t_total}}
         except Exception as e:  # e.g. the box cannot pin the whole buffer
@@ -457,19 +523,17 @@ def run_ours(args, world):
         "warmup": args.warmup, "ms_per_step": ms_step, "ms_per_step_median": float(np.median(step_list)),
         "ms_per_step_best": float(np.min(step_list)), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "int64", "data": "synthetic",
-        "config": {"workload": s.name, "n_ranks": s.n_ranks, "n_steps": s.n_steps,
-                   "events_per_rank_step": s.n_events, "n_sigs": s.n_sigs, "n_phases": s.n_phases,
-                   "events": n, "raw_bytes": 32 * n, "table_bytes": ctx.table_bytes,
-                   "workspace_bytes": ctx.workspace_bytes,
-                   "l2": "inputs (raw events) are larger than L2; no flush needed",
-                   "jobs": "one independent job of this size per GPU"},
+        "config": workload_config(s), "workspace_bytes": ctx.workspace_bytes,
         "raw_event_gbs": 32 * value / 1e9,
         "hbm_frac_step": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
         "hbm_frac_step_vs_8tbs": step_bytes / (ms_step * 1e-3) / 1e9 / 8000.0,
         "roofline": {"bound": "hbm", "kernel": "aggregate_seg_kernel" if not s.shuffle else
                      "argus_aggregate = grouping pass + aggregate_seg_kernel",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src, "kernel_ms": agg_ms,
+                     "traffic": traffic,
+                     "traffic_source": None if traffic is None else
+                     f"committed ncu --set full capture profiles/{s.name}_seg_traffic.txt (a constant read from that "
+                     "file, not measured in this run)", "peak_source": peak_src, "kernel_ms": agg_ms,
                      "kernel_ms_median": float(np.median(agg_list)), "kernel_ms_best": float(np.min(agg_list)),
                      "algorithmic_bytes": alg_bytes, "share_of_step": agg_ms / ms_step},
         "clocks": clocks, "e2e": e2e,
@@ -537,6 +601,8 @@ def main():
                     help="--scaling strong: all_to_all_single (NCCL) or peer stores through symmetric memory")
     ap.add_argument("--bimodal", type=float, default=0.0,
                     help="stress knob: share of the sigs with a second duration mode 8-64x the first (PAPER.md:166)")
+    ap.add_argument("--sigs", type=int, default=0,
+                    help="override the workload's signature count (e.g. 128: the paper's ~100 keys per rank)")
     ap.add_argument("--spill", type=int, default=-1,
                     help="argus_config.max_spill_events: -1 = a quarter of the events (default), 0 = no spill area")
     ap.add_argument("--e2e-steps", type=int, default=3)

@@ -439,6 +439,13 @@ int argus_stats(argus_ctx* ctx, uint64_t* n_valid, uint64_t* n_invalid);
  * it.  Synchronises like argus_stats.  [host] outputs, may be NULL. */
 int argus_refused_count(argus_ctx* ctx, uint64_t* n_requeued, uint64_t* n_overflow);
 
+/* Keys argus_l3_detect has scored since argus_reset, by the way the kernel took: n_class = the ranks of the key
+ * fell into at most 256 classes of identical mixtures (the score is a weighted sum over classes), n_general = more
+ * distinct mixtures than that (a sort of the R CDF values per grid point; about an order of magnitude slower per
+ * key), n_empty = no rank had a cluster.  A throughput diagnostic: results do not depend on the path.
+ * Synchronises like argus_stats.  [host] outputs, may be NULL. */
+int argus_l3_path_count(argus_ctx* ctx, uint64_t* n_class, uint64_t* n_general, uint64_t* n_empty);
+
 /* Kernels and memsets this ctx has launched since argus_create (what bench.py reports as gpu_launches).
  * [host] outputs, may be NULL. */
 int argus_launch_count(const argus_ctx* ctx, uint64_t* kernels, uint64_t* memsets);

@@ -44,7 +44,7 @@ EXPORTS = ["argus_create", "argus_destroy", "argus_record_bytes", "argus_table_b
            "argus_aggregate_host", "argus_phase_times", "argus_diagnose", "argus_forget", "argus_pack_planes",
            "argus_diagnose_planes", "argus_diagnose_planes_static", "argus_fine_hist", "argus_kde_clusters", "argus_kde_clusters_records",
            "argus_sparse_bound", "argus_sparse_encode", "argus_triple_bound", "argus_triple_encode",
-           "argus_clusters_to_l3", "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count",
+           "argus_clusters_to_l3", "argus_l3_detect", "argus_l2_groups", "argus_l1_detect", "argus_stats", "argus_refused_count", "argus_l3_path_count",
            "argus_launch_count", "argus_tune", "argus_strerror", "argus_last_cuda_error",
            "argus_version"]
 
@@ -166,6 +166,8 @@ def load() -> ctypes.CDLL:
     lib.argus_stats.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_refused_count.restype = i32
     lib.argus_refused_count.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    lib.argus_l3_path_count.restype = i32
+    lib.argus_l3_path_count.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_launch_count.restype = i32
     lib.argus_launch_count.argtypes = [vp, ctypes.POINTER(u64), ctypes.POINTER(u64)]
     lib.argus_tune.restype = i32
@@ -402,6 +404,12 @@ class Argus:
         q = ArgusL1Params(window, min_seg, theta, beta, ratio_min, rsd_max)
         self._check(self.lib.argus_l1_detect(self._h, _ptr(d_base), series_stride, step_stride, n_series, n_steps,
                                              ctypes.byref(q), _ptr(d_out), _stream(stream)))
+
+    def l3_path_count(self):
+        """(keys on the class path, keys on the general path, keys without clusters) since reset."""
+        a, b, c = ctypes.c_uint64(), ctypes.c_uint64(), ctypes.c_uint64()
+        self._check(self.lib.argus_l3_path_count(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+        return a.value, b.value, c.value
 
     def stats(self):
         a, b = ctypes.c_uint64(), ctypes.c_uint64()

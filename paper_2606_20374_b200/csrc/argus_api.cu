@@ -48,7 +48,7 @@ void argus_ws_plan(const argus_config* c, int sm_count, int max_smem_optin, argu
   const size_t RT = (size_t)c->n_ranks * c->n_steps;
   size_t o = 0;
   L->state = o;     o += up256(sizeof(uint32_t) * RT);
-  L->counters = o;  o += up256(4 * sizeof(unsigned long long));
+  L->counters = o;  o += up256(16 * sizeof(unsigned long long));   // [0..3] events, [4..6] L3 paths, [8] encoder ticket
   L->hist = o;      o += up256(sizeof(uint32_t) * (RT + 1u));
   L->sums = o;      o += up256(sizeof(unsigned long long) * RT * c->n_sigs);
   L->ovf = o;       o += up256((size_t)ARGUS_MAX_SEG_CTAS * ARGUS_OVF_CAP * sizeof(uint4));
@@ -533,6 +533,18 @@ extern "C" int argus_refused_count(argus_ctx* ctx, uint64_t* n_requeued, uint64_
   CU(ctx, cudaMemcpy(h, ctx->d_counters + 2, sizeof h, cudaMemcpyDeviceToHost));
   if (n_overflow) *n_overflow = h[0];
   if (n_requeued) *n_requeued = h[1];
+  return ARGUS_OK;
+}
+
+extern "C" int argus_l3_path_count(argus_ctx* ctx, uint64_t* n_class, uint64_t* n_general, uint64_t* n_empty) {
+  if (!ctx) return ARGUS_EINVAL;
+  int rc = argus_stats(ctx, nullptr, nullptr);      // synchronises the streams
+  if (rc != ARGUS_OK) return rc;
+  unsigned long long h[3] = {0, 0, 0};
+  CU(ctx, cudaMemcpy(h, ctx->d_counters + 4, sizeof h, cudaMemcpyDeviceToHost));
+  if (n_class) *n_class = h[0];
+  if (n_general) *n_general = h[1];
+  if (n_empty) *n_empty = h[2];
   return ARGUS_OK;
 }
 

@@ -639,7 +639,7 @@ __device__ double l3_cdf_of(const uint32_t* cnt, const double* p50, const double
 
 __global__ void __launch_bounds__(1024)
 l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, argus_l3_stat* __restrict__ stat_out,
-          uint8_t* __restrict__ flags_out) {
+          uint8_t* __restrict__ flags_out, unsigned long long* __restrict__ path_count) {
   const uint32_t R = in.n_ranks, C = in.max_clusters, key = blockIdx.x, G = P.n_grid;
   uint32_t n2 = 1;
   while (n2 < R) n2 <<= 1;
@@ -771,6 +771,9 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
     }
     __syncthreads();
   }
+  // which way this key went (argus_l3_path_count): [0] ranks fell into <= 256 classes of identical mixtures,
+  // [1] the general path below (a sort of R CDF values per grid point), [2] no cluster at all
+  if (threadIdx.x == 0 && path_count) atomicAdd(&path_count[empty ? 2 : (by_class ? 0 : 1)], 1ull);
   if (!empty && !by_class) {
     // per-thread totals and, when they fit, the cached parameters of this thread's NON-EMPTY (rank, cluster)
     // pairs in (rank slot, cluster) order — the order the sums below take; a thread with more than L3_CACHE of
@@ -913,11 +916,11 @@ l3_kernel(argus_l3_in in, argus_l3_params P, double* __restrict__ score_out, arg
 // integer atomics, a group of one is its member's value, and every larger group is summed by one warp — lane l
 // adds its members r = l, l + 32, ... in ascending order, then the 32 partial sums meet in a fixed shuffle tree —
 // so that mu, sigma, CV, z and with them the CV class and the z > threshold flag are the same bits in every run.
-__device__ __forceinline__ double l2_group_sum(const uint32_t* __restrict__ gid, const double* xb, uint32_t R, uint32_t g,
-                                               double mu, bool squared) {
+__device__ __forceinline__ double l2_group_sum(const uint32_t* __restrict__ gid, const double* xb, uint32_t first, uint32_t last,
+                                               uint32_t g, double mu, bool squared) {
   const uint32_t lane = threadIdx.x & 31u;
   double acc = 0.0;
-  for (uint32_t r = lane; r < R; r += 32u)
+  for (uint32_t r = first + lane; r <= last; r += 32u)      // only the span of ranks that holds the group's members
     if (gid[r] == g) {
       const double d = squared ? xb[r] - mu : xb[r];
       acc += squared ? d * d : d;
@@ -944,23 +947,35 @@ l2_kernel(const uint8_t* __restrict__ records, argus_dims D, const uint8_t* __re
     }
     xb[r] = s / (double)D.T;
     argus_l2_group g;
-    g.n = 0u; g.cls = 0u; g.mu = 0.0; g.sigma = 0.0; g.cv = 0.0;
+    g.n = 0u; g.cls = 0xFFFFFFFFu; g.mu = 0.0; g.sigma = 0.0; g.cv = 0.0;
     G[r] = g;
   }
   __threadfence();
   __syncthreads();
+  // member count, first and last member of every group: integer atomics, exact whatever the order.  Until the
+  // group's entry is written below, its cls word holds the first member and the low word of cv the last one.
   for (uint32_t r = threadIdx.x; r < R; r += blockDim.x)
-    if (routed && gid[r] < R) atomicAdd(&G[gid[r]].n, 1u);       // integer: exact whatever the order
+    if (routed && gid[r] < R) {
+      argus_l2_group* q = &G[gid[r]];
+      atomicAdd(&q->n, 1u);
+      atomicMin(&q->cls, r);
+      atomicMax(reinterpret_cast<uint32_t*>(&q->cv), r);
+    }
   __threadfence();
   __syncthreads();
   const uint32_t warp = threadIdx.x >> 5, n_warps = blockDim.x >> 5, lane = threadIdx.x & 31u;
   for (uint32_t g = warp; g < R; g += n_warps) {
     const uint32_t n = G[g].n;
-    if (n == 0u) continue;
+    if (n == 0u) {                                          // no such group: the entry reads n = 0 and zeros
+      if (lane == 0u) G[g].cls = 0u;
+      continue;
+    }
+    const uint32_t first = G[g].cls, last = *reinterpret_cast<const uint32_t*>(&G[g].cv);
+    __syncwarp();                                           // every lane has read the bounds before lane 0 overwrites them
     argus_l2_group q;
     q.n = n;
-    q.mu = l2_group_sum(gid, xb, R, g, 0.0, false) / (double)n;
-    const double ss = n > 1u ? l2_group_sum(gid, xb, R, g, q.mu, true) : 0.0;
+    q.mu = l2_group_sum(gid, xb, first, last, g, 0.0, false) / (double)n;
+    const double ss = n > 1u ? l2_group_sum(gid, xb, first, last, g, q.mu, true) : 0.0;
     q.sigma = n > 1u ? sqrt(ss / (double)(n - 1u)) : 0.0;                       // eq. (5): |G| - 1
     q.cv = (q.mu > 0.0 && q.sigma > 0.0) ? q.sigma / q.mu : 0.0;                // R34
     q.cls = q.cv < 0.02 ? 0u : (q.cv < 0.05 ? 1u : 2u);
@@ -1149,7 +1164,7 @@ cudaError_t argus_launch_l3(argus_ctx* ctx, const argus_l3_in* in, const argus_l
   uint32_t n2 = 1;
   while (n2 < in->n_ranks) n2 <<= 1;
   const unsigned threads = n2 >= 1024u ? 1024u : (n2 < 64u ? 64u : n2);
-  l3_kernel<<<in->n_keys, threads, smem, s>>>(*in, *P, d_score, d_stat, d_flags);
+  l3_kernel<<<in->n_keys, threads, smem, s>>>(*in, *P, d_score, d_stat, d_flags, ctx->d_counters + 4);
   ctx->n_kernels += 1;
   return cudaGetLastError();
 }

@@ -185,3 +185,44 @@ def test_ingest_then_aggregate_host_keeps_the_dependency():
     ctx.aggregate(d_first, half, rec)                                      # must see the ingested bytes
     _finish(ctx, rec, ev, dims)
     ctx.close()
+
+
+def test_host_to_host_events_in_summary_stream_out():
+    """The whole e2e shape bench.py times (NS (2)-(5); the reducer's upload of its summaries):
+    pinned host events -> argus_aggregate_host -> phase_times -> diagnose -> argus_sparse_encode -> the stream and
+    its offsets copied to pinned HOST memory.  The host-side bytes, decoded by the independent reader of
+    tests/helpers.py, must rebuild the oracle's table byte for byte."""
+    import torch
+    from gpu_util import run_oracle
+    from helpers import sparse_to_dense
+    from paper_2606_20374_b200 import argus as A
+    wl = build_workload(scaled("mid", n_ranks=12, n_steps=3, n_events=5000, n_sigs=300))
+    ev = wl.expand_host()
+    dims = _dims(wl.spec)
+    R, T, S, P, base = dims
+    chunk = 7777                                         # ragged: cuts rank-steps anywhere
+    ctx = A.Argus(R, T, S, P, base)
+    h = _pinned(ev)
+    ring = torch.empty(2 * chunk * 32, dtype=torch.uint8, device="cuda")
+    rec = ctx.alloc_records()
+    rec.fill_(0xAB)
+    ctx.reset(rec)
+    ctx.aggregate_host(h, ev.size, chunk, ring, 2, rec)
+    ctx.phase_times(rec)
+    outs = ctx.alloc_diag()
+    ctx.diagnose(rec, outs)
+    d_out = torch.empty(ctx.sparse_bound(), dtype=torch.uint8, device="cuda")
+    d_off = torch.zeros(R * T + 1, dtype=torch.int64, device="cuda")
+    ctx.sparse_encode(rec, d_out, d_off)
+    h_off = torch.empty(R * T + 1, dtype=torch.int64, pin_memory=True)
+    h_off.copy_(d_off, non_blocking=True)
+    torch.cuda.current_stream().synchronize()
+    total = int(h_off[-1])
+    h_out = torch.empty(total, dtype=torch.uint8, pin_memory=True)
+    h_out.copy_(d_out[:total], non_blocking=True)
+    ctx.stats()
+    o, orec, _ = run_oracle(ev, *dims)
+    assert 0 < total < orec.size                          # it is a compression
+    dense = sparse_to_dense(bytes(h_out.numpy()), [int(v) for v in h_off.numpy()], S, P)
+    assert dense.shape == orec.shape and (dense == orec).all()      # the reader restores the dense header too
+    ctx.close()

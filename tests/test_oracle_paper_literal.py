@@ -232,3 +232,39 @@ def test_l1_change_point_finds_the_step():
     assert PL.l1_change_point(x[:6])[0] == 0                              # too short for two segments of 4
     assert PL.l1_classify(PL.l1_jitter(x), PL.l1_change_point(x)) in (2, 3)
     assert PL.l1_classify([], (0, 0, 0.0)) == 0
+
+
+def test_plateau_valley_belongs_to_its_left_edge():
+    """R27 ("local minima ... as candidate cluster boundaries"): bin j is a valley when f[j] < f[j-1] and
+    f[j] <= f[j+1], so a flat valley floor yields ONE boundary, at its left edge.  Two equal modes an odd number of
+    bins apart put the floor on two bins with exactly equal density (checked, not assumed): a rule strict on both
+    sides would find no valley at all, a rule lax on the left would pick the right-hand bin."""
+    for per_octave, n_bins, b1, b2 in ((1, 32, 10, 15), (8, 256, 40, 53)):
+        h = np.zeros(n_bins, dtype=np.int64)
+        h[b1] = h[b2] = 100
+        f, _, bounds, clusters = PL.kde_clusters(h, per_octave=per_octave, min_gap_bins=0)
+        j = (b1 + b2) // 2
+        assert f[j] == f[j + 1] and f[j] < f[j - 1] and f[j + 1] < f[j + 2]      # a two-bin plateau at the bottom
+        assert bounds == [j]
+        assert clusters == [(100, b1, b1), (100, b2, b2)]
+
+
+def test_l1_classify_exact_values():
+    """PAPER.md:222 "stable, jitter, regression, or both": bit 0 = some jitter interval of non-zero effective width,
+    bit 1 = a change point was found."""
+    spike = [(10, 17, 100.0, 3)]           # (first, last, baseline, width)
+    none_wide = [(10, 17, 100.0, 0)]       # a candidate whose run above beta x baseline is empty: not jitter
+    assert PL.l1_classify([], (0, 0, 0.0)) == 0
+    assert PL.l1_classify(none_wide, (0, 0, 0.0)) == 0
+    assert PL.l1_classify(spike, (0, 0, 0.0)) == 1
+    assert PL.l1_classify([], (1, 40, 1.3)) == 2
+    assert PL.l1_classify(none_wide, (1, 40, 1.3)) == 2
+    assert PL.l1_classify(spike + none_wide, (1, 40, 1.3)) == 3
+    # and on real series: a clean step is a regression only, a spike on a flat line jitter only, both together both
+    step = [100.0 + (i % 3) for i in range(40)] + [130.0 + (i % 3) for i in range(24)]
+    assert PL.l1_classify(PL.l1_jitter(step), PL.l1_change_point(step)) == 2
+    flat = [100.0] * 64
+    spiky = list(flat)
+    spiky[30] = spiky[31] = 200.0
+    assert PL.l1_classify(PL.l1_jitter(spiky), PL.l1_change_point(spiky)) == 1
+    assert PL.l1_classify(PL.l1_jitter(flat), PL.l1_change_point(flat)) == 0
