@@ -509,6 +509,18 @@ def run_ours(args, world):
             e2e = {"value": None, "unit": "events/s", "error": repr(e)[:200],
                    "h2d_bytes_per_step": 32 * n, "d2h_bytes_per_step": None}
 
+    # ---- N > 1: the SAME workload once more as ONE job sharded by trace rank: aggregation per
+    # shard, one exchange of the 8-byte-per-cell sum plane, selection per sig slice.  Reported beside the
+    # weak-scaling headline, never instead of it; unmeasured on hardware so far, hence guarded.
+    sharded_job = None
+    if world.size > 1 and args.scaling == "both" and not s.shuffle and args.bimodal == 0.0 and args.sigs == 0:
+        try:
+            from paper_2606_20374_b200 import sharded
+            torch.cuda.empty_cache()
+            sharded_job = sharded.bench_strong(args, world, METRIC, measured_peak_gbs, ClockSampler, emit=False)
+        except Exception as e:
+            sharded_job = {"error": repr(e)[:300]}
+
     if world.rank != 0:
         return
     peak, peak_src = measured_peak_gbs()
@@ -548,6 +560,8 @@ def run_ours(args, world):
         out["config"]["bimodal_sigs"] = wl.n_bimodal
     if nxt is not None:
         out["next_rows"] = nxt
+    if sharded_job is not None:
+        out["sharded_job"] = sharded_job
     if world.size == 1 and not args.no_cpu_baseline:
         k = args.cpu_baseline_ranks if args.cpu_baseline_ranks > 0 else s.n_ranks
         if args.cpu_baseline_ranks < 0:      # default: a bounded sample, about 15 s of oracle time
@@ -595,8 +609,10 @@ def main():
     ap.add_argument("--workload", default="production",
                     help="tiny | mid | scale | unsorted | production (BASELINE.json configs[0..4])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
-                    help="N > 1: weak = one job of the named size per GPU; strong = ONE job sharded by trace rank")
+    ap.add_argument("--scaling", default=None, choices=["weak", "strong", "both"],
+                    help="N > 1: weak = one job of the named size per GPU; strong = ONE job sharded by trace rank; "
+                         "both (the default for N > 1) = the weak line with the sharded job's numbers under "
+                         "\"sharded_job\"; N = 1 defaults to weak")
     ap.add_argument("--exchange", default="a2a", choices=["a2a", "p2p"],
                     help="--scaling strong: all_to_all_single (NCCL) or peer stores through symmetric memory")
     ap.add_argument("--bimodal", type=float, default=0.0,
@@ -615,6 +631,8 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
+    if args.scaling is None:
+        args.scaling = "both" if args.gpus > 1 else "weak"
     from paper_2606_20374_b200 import dist as D
     if args.impl == "reference":
         rank = int(os.environ.get("RANK", "0"))

@@ -215,9 +215,11 @@ class PeerPlanes:
 
 
 # ---- bench.py --gpus N --scaling strong -------------------------------------------------------------------
-def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
+def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler, emit=True):
     """ONE job of the named workload over world.size GPUs: every GPU expands and aggregates its own ranks,
-    one exchange, selection per sig slice.  Timed like the single-GPU step: CUDA events, max over ranks."""
+    one exchange, selection per sig slice.  Timed like the single-GPU step: CUDA events, max over ranks.
+    emit=True: rank 0 prints the JSON line; emit=False: rank 0 returns it as a dict (the other ranks None), for
+    bench.py's default N > 1 line, which carries the sharded job beside the weak-scaling headline."""
     import json
     import torch.distributed as dist
     from . import dist as D
@@ -286,13 +288,13 @@ def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
     nv, ni = sh.ctx.stats()
     total = D.sum_over_ranks(world, float(n))
     valid = D.sum_over_ranks(world, float(nv))
+    sh.close()                                       # every rank releases its context, not only the one that prints
     if g != 0:
-        sh.close()                                   # every rank releases its context, not only the one that prints
-        return
+        return None
     peak, peak_src = measured_peak_gbs()
     table_bytes = s.n_ranks * s.n_steps * (64 + 32 * (s.n_phases + 1) + 160 * s.n_sigs)
     step_bytes = 32 * total + table_bytes
-    print(json.dumps({
+    line = {
         "metric": metric, "value": total / (ms_step * 1e-3), "unit": "events/s", "n_gpus": G,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "strong", "vs_baseline": None, "dtype": "int64", "data": "synthetic",
@@ -305,5 +307,7 @@ def bench_strong(args, world, metric, measured_peak_gbs, ClockSampler):
         "hbm_frac_step_aggregate": step_bytes / (ms_step * 1e-3) / 1e9 / (peak * G),
         "roofline": None, "clocks": clocks, "e2e": None,
         "counters": {"n_valid": int(valid), "n_events": int(total)},
-    }))
-    sh.close()
+    }
+    if emit:
+        print(json.dumps(line))
+    return line
